@@ -1,0 +1,374 @@
+"""Seeded synthetic workloads for the viscoelastic FDTD step (numpy only).
+
+This module is the ONLY code shared by the fp64 oracle (``oracle/``) and the CUDA path
+(``paper_2301_12727_b200/csrc``).  It holds none of the method's arithmetic: it builds
+inputs only -- the uint8 material index map, the material table (rho, cL, cS, alphaL,
+alphaS), the source cell list (cell, amplitude, delay), the time step and the sensor
+windows -- for the five configurations of ``BASELINE.json:configs`` as made concrete in
+SURVEY.md section 8(d) and restated in DESIGN.md ("Input recipe").
+
+The paper's own workloads are patient CT/MRI datasets that are not available
+(PAPER.md:L128); these synthetic domains take their shapes, sizes and value ranges
+(three-layer skull 10/80/10; Table 1 property ranges, PAPER.md:L65-L73;
+6-9 PPW grids, L57/L148; focused apertures at F# ~ 1, L35/L146) and stand in for them.
+
+Conventions: node (i, j, k) sits at (x, y, z) = (i, j, k) * dx, the linear cell index is
+``i + nx * (j + ny * k)`` (x fastest, z = acoustic axis); numpy arrays are
+shaped (nz, ny, nx).  RNG: ``numpy.random.Generator(PCG64(230112727 + cfg))``; random
+fields are drawn plane by plane along z (identical stream to one (nz, ny, nx) draw).
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+WATER = (1000.0, 1500.0, 0.0, 0.0, 0.0)
+SEED_BASE = 230112727
+CFL = 0.3
+
+
+@dataclass
+class Workload:
+    """Everything ``bvfdtd_create`` / ``bvfdtd_set_source`` (and the oracle) need."""
+
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    pml: int
+    dx: float
+    dt: float
+    f0: float
+    spp: int                       # time steps per source period (integer by construction)
+    steps: int
+    table: np.ndarray              # (n_mat, 5) float64: rho, cL, cS, alphaL, alphaS (Np/m at f0)
+    index_map: np.ndarray          # (nz, ny, nx) uint8
+    src_cell: np.ndarray           # (n_src,) int64 linear cell indices
+    src_amp: np.ndarray            # (n_src,) float32
+    src_delay: np.ndarray          # (n_src,) float32 seconds
+    waveform: int                  # 0 = burst, 1 = ramped CW
+    f_src: float
+    n_cycles: int
+    peak_begin: int = 0
+    rms_begin: int = -1            # < 0: no rms window (set to `steps`, i.e. empty)
+    sensor_end: int = -1           # < 0: unbounded
+    pml_R: float = 1e-4
+    notes: dict = field(default_factory=dict)
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+    def mean_mask_bits(self) -> float:
+        p = self.pml
+        return 2.0 * p / self.nx + 2.0 * p / self.ny + 2.0 * p / self.nz
+
+    def bytes_per_cell_step(self, rms_on: bool = False) -> float:
+        """Algorithmic bytes per cell-step, B_dense of SURVEY.md 8(d): 49 (S2) + 109 (S3)
+        + 8 (peak) + 8 (sumsq, when on) + 48 per PML mask bit set."""
+        return 49.0 + 109.0 + 8.0 + (8.0 if rms_on else 0.0) + 48.0 * self.mean_mask_bits()
+
+
+def snapped_dt(dx: float, f0: float, c_max: float, cfl: float = CFL):
+    """Reading P6: dt0 = CFL dx / c_max, snapped so that one period is a whole number of
+    steps.  Returns (dt, steps_per_period)."""
+    dt0 = cfl * dx / c_max
+    spp = int(math.ceil(1.0 / (f0 * dt0) - 1e-9))
+    return 1.0 / (f0 * spp), spp
+
+
+def bone_shear_speed(cL):
+    """cS = 0.55 cL where cL >= 1800 m/s, else 0 (chosen)."""
+    cL = np.asarray(cL, dtype=np.float64)
+    return np.where(cL >= 1800.0, 0.55 * cL, 0.0)
+
+
+def _disc_cells(nx, ny, k_s, radius_cells, xc, yc):
+    j, i = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    m = (i - xc) ** 2 + (j - yc) ** 2 <= radius_cells ** 2
+    return (i[m] + nx * (j[m] + ny * k_s)).astype(np.int64), i[m], j[m]
+
+
+# ----------------------------------------------------------------------------------------
+# config 0: water + flat cortical plate, piston burst
+# ----------------------------------------------------------------------------------------
+def config0() -> Workload:
+    nx = ny = nz = 64
+    P = 8
+    dx = 1e-3 / 3.0
+    f0 = 500e3
+    table = np.array([WATER, (1900.0, 2800.0, 1500.0, 200.0, 200.0)], dtype=np.float64)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    idx = np.zeros((nz, ny, nx), dtype=np.uint8)
+    idx[29:35] = 1
+    cells, _, _ = _disc_cells(nx, ny, 12, 10.0, 31.5, 31.5)
+    n = cells.size
+    return Workload("cfg0_plate64", nx, ny, nz, P, dx, dt, f0, spp, 300, table, idx,
+                    cells, np.ones(n, np.float32), np.zeros(n, np.float32),
+                    waveform=0, f_src=f0, n_cycles=3, peak_begin=0, rms_begin=-1)
+
+
+# ----------------------------------------------------------------------------------------
+# config 1: spherical shell with 64 HU-like materials, CW piston
+# ----------------------------------------------------------------------------------------
+def config1(steps: int = 800) -> Workload:
+    nx = ny = nz = 128
+    P = 12
+    dx = 1e-3 / 3.0
+    f0 = 500e3
+    fm = f0 / 1e6
+    t = np.arange(64) / 63.0
+    cL = 1500.0 + 1600.0 * t
+    rows = [WATER] + [
+        (1000.0 + 1100.0 * t[e], cL[e], float(bone_shear_speed(cL[e])), 163.0 * fm * t[e],
+         (329.0 * fm * t[e]) if cL[e] >= 1800.0 else 0.0)
+        for e in range(64)
+    ]
+    table = np.array(rows, dtype=np.float64)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 1))
+    idx = np.zeros((nz, ny, nx), dtype=np.uint8)
+    jj, ii = np.meshgrid(np.arange(ny) - 63.5, np.arange(nx) - 63.5, indexing="ij")
+    for k in range(nz):
+        g = rng.standard_normal((ny, nx))
+        hu = np.clip(1200.0 + 300.0 * g, 200.0, 2200.0)
+        e = np.minimum(63, np.floor((hu - 200.0) * 64.0 / 2000.0)).astype(np.int64)
+        r = np.sqrt(ii ** 2 + jj ** 2 + (k - 63.5) ** 2)
+        shell = (r > 19.0) & (r <= 40.0)
+        idx[k] = np.where(shell, 1 + e, 0).astype(np.uint8)
+    cells, _, _ = _disc_cells(nx, ny, 16, 20.0, 63.5, 63.5)
+    n = cells.size
+    return Workload("cfg1_shell128", nx, ny, nz, P, dx, dt, f0, spp, steps, table, idx,
+                    cells, np.ones(n, np.float32), np.zeros(n, np.float32),
+                    waveform=1, f_src=f0, n_cycles=3, peak_begin=0,
+                    rms_begin=max(0, steps - 3 * spp))
+
+
+# ----------------------------------------------------------------------------------------
+# configs 2-4: layered ellipsoidal skull + brain
+# ----------------------------------------------------------------------------------------
+def _skull_table(n_rows: int, f0: float) -> np.ndarray:
+    """water; brain; nb = n_rows - 2 bone entries indexed by porosity (0 .. 0.5)."""
+    fm = f0 / 1e6
+    nb = n_rows - 2
+    phi = 0.5 * np.arange(nb) / (nb - 1)
+    rho = 1000.0 * phi + 2100.0 * (1.0 - phi)
+    cL = 1500.0 * phi + 3100.0 * (1.0 - phi)
+    cS = bone_shear_speed(cL)
+    rows = [WATER, (1040.0, 1546.0, 0.0, 60.0 * fm, 0.0)]
+    rows += [(rho[e], cL[e], cS[e], 163.0 * fm, 329.0 * fm if cS[e] > 0 else 0.0)
+             for e in range(nb)]
+    return np.array(rows, dtype=np.float64)
+
+
+def _layered_skull_map(nx, ny, nz, dx, zc_mm, outer_mm, thick_mm, nb, rng, thick_sd_mm=0.0):
+    """Material ids: 0 water, 1 brain, 2 + e bone entry e (porosity phi = 0.5 e / (nb-1)).
+
+    Ellipsoid centred (x_c, y_c, zc); outer semi-axes `outer_mm`, inner = outer - T with
+    T = thick_mm (+ clip(G, -3, 3) * thick_sd_mm per voxel when thick_sd_mm > 0, config 4).
+    Depth fraction u = (1 - s_out) / ((1 - s_out) + (s_in - 1)); cortical if u < 0.1 or
+    u >= 0.9 else trabecular (10/80/10).  Porosity: 0.1 U (cortical),
+    0.1 + 0.4 U (trabecular), U = random().  Draw order per z-plane: all G planes first
+    (config 4 only), then all U planes, each as one pass over z.
+    """
+    idx = np.zeros((nz, ny, nx), dtype=np.uint8)
+    xmm = (np.arange(nx) - (nx - 1) / 2.0) * dx * 1e3
+    ymm = (np.arange(ny) - (ny - 1) / 2.0) * dx * 1e3
+    Y, X = np.meshgrid(ymm, xmm, indexing="ij")
+    ax, ay, az = outer_mm
+    gs = None
+    if thick_sd_mm > 0.0:
+        gs = np.empty((nz, ny, nx), dtype=np.float32)  # kept as the float32 cast of the draw
+        for k in range(nz):
+            gs[k] = rng.standard_normal((ny, nx)).astype(np.float32)
+    for k in range(nz):
+        zmm = k * dx * 1e3 - zc_mm
+        U = rng.random((ny, nx))
+        s_out = np.sqrt((X / ax) ** 2 + (Y / ay) ** 2 + (zmm / az) ** 2)
+        if gs is None:
+            T = thick_mm
+        else:
+            T = thick_mm + np.clip(gs[k].astype(np.float64), -3.0, 3.0) * thick_sd_mm
+        s_in = np.sqrt((X / (ax - T)) ** 2 + (Y / (ay - T)) ** 2 + (zmm / (az - T)) ** 2)
+        water = s_out > 1.0
+        brain = s_in <= 1.0
+        skull = ~(water | brain)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            u = (1.0 - s_out) / ((1.0 - s_out) + (s_in - 1.0))
+        cortical = (u < 0.1) | (u >= 0.9)
+        phi = np.where(cortical, 0.1 * U, 0.1 + 0.4 * U)
+        e = np.rint(phi / 0.5 * (nb - 1)).astype(np.int64)
+        plane = np.where(brain, 1, 0)
+        plane = np.where(skull, 2 + e, plane)
+        idx[k] = plane.astype(np.uint8)
+    return idx
+
+
+def _focused_aperture(nx, ny, k_s, dx, radius_mm, focal_mm):
+    """Focused bowl projected on plane k_s (stand-in for the Rayleigh-Sommerfeld step,
+    PAPER.md:L95): amp = F / d, delay = (d_max - d) / 1500 with d the distance to the focus."""
+    xc, yc = (nx - 1) / 2.0, (ny - 1) / 2.0
+    cells, i, j = _disc_cells(nx, ny, k_s, radius_mm * 1e-3 / dx, xc, yc)
+    rho_mm = np.sqrt((i - xc) ** 2 + (j - yc) ** 2) * dx * 1e3
+    d = np.sqrt(rho_mm ** 2 + focal_mm ** 2)
+    d_max = math.sqrt(radius_mm ** 2 + focal_mm ** 2)
+    amp = (focal_mm / d).astype(np.float32)
+    delay = ((d_max - d) * 1e-3 / 1500.0).astype(np.float32)
+    return cells, amp, delay
+
+
+def config2(steps: int = 3000) -> Workload:
+    nx, ny, nz, P = 300, 300, 450, 16
+    dx = 1e-3 / 3.0
+    f0 = 500e3
+    table = _skull_table(128, f0)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    k_s = P + 4
+    zc_mm = k_s * dx * 1e3 + 10.0 + 95.0
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 2))
+    idx = _layered_skull_map(nx, ny, nz, dx, zc_mm, (85.0, 70.0, 95.0), 7.0, 126, rng)
+    cells, amp, delay = _focused_aperture(nx, ny, k_s, dx, 32.0, 60.0)
+    return Workload("cfg2_skull300x300x450", nx, ny, nz, P, dx, dt, f0, spp, steps, table, idx,
+                    cells, amp, delay, waveform=1, f_src=f0, n_cycles=3, peak_begin=0,
+                    rms_begin=max(0, steps - 3 * spp))
+
+
+def config3(steps: int = 5000) -> Workload:
+    nx, ny, nz, P = 504, 504, 672, 20
+    f0 = 700e3
+    dx = 1500.0 / (f0 * 9.0)
+    table = _skull_table(255, f0)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    k_s = P + 4
+    zc_mm = k_s * dx * 1e3 + 10.0 + 95.0
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 3))
+    idx = _layered_skull_map(nx, ny, nz, dx, zc_mm, (85.0, 70.0, 95.0), 7.0, 253, rng)
+    cells, amp, delay = _focused_aperture(nx, ny, k_s, dx, 32.0, 60.0)
+    return Workload("cfg3_skull504x504x672", nx, ny, nz, P, dx, dt, f0, spp, steps, table, idx,
+                    cells, amp, delay, waveform=1, f_src=f0, n_cycles=3, peak_begin=0,
+                    rms_begin=max(0, steps - 3 * spp))
+
+
+def config4(steps: int = 6000) -> Workload:
+    nx, ny, nz, P = 480, 480, 600, 24
+    dx = 0.25e-3
+    f0 = 250e3
+    table = _skull_table(128, f0)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    k_s = P + 4
+    z_cap_mm = k_s * dx * 1e3
+    zc_mm = z_cap_mm + 30.0 + 95.0
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 4))
+    idx = _layered_skull_map(nx, ny, nz, dx, zc_mm, (85.0, 70.0, 95.0), 7.0, 126, rng,
+                             thick_sd_mm=1.0)
+    # 128-element array on a spherical cap (radius of curvature 80 mm, aperture 100 mm),
+    # apex (x_c, y_c, z_cap), concave toward +z; sunflower lattice of element centres.
+    u0 = rng.random()
+    n_el = 128
+    Rc = 80.0
+    th_max = math.asin(50.0 / Rc)
+    m = np.arange(n_el)
+    th = np.arccos(1.0 - (m + 0.5) / n_el * (1.0 - math.cos(th_max)))
+    ph = m * math.pi * (3.0 - math.sqrt(5.0)) + 2.0 * math.pi * u0
+    xc_mm = (nx - 1) / 2.0 * dx * 1e3
+    yc_mm = (ny - 1) / 2.0 * dx * 1e3
+    centre = np.array([xc_mm, yc_mm, z_cap_mm + Rc])          # centre of curvature
+    el = np.stack([centre[0] + Rc * np.sin(th) * np.cos(ph),
+                   centre[1] + Rc * np.sin(th) * np.sin(ph),
+                   centre[2] - Rc * np.cos(th)], axis=1)     # (128, 3) mm
+    target = np.array([xc_mm + 10.0, yc_mm, centre[2]])       # geometric focus + 10 mm in x
+    d_el = np.linalg.norm(el - target, axis=1)
+    jitter = rng.standard_normal(n_el) * (1.0 / f0) / 50.0
+    delay_el = (d_el.max() - d_el) * 1e-3 / 1500.0 + jitter
+    delay_el -= delay_el.min()
+    # voxels of the cap: |dist to centre of curvature - Rc| <= dx/2 and within 3.5 mm of
+    # the nearest element centre.  Only planes the cap can reach are scanned.
+    sag_mm = Rc - math.sqrt(Rc ** 2 - 50.0 ** 2)
+    k_hi = int(math.ceil((z_cap_mm + sag_mm + 4.0) / (dx * 1e3)))
+    xs = np.arange(nx) * dx * 1e3
+    ys = np.arange(ny) * dx * 1e3
+    Y, X = np.meshgrid(ys, xs, indexing="ij")
+    cells_l, delay_l = [], []
+    for k in range(max(P, k_s - 2), min(nz - P, k_hi + 1)):
+        z = k * dx * 1e3
+        dist = np.sqrt((X - centre[0]) ** 2 + (Y - centre[1]) ** 2 + (z - centre[2]) ** 2)
+        on = np.abs(dist - Rc) <= dx * 1e3 / 2.0
+        on &= (np.arange(ny)[:, None] >= P) & (np.arange(ny)[:, None] < ny - P)
+        on &= (np.arange(nx)[None, :] >= P) & (np.arange(nx)[None, :] < nx - P)
+        if not on.any():
+            continue
+        jj, ii = np.nonzero(on)
+        pts = np.stack([xs[ii], ys[jj], np.full(ii.size, z)], axis=1)
+        d2 = ((pts[:, None, :] - el[None, :, :]) ** 2).sum(axis=2)
+        near = d2.argmin(axis=1)
+        ok = d2[np.arange(ii.size), near] <= 3.5 ** 2
+        cells_l.append((ii[ok] + nx * (jj[ok] + ny * k)).astype(np.int64))
+        delay_l.append(delay_el[near[ok]])
+    cells = np.concatenate(cells_l)
+    delay = np.concatenate(delay_l).astype(np.float32)
+    order = np.argsort(cells, kind="stable")
+    cells, delay = cells[order], delay[order]
+    return Workload("cfg4_array480x480x600", nx, ny, nz, P, dx, dt, f0, spp, steps, table, idx,
+                    cells, np.ones(cells.size, np.float32), delay, waveform=1, f_src=f0,
+                    n_cycles=3, peak_begin=0, rms_begin=-1)
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+
+
+def make(cfg: int, **kw) -> Workload:
+    return CONFIGS[cfg](**kw)
+
+
+# ----------------------------------------------------------------------------------------
+# small seeded domains for unit / edge-case parity tests
+# ----------------------------------------------------------------------------------------
+def random_domain(nx, ny, nz, pml, seed, n_mat=6, solid_fraction=0.5, lossy=True,
+                  f0=500e3, dx=1e-3 / 3.0, steps=20, waveform=0) -> Workload:
+    """A small heterogeneous fluid + solid block map for kernel-level parity tests.
+
+    Blocks of 3x3x3 voxels get a random material so that every averaging case (fluid-fluid,
+    fluid-solid, solid-solid, lossy/lossless) appears next to every kind of node."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 1000 + seed))
+    rows = [WATER]
+    for m in range(1, n_mat):
+        solid = rng.random() < solid_fraction
+        rho = 1000.0 + 1100.0 * rng.random()
+        cL = 1500.0 + 1600.0 * rng.random()
+        cS = (0.45 + 0.1 * rng.random()) * cL if solid else 0.0
+        aL = 200.0 * rng.random() if lossy else 0.0
+        aS = 300.0 * rng.random() if (lossy and solid) else 0.0
+        rows.append((rho, cL, cS, aL, aS))
+    table = np.array(rows, dtype=np.float64)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    bz, by, bx = (nz + 2) // 3, (ny + 2) // 3, (nx + 2) // 3
+    blocks = rng.integers(0, n_mat, size=(bz, by, bx), dtype=np.int64)
+    idx = np.repeat(np.repeat(np.repeat(blocks, 3, 0), 3, 1), 3, 2)[:nz, :ny, :nx]
+    idx = np.ascontiguousarray(idx).astype(np.uint8)
+    # sources: a few cells in the interior (outside the PML mask)
+    lo = pml
+    ci = rng.integers(lo, nx - lo, size=5)
+    cj = rng.integers(lo, ny - lo, size=5)
+    ck = rng.integers(lo, nz - lo, size=5)
+    cells = np.unique((ci + nx * (cj + ny * ck)).astype(np.int64))
+    amp = (0.5 + rng.random(cells.size)).astype(np.float32)
+    delay = (rng.random(cells.size) * 2.0 / f0 * 0.25).astype(np.float32)
+    return Workload(f"rand_{nx}x{ny}x{nz}_p{pml}_s{seed}", nx, ny, nz, pml, dx, dt, f0, spp,
+                    steps, table, idx, cells, amp, delay, waveform=waveform, f_src=f0,
+                    n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
+
+
+def random_state(w: Workload, seed: int, scale_v: float = 1e-6) -> dict:
+    """Seeded random state for single-pass parity tests: 3 v, 6 sigma, 6 r as float32 arrays
+    shaped (nz, ny, nx) (values exactly representable in fp32 so both sides start equal)."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 2000 + seed))
+    out = {}
+    for name in ("vx", "vy", "vz"):
+        out[name] = (scale_v * rng.standard_normal((w.nz, w.ny, w.nx))).astype(np.float32)
+    for name in ("sxx", "syy", "szz", "sxy", "sxz", "syz"):
+        out[name] = rng.standard_normal((w.nz, w.ny, w.nx)).astype(np.float32)
+    for name in ("rxx", "ryy", "rzz", "rxy", "rxz", "ryz"):
+        out[name] = (1e5 * rng.standard_normal((w.nz, w.ny, w.nx))).astype(np.float32)
+    return out
