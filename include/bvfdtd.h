@@ -1,0 +1,214 @@
+/*
+ * bvfdtd.h -- C ABI of the B200-native 3-D staggered-grid viscoelastic FDTD time step.
+ *
+ * What the library computes: the time iteration that arXiv 2301.12727 ("BabelBrain") runs through
+ * its BabelViscoFDTD solver (PAPER.md = /root/reference/PAPER.md):
+ *   - PAPER.md:L91 (Eq. 1)   velocity-stress viscoelastic system, rows 1-3 velocity, 4-9 stress;
+ *   - PAPER.md:L93           "4th-order in space and 2nd-order in time ... staggered-grid";
+ *   - PAPER.md:L148-L152     attenuation as a quality factor Q (Eq. 3) realised with relaxation
+ *                            constants and memory variables;
+ *   - PAPER.md:L95           the incident field enters "as a stress source perpendicular to the
+ *                            acoustic axis";
+ *   - PAPER.md:L65-L73       material rows (rho, cL, cS, alphaL, alphaS), Table 1;
+ *   - PAPER.md:L107-L110, L158, L220-L229   outputs are pressure / peak / pulse-average maps.
+ * Every discrete detail the paper defers to its reference [23] (L93) is fixed by the readings
+ * P1-P9 in DESIGN.md; each call below names the readings it implements.
+ *
+ * Conventions
+ *   - Grid nx x ny x nz INCLUDING the PML cells; cell (i,j,k) has linear index i + nx*(j + ny*k)
+ *     (x fastest; z is the acoustic axis).  All grid arrays that cross this ABI are
+ *     dense in that order, whatever the private device layout is.
+ *   - SI units.  fp32 state and arithmetic on the device; coefficients are derived in fp64 on the
+ *     host and rounded to fp32 once (reading P9).
+ *   - "host" / "device" is stated for every pointer.  The caller owns every pointer it passes; the
+ *     library copies host inputs during the call and never frees caller memory.
+ *   - Every call returns 0 (BVFDTD_OK) or a negative bvfdtd_status; no exceptions, no aborts.
+ *     A failed bvfdtd_create leaves *out = NULL.
+ *   - One context = one CUDA stream = one simulation.  A context is not thread-safe; distinct
+ *     contexts are independent.
+ *   - There is no CPU fallback: every call that touches the device returns BVFDTD_ECUDA when no
+ *     CUDA device / driver is present.
+ */
+#ifndef BVFDTD_H
+#define BVFDTD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bvfdtd_ctx bvfdtd_ctx; /* opaque */
+
+typedef enum {
+    BVFDTD_OK = 0,
+    BVFDTD_EINVAL = -1,     /* an argument violates a documented rule */
+    BVFDTD_ENOMEM = -2,     /* the caller's device workspace is too small (or host malloc failed) */
+    BVFDTD_ESTABILITY = -3, /* max unrelaxed speed * dt / dx > 0.494 (reading P6) */
+    BVFDTD_ECUDA = -4,      /* a CUDA runtime / driver call failed (bvfdtd_last_cuda_error) */
+    BVFDTD_ESTATE = -5      /* call not legal in the context's current state */
+} bvfdtd_status;
+
+/* Grid descriptor.  Dimensions INCLUDE the pml cells on every face. */
+typedef struct {
+    int32_t nx, ny, nz; /* each must be >= 2*pml + 8 */
+    int32_t pml;        /* C-PML thickness in cells on all six faces, >= 0 (0 = rigid box, P4) */
+} bvfdtd_grid;
+
+/* One row of the material table = the columns of PAPER.md Table 1 (L65-L73).  alpha in Np/m AT
+ * THE CENTRE FREQUENCY f0: the caller has already applied the frequency scaling and the paper's
+ * Q correction factor q_c (alpha / q_c).  cS = 0 marks a fluid. */
+typedef struct {
+    double rho;    /* kg/m^3, > 0 */
+    double cL;     /* m/s, > 0: longitudinal phase speed at f0 */
+    double cS;     /* m/s, >= 0 and < (sqrt(3)/2) cL: shear phase speed at f0 */
+    double alphaL; /* Np/m at f0, >= 0, alphaL*cL/(2 pi f0) < tan(pi/8) (Q > 1, reading P3) */
+    double alphaS; /* Np/m at f0, >= 0, same bound with cS */
+} bvfdtd_material;
+
+enum { /* bvfdtd_opts.flags */
+    BVFDTD_FLAG_REFERENCE_KERNELS = 1 /* debug: run the one-thread-per-cell kernels instead of
+                                         the tiled TMA kernels (same arithmetic, same results up
+                                         to fp32 rounding order) */
+};
+
+typedef struct {
+    double f0;          /* Hz > 0: relaxation centre frequency, tau_sigma = 1/(2 pi f0) (P3), also
+                           the frequency of the C-PML frequency shift (P5) */
+    double pml_R;       /* theoretical PML reflection coefficient in (0,1); 0 selects 1e-4 (P5) */
+    int64_t peak_begin; /* first step index n sampled into the running peak (P8) */
+    int64_t rms_begin;  /* first step index n sampled into the sum of squares (P8) */
+    int64_t sensor_end; /* one past the last sampled step for both windows; < 0 = unbounded */
+    uint32_t flags;     /* BVFDTD_FLAG_* */
+    uint32_t reserved;  /* must be 0 */
+} bvfdtd_opts;
+
+/* Field ids for bvfdtd_read_fields / bvfdtd_write_fields. */
+enum {
+    BVFDTD_F_VX = 0, BVFDTD_F_VY = 1, BVFDTD_F_VZ = 2,          /* particle velocity, fp32      */
+    BVFDTD_F_SXX = 3, BVFDTD_F_SYY = 4, BVFDTD_F_SZZ = 5,       /* normal stresses, fp32        */
+    BVFDTD_F_SXY = 6, BVFDTD_F_SXZ = 7, BVFDTD_F_SYZ = 8,       /* shear stresses, fp32         */
+    BVFDTD_F_RXX = 9, BVFDTD_F_RYY = 10, BVFDTD_F_RZZ = 11,     /* memory variables, fp32       */
+    BVFDTD_F_RXY = 12, BVFDTD_F_RXZ = 13, BVFDTD_F_RYZ = 14,
+    BVFDTD_F_PRESSURE = 15,  /* p = -(sxx+syy+szz)/3, fp32, computed on read (reading P8)       */
+    BVFDTD_F_MATERIAL = 16,  /* the uint8 index map, round trip (nx*ny*nz bytes)                */
+    BVFDTD_F_PML_MASK = 17,  /* uint8: bit0 x-slab, bit1 y-slab, bit2 z-slab (reading P5)       */
+    BVFDTD_F_DERIVED = 18,   /* n_materials x 8 fp32: rho, pi_R, mu_R, tau_p, tau_s, pi_U, mu_U,
+                                c_U (reading P3); host destination only                         */
+    BVFDTD_F_PML_PROFILES = 19, /* fp32, host destination only: for axis x then y then z, the four
+                                arrays a_int, b_int, a_half, b_half, each of that axis' length:
+                                4*(nx+ny+nz) floats (reading P5)                                */
+    BVFDTD_F_SUMSQ = 20      /* running sum of p^2 over the rms window, fp32                    */
+};
+
+/* Bytes of caller-owned DEVICE workspace bvfdtd_create needs for this grid: 15 state arrays, the
+ * peak and sum-of-squares maps, the index map, the slab-compact C-PML memory variables and the
+ * coefficient tables, in the library's private padded layout.  Host-only computation. */
+int bvfdtd_workspace_bytes(const bvfdtd_grid *grid, size_t *out_bytes);
+
+/*
+ * Create a simulation (step S0 of DESIGN.md: per-material constants, C-PML profiles and mask are
+ * derived in fp64 and rounded to fp32 once; readings P2, P3, P5, P6).
+ *   out            host; receives the context (NULL on failure)
+ *   grid, dx, dt   grid descriptor, grid step (m), time step (s); the library does not choose dt
+ *   table          host, n_materials rows, 1 <= n_materials <= 256
+ *   index_map      host, nx*ny*nz uint8, each < n_materials
+ *   opts           host
+ *   d_workspace    DEVICE, caller-owned, >= bvfdtd_workspace_bytes(), 256-byte aligned; must
+ *                  outlive the context.  The library zeroes all state in it (reading P9).
+ *   cuda_stream    a cudaStream_t (NULL = the legacy default stream); all work of this context is
+ *                  enqueued on it
+ * Errors: EINVAL for any violated rule above / in the struct comments (dim < 2*pml + 8, index >=
+ * n_materials, cS >= sqrt(3)/2 cL, Q <= 1, ...); ESTABILITY when max c_U*dt/dx > 0.494; ENOMEM
+ * when workspace_bytes is too small; ECUDA.
+ */
+int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double dt,
+                  const bvfdtd_material *table, int32_t n_materials, const uint8_t *index_map,
+                  const bvfdtd_opts *opts, void *d_workspace, size_t workspace_bytes,
+                  void *cuda_stream);
+
+/*
+ * Additive isotropic stress source (step S1; reading P7): at step n (t_n = n*dt), for
+ * every source cell s:  sxx, syy, szz -= amp[s] * w(t_n - delay_s[s]), injected before the
+ * velocity update.  w: waveform 0 = burst  sin(2 pi f t) for 0 <= t < n_cycles/f, else 0;
+ * waveform 1 = ramped CW  ramp(t) sin(2 pi f t), ramp = (1 - cos(pi t f / n_cycles))/2 for
+ * t < n_cycles/f, 1 after; w = 0 for t < 0.
+ *   cell, amp, delay_s   host arrays of n_src entries; cells are linear indices, unique, inside
+ *                        the grid and outside the PML mask.  n_src = 0 removes the source.
+ * The library keeps its own device copy (the only device memory it allocates itself).
+ * Errors: EINVAL (cell outside the grid / inside the PML / duplicate, f_src <= 0, n_cycles < 1,
+ * waveform not 0/1), ECUDA.
+ */
+int bvfdtd_set_source(bvfdtd_ctx *ctx, int64_t n_src, const int64_t *cell, const float *amp,
+                      const float *delay_s, int32_t waveform, double f_src, int32_t n_cycles);
+
+/*
+ * Enqueue n full time steps on the context's stream, asynchronously: per step S1 inject -> S2
+ * velocity update (Eq. 1 rows 1-3) -> S3 stress + memory-variable update (Eq. 1 rows 4-9, L148-L152)
+ * with the S4 sensor (running peak of |p|, sum of p^2) fused into it.  No host<->device traffic.
+ * Legal before bvfdtd_set_source (zero source).  n >= 0.
+ */
+int bvfdtd_step(bvfdtd_ctx *ctx, int64_t n);
+
+/* Number of steps enqueued so far (the index n of the next step). */
+int64_t bvfdtd_step_index(const bvfdtd_ctx *ctx);
+
+/*
+ * Copy one field out in the dense external layout.  dst_bytes must equal the field's size
+ * (nx*ny*nz*4 for fp32 grid fields, nx*ny*nz for the uint8 fields, see the enum).  If
+ * dst_is_device == 0, dst is host memory and the call synchronises the stream; otherwise dst is
+ * device memory and the copy is enqueued on the stream.
+ */
+int bvfdtd_read_fields(bvfdtd_ctx *ctx, uint32_t field_id, void *dst, size_t dst_bytes,
+                       int32_t dst_is_device);
+
+/* Overwrite one of the 15 state fields (ids 0..14) from a dense fp32 array (restart, unit tests).
+ * The outermost normal-velocity layer (reading P4) is forced to 0 whatever src holds. */
+int bvfdtd_write_fields(bvfdtd_ctx *ctx, uint32_t field_id, const void *src, size_t src_bytes,
+                        int32_t src_is_device);
+
+/*
+ * Sensor outputs (step S4; reading P8), dense fp32 nx*ny*nz each, either pointer may be NULL:
+ *   peak     max |p| over steps n with peak_begin <= n < sensor_end
+ *   rms_amp  sqrt(2 * sum p^2 / count) over steps n with rms_begin <= n < sensor_end (the amplitude
+ *            of a sinusoid in steady state); 0 when count = 0
+ */
+int bvfdtd_read_peak_pressure(bvfdtd_ctx *ctx, float *peak, float *rms_amp, int32_t dst_is_device);
+
+/* Release the context (host structs, the source copy, CUDA graphs).  Never touches the workspace. */
+int bvfdtd_destroy(bvfdtd_ctx *ctx);
+
+const char *bvfdtd_strerror(int code);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char *bvfdtd_last_cuda_error(void);
+
+/* Device-time accounting for benchmarks: when enabled the library brackets every kernel of
+ * bvfdtd_step with CUDA events on the context's stream; bvfdtd_kernel_times (which synchronises)
+ * returns the accumulated milliseconds and launch counts per kernel (0 inject, 1 velocity,
+ * 2 stress+sensor) since the last call and resets them.  At most `BVFDTD_MAX_TIMED_STEPS` steps
+ * are recorded between two reads. */
+enum { BVFDTD_MAX_TIMED_STEPS = 4096 };
+int bvfdtd_enable_kernel_timing(bvfdtd_ctx *ctx, int32_t on);
+int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[3], int64_t launches[3]);
+
+/* ---- host-only helpers (no CUDA device needed): the S0 constructions, exposed so that the
+ * construction-parity tests can run anywhere.  Same code path bvfdtd_create uses. ---- */
+
+/* Per-material derived constants (reading P3): out[8*m + 0..7] = rho, pi_R, mu_R, tau_p, tau_s,
+ * pi_U, mu_U, c_U rounded to fp32.  Returns EINVAL on an invalid row. */
+int bvfdtd_derive_materials(const bvfdtd_material *table, int32_t n_materials, double f0,
+                            float *out);
+/* C-PML profiles of one axis of n nodes (reading P5), each output of length n. */
+int bvfdtd_pml_profiles(int32_t n, int32_t pml, double dx, double dt, double f0, double pml_R,
+                        double c_ref, float *a_int, float *b_int, float *a_half, float *b_half);
+/* PML mask (reading P5), nx*ny*nz uint8. */
+int bvfdtd_pml_mask(const bvfdtd_grid *grid, uint8_t *mask);
+/* Largest unrelaxed Courant number c_U*dt/dx of the table (reading P6), or a negative status. */
+double bvfdtd_max_courant(const bvfdtd_material *table, int32_t n_materials, double f0, double dt,
+                          double dx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BVFDTD_H */

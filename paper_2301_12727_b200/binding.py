@@ -1,0 +1,294 @@
+"""Thin ctypes binding of ``include/bvfdtd.h`` -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; this module never computes
+fields.  PyTorch is used for device memory (the caller-owned workspace) and the CUDA stream only.
+There is no CPU fallback: if ``libbvfdtd.so`` is missing or no CUDA device is present, the calls
+raise.  Names mirror the C entry points (``bvfdtd_create`` -> ``Simulation.__init__``,
+``bvfdtd_set_source`` -> ``set_source``, ``bvfdtd_step`` -> ``step``, ``bvfdtd_read_fields`` ->
+``read_fields``, ``bvfdtd_read_peak_pressure`` -> ``read_peak_pressure``).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbvfdtd.so")
+
+FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "sxy", "sxz", "syz",
+          "rxx", "ryy", "rzz", "rxy", "rxz", "ryz")
+FIELD_ID = {n: i for i, n in enumerate(FIELDS)}
+FIELD_ID.update(p=15, material=16, pml_mask=17, derived=18, pml_profiles=19, sumsq=20)
+FLAG_REFERENCE_KERNELS = 1
+
+OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
+
+# every symbol include/bvfdtd.h declares (tests check that the library exports all of them)
+SYMBOLS = (
+    "bvfdtd_workspace_bytes", "bvfdtd_create", "bvfdtd_set_source", "bvfdtd_step",
+    "bvfdtd_step_index", "bvfdtd_read_fields", "bvfdtd_write_fields",
+    "bvfdtd_read_peak_pressure", "bvfdtd_destroy", "bvfdtd_strerror", "bvfdtd_last_cuda_error",
+    "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
+    "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
+)
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("pml", C.c_int32)]
+
+
+class Material(C.Structure):
+    _fields_ = [("rho", C.c_double), ("cL", C.c_double), ("cS", C.c_double),
+                ("alphaL", C.c_double), ("alphaS", C.c_double)]
+
+
+class Opts(C.Structure):
+    _fields_ = [("f0", C.c_double), ("pml_R", C.c_double), ("peak_begin", C.c_int64),
+                ("rms_begin", C.c_int64), ("sensor_end", C.c_int64), ("flags", C.c_uint32),
+                ("reserved", C.c_uint32)]
+
+
+class BvfdtdError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib().bvfdtd_strerror(code).decode()
+        if code == ECUDA:
+            msg += ": " + lib().bvfdtd_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({code})")
+
+
+_lib = None
+
+
+def lib():
+    """Load the C-ABI library (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2301_12727_b200.build`"
+                              " (there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, u32, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_double
+        fp = C.POINTER(C.c_float)
+        L.bvfdtd_workspace_bytes.argtypes = [C.POINTER(Grid), C.POINTER(C.c_size_t)]
+        L.bvfdtd_create.argtypes = [C.POINTER(vp), C.POINTER(Grid), dbl, dbl, C.POINTER(Material),
+                                    i32, vp, C.POINTER(Opts), vp, C.c_size_t, vp]
+        L.bvfdtd_set_source.argtypes = [vp, i64, vp, vp, vp, i32, dbl, i32]
+        L.bvfdtd_step.argtypes = [vp, i64]
+        L.bvfdtd_step_index.argtypes = [vp]
+        L.bvfdtd_step_index.restype = i64
+        L.bvfdtd_read_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
+        L.bvfdtd_write_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
+        L.bvfdtd_read_peak_pressure.argtypes = [vp, vp, vp, i32]
+        L.bvfdtd_destroy.argtypes = [vp]
+        L.bvfdtd_strerror.argtypes = [C.c_int]
+        L.bvfdtd_strerror.restype = C.c_char_p
+        L.bvfdtd_last_cuda_error.restype = C.c_char_p
+        L.bvfdtd_enable_kernel_timing.argtypes = [vp, i32]
+        L.bvfdtd_kernel_times.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+        L.bvfdtd_derive_materials.argtypes = [C.POINTER(Material), i32, dbl, fp]
+        L.bvfdtd_pml_profiles.argtypes = [i32, i32, dbl, dbl, dbl, dbl, dbl, fp, fp, fp, fp]
+        L.bvfdtd_pml_mask.argtypes = [C.POINTER(Grid), vp]
+        L.bvfdtd_max_courant.argtypes = [C.POINTER(Material), i32, dbl, dbl, dbl]
+        L.bvfdtd_max_courant.restype = dbl
+        _lib = L
+    return _lib
+
+
+def _check(code, where):
+    if code != OK:
+        raise BvfdtdError(code, where)
+
+
+def _materials(table):
+    t = np.ascontiguousarray(table, dtype=np.float64).reshape(-1, 5)
+    arr = (Material * t.shape[0])()
+    C.memmove(arr, t.ctypes.data, t.nbytes)
+    return arr, t.shape[0]
+
+
+def _fp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+# ---- host-only helpers (no GPU needed) -----------------------------------------------------
+
+def workspace_bytes(nx, ny, nz, pml):
+    g = Grid(nx, ny, nz, pml)
+    out = C.c_size_t(0)
+    _check(lib().bvfdtd_workspace_bytes(C.byref(g), C.byref(out)), "bvfdtd_workspace_bytes")
+    return out.value
+
+
+def derive_materials(table, f0):
+    arr, n = _materials(table)
+    out = np.zeros((n, 8), dtype=np.float32)
+    _check(lib().bvfdtd_derive_materials(arr, n, float(f0), _fp(out)), "bvfdtd_derive_materials")
+    return out
+
+
+def pml_profiles(n, pml, dx, dt, f0, pml_R, c_ref):
+    arrs = [np.zeros(n, dtype=np.float32) for _ in range(4)]
+    _check(lib().bvfdtd_pml_profiles(n, pml, dx, dt, f0, pml_R, c_ref, *[_fp(a) for a in arrs]),
+           "bvfdtd_pml_profiles")
+    return arrs
+
+
+def pml_mask(nx, ny, nz, pml):
+    g = Grid(nx, ny, nz, pml)
+    m = np.zeros((nz, ny, nx), dtype=np.uint8)
+    _check(lib().bvfdtd_pml_mask(C.byref(g), m.ctypes.data), "bvfdtd_pml_mask")
+    return m
+
+
+def max_courant(table, f0, dt, dx):
+    arr, n = _materials(table)
+    v = lib().bvfdtd_max_courant(arr, n, float(f0), float(dt), float(dx))
+    if v < 0:
+        raise BvfdtdError(int(v), "bvfdtd_max_courant")
+    return v
+
+
+# ---- the simulation -----------------------------------------------------------------------
+
+class Simulation:
+    """``bvfdtd_create`` .. ``bvfdtd_destroy`` around a torch-owned device workspace."""
+
+    def __init__(self, nx, ny, nz, pml, dx, dt, table, index_map, f0, pml_R=1e-4, peak_begin=0,
+                 rms_begin=None, sensor_end=-1, flags=0, device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("bvfdtd needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.nx, self.ny, self.nz, self.pml = int(nx), int(ny), int(nz), int(pml)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.cells = self.nx * self.ny * self.nz
+        self.device = torch.device(device)
+        idx = np.ascontiguousarray(index_map, dtype=np.uint8)
+        if idx.size != self.cells:
+            raise ValueError("index_map size does not match the grid")
+        if rms_begin is None or rms_begin < 0:
+            rms_begin = np.iinfo(np.int64).max
+        g = Grid(self.nx, self.ny, self.nz, self.pml)
+        nbytes = C.c_size_t(0)
+        _check(lib().bvfdtd_workspace_bytes(C.byref(g), C.byref(nbytes)), "bvfdtd_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        arr, n = _materials(table)
+        self.n_materials = n
+        o = Opts(float(f0), float(pml_R), int(peak_begin), int(rms_begin), int(sensor_end),
+                 int(flags), 0)
+        h = C.c_void_p(None)
+        with torch.cuda.device(self.device):
+            rc = lib().bvfdtd_create(C.byref(h), C.byref(g), float(dx), float(dt), arr, n,
+                                     idx.ctypes.data, C.byref(o), self.workspace.data_ptr(),
+                                     nbytes.value, self._stream.cuda_stream)
+        _check(rc, "bvfdtd_create")
+        self._h = h
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        sim = cls(w.nx, w.ny, w.nz, w.pml, w.dx, w.dt, w.table, w.index_map, w.f0, w.pml_R,
+                  w.peak_begin, w.rms_begin, w.sensor_end, **kw)
+        sim.set_source(w.src_cell, w.src_amp, w.src_delay, w.waveform, w.f_src, w.n_cycles)
+        return sim
+
+    def close(self):
+        h = getattr(self, "_h", None)
+        if h:
+            lib().bvfdtd_destroy(h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_source(self, cell, amp, delay, waveform, f_src, n_cycles):
+        cell = np.ascontiguousarray(cell, dtype=np.int64)
+        amp = np.ascontiguousarray(amp, dtype=np.float32)
+        delay = np.ascontiguousarray(delay, dtype=np.float32)
+        if not (cell.size == amp.size == delay.size):
+            raise ValueError("source arrays differ in length")
+        _check(lib().bvfdtd_set_source(self._h, cell.size, cell.ctypes.data, amp.ctypes.data,
+                                       delay.ctypes.data, int(waveform), float(f_src),
+                                       int(n_cycles)), "bvfdtd_set_source")
+
+    def step(self, n=1):
+        _check(lib().bvfdtd_step(self._h, int(n)), "bvfdtd_step")
+
+    @property
+    def step_index(self):
+        return lib().bvfdtd_step_index(self._h)
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    # -- readback -------------------------------------------------------------------------
+    def read_fields(self, name, out=None):
+        """Host numpy copy of one field, shaped (nz, ny, nx) for grid fields.  ``out`` may be a
+        preallocated (pinned) numpy array of the right size."""
+        fid = FIELD_ID[name]
+        if name == "derived":
+            a = np.zeros((self.n_materials, 8), dtype=np.float32)
+        elif name == "pml_profiles":
+            a = np.zeros(4 * (self.nx + self.ny + self.nz), dtype=np.float32)
+        elif name in ("material", "pml_mask"):
+            a = np.zeros(self.shape, dtype=np.uint8)
+        else:
+            a = np.zeros(self.shape, dtype=np.float32) if out is None else out
+        _check(lib().bvfdtd_read_fields(self._h, fid, a.ctypes.data, a.nbytes, 0),
+               "bvfdtd_read_fields")
+        return a
+
+    def read_fields_device(self, name):
+        """Dense torch tensor on the device (enqueued on the context's stream)."""
+        torch = self._torch
+        fid = FIELD_ID[name]
+        dt = torch.uint8 if name in ("material", "pml_mask") else torch.float32
+        t = torch.empty(self.shape, dtype=dt, device=self.device)
+        _check(lib().bvfdtd_read_fields(self._h, fid, t.data_ptr(), t.numel() * t.element_size(),
+                                        1), "bvfdtd_read_fields")
+        return t
+
+    def write_fields(self, name, arr):
+        a = np.ascontiguousarray(arr, dtype=np.float32)
+        if a.size != self.cells:
+            raise ValueError("field size does not match the grid")
+        _check(lib().bvfdtd_write_fields(self._h, FIELD_ID[name], a.ctypes.data, a.nbytes, 0),
+               "bvfdtd_write_fields")
+
+    def read_peak_pressure(self, peak=True, rms=True, out_peak=None, out_rms=None):
+        """(peak, rms_amp) as host numpy arrays (None for the one not requested)."""
+        p = (np.zeros(self.shape, dtype=np.float32) if out_peak is None else out_peak) if peak else None
+        r = (np.zeros(self.shape, dtype=np.float32) if out_rms is None else out_rms) if rms else None
+        _check(lib().bvfdtd_read_peak_pressure(self._h, p.ctypes.data if peak else None,
+                                               r.ctypes.data if rms else None, 0),
+               "bvfdtd_read_peak_pressure")
+        return p, r
+
+    def read_peak_pressure_device(self):
+        torch = self._torch
+        p = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        r = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        _check(lib().bvfdtd_read_peak_pressure(self._h, p.data_ptr(), r.data_ptr(), 1),
+               "bvfdtd_read_peak_pressure")
+        return p, r
+
+    # -- device-time accounting (bench) ---------------------------------------------------
+    def enable_kernel_timing(self, on=True):
+        _check(lib().bvfdtd_enable_kernel_timing(self._h, 1 if on else 0),
+               "bvfdtd_enable_kernel_timing")
+
+    def kernel_times(self):
+        ms = (C.c_double * 3)()
+        n = (C.c_int64 * 3)()
+        _check(lib().bvfdtd_kernel_times(self._h, ms, n), "bvfdtd_kernel_times")
+        names = ("inject", "velocity", "stress_sensor")
+        return {k: {"ms": ms[i], "launches": n[i]} for i, k in enumerate(names)}

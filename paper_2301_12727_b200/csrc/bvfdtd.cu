@@ -1,0 +1,548 @@
+// bvfdtd.cu -- the C ABI of include/bvfdtd.h: context, private layout, uploads, launches, readback.
+// All arithmetic of the hot path runs in the kernels (kernels_ref.cuh, kernels_tiled.cuh); the
+// host side only derives the S0 tables (host_tables.cpp) and enqueues work.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/bvfdtd.h"
+#include "device_params.hpp"
+#include "kernels_ref.cuh"
+#include "kernels_tiled.cuh"
+
+using namespace bvfdtd;
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+int cuda_fail(cudaError_t e, const char *what) {
+    std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return BVFDTD_ECUDA;
+}
+#define CU(call)                                              \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
+
+bool grid_ok(const bvfdtd_grid *g) {
+    if (!g || g->pml < 0) return false;
+    const long long lim = 2LL * g->pml + 8;
+    if (g->nx < lim || g->ny < lim || g->nz < lim) return false;
+    if ((long long)g->nx * g->ny * g->nz > (1LL << 40)) return false;
+    return g->nx <= 65535 * 16 && g->ny <= 65535 && g->nz <= 65535;
+}
+
+Layout make_layout(const bvfdtd_grid &g) {
+    Layout L;
+    L.nx = g.nx; L.ny = g.ny; L.nz = g.nz; L.P = g.pml;
+    L.px = (int)round_up(g.nx + 2, 32);
+    L.py = g.ny + 2;
+    L.sz = (long long)L.px * L.py;
+    L.org = 2 * L.sz + 2 * L.px + 32;
+    L.field_floats = round_up(L.org + L.sz * (g.nz + 2) + 2 * L.px + 32, 64);
+    L.mat_bytes = round_up(L.sz * (g.nz + 1), 256);
+    L.wx = (int)round_up(2 * g.pml, 4);
+    L.psi_floats[0] = round_up((long long)L.wx * g.ny * g.nz, 64);
+    L.psi_floats[1] = round_up((long long)L.px * (2 * g.pml) * g.nz, 64);
+    L.psi_floats[2] = round_up((long long)L.px * g.ny * (2 * g.pml), 64);
+    if (g.pml == 0) L.psi_floats[0] = L.psi_floats[1] = L.psi_floats[2] = 64;
+    return L;
+}
+
+// Offsets (bytes) of every region of the caller's workspace.
+struct WsMap {
+    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, total;
+};
+
+WsMap make_wsmap(const Layout &L) {
+    WsMap w;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+    for (int q = 0; q < NSTATE; ++q) w.field[q] = take(L.field_floats * 4);
+    w.peak = take(L.field_floats * 4);
+    w.sumsq = take(L.field_floats * 4);
+    w.scratch = take((size_t)L.nx * L.ny * L.nz * 4);
+    w.mat = take(L.mat_bytes);
+    for (int a = 0; a < 3; ++a)
+        for (int t = 0; t < 6; ++t) w.psi[a * 6 + t] = take(L.psi_floats[a] * 4);
+    w.rows = take(256 * sizeof(KRow));
+    w.prof = take((size_t)4 * (L.nx + L.ny + L.nz) * 4);
+    w.total = off;
+    return w;
+}
+
+}  // namespace
+
+struct bvfdtd_ctx {
+    Layout L;
+    WsMap W;
+    char *ws = nullptr;
+    cudaStream_t stream = nullptr;
+    double dx = 0, dt = 0;
+    bvfdtd_opts opts{};
+    int n_materials = 0;
+    std::vector<Derived> derived;
+    PmlAxis pml[3];
+    Params prm{};
+    int64_t step = 0;
+    int64_t rms_count = 0;
+    // source
+    int64_t n_src = 0;
+    long long *d_cell = nullptr;
+    float *d_amp = nullptr, *d_delay = nullptr;
+    int waveform = 0, n_cycles = 1;
+    double f_src = 0;
+    // tiled-kernel plan (tensor maps etc.)
+    TiledPlan plan;
+    // kernel timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;
+    int64_t timed_steps = 0;
+};
+
+namespace {
+
+__global__ void k_unpack(float *__restrict__ dst, const float *__restrict__ src, Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = src[p.org + i + (long long)p.px * j + p.sz * k];
+}
+__global__ void k_pack(float *__restrict__ dst, const float *__restrict__ src, Params p, int hold_axis) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    float v = src[i + (long long)p.nx * (j + (long long)p.ny * k)];
+    if ((hold_axis == 0 && i == p.nx - 1) || (hold_axis == 1 && j == p.ny - 1) || (hold_axis == 2 && k == p.nz - 1)) v = 0.0f;
+    dst[p.org + i + (long long)p.px * j + p.sz * k] = v;
+}
+__global__ void k_pressure(float *__restrict__ dst, Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    const long long c = p.org + i + (long long)p.px * j + p.sz * k;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = (p.f[SXX][c] + p.f[SYY][c] + p.f[SZZ][c]) * (-1.0f / 3.0f);
+}
+__global__ void k_rms_amp(float *__restrict__ dst, Params p, float two_over_count) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    const long long c = p.org + i + (long long)p.px * j + p.sz * k;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = sqrtf(p.sumsq[c] * two_over_count);
+}
+__global__ void k_unpack_u8(uint8_t *__restrict__ dst, const uint8_t *__restrict__ src, Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = src[i + (long long)p.px * j + p.sz * k];
+}
+__global__ void k_mask(uint8_t *__restrict__ dst, Params p) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    const int P = p.P;
+    uint8_t m = 0;
+    if (i < P || i >= p.nx - P) m |= 1;
+    if (j < P || j >= p.ny - P) m |= 2;
+    if (k < P || k >= p.nz - P) m |= 4;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = m;
+}
+
+dim3 grid3(const Layout &L) { return dim3((L.nx + 127) / 128, L.ny, L.nz); }
+
+size_t field_bytes(const bvfdtd_ctx *c, uint32_t id) {
+    const size_t cells = (size_t)c->L.nx * c->L.ny * c->L.nz;
+    if (id <= BVFDTD_F_PRESSURE || id == BVFDTD_F_SUMSQ) return cells * 4;
+    if (id == BVFDTD_F_MATERIAL || id == BVFDTD_F_PML_MASK) return cells;
+    if (id == BVFDTD_F_DERIVED) return (size_t)c->n_materials * 8 * 4;
+    if (id == BVFDTD_F_PML_PROFILES) return (size_t)4 * (c->L.nx + c->L.ny + c->L.nz) * 4;
+    return 0;
+}
+
+// dense device buffer `d_dense` -> caller's dst (host: via async copy + sync)
+int deliver(bvfdtd_ctx *c, void *dst, const void *d_dense, size_t bytes, int dst_is_device) {
+    if (dst_is_device) {
+        if (dst != d_dense) CU(cudaMemcpyAsync(dst, d_dense, bytes, cudaMemcpyDeviceToDevice, c->stream));
+        return BVFDTD_OK;
+    }
+    CU(cudaMemcpyAsync(dst, d_dense, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return BVFDTD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *bvfdtd_strerror(int code) {
+    switch (code) {
+        case BVFDTD_OK: return "ok";
+        case BVFDTD_EINVAL: return "invalid argument";
+        case BVFDTD_ENOMEM: return "workspace too small or out of host memory";
+        case BVFDTD_ESTABILITY: return "time step violates the stability bound c_U dt/dx <= 0.494";
+        case BVFDTD_ECUDA: return "CUDA error (see bvfdtd_last_cuda_error)";
+        case BVFDTD_ESTATE: return "call not legal in the current state";
+        default: return "unknown status";
+    }
+}
+
+const char *bvfdtd_last_cuda_error(void) { return g_cuda_err; }
+
+int bvfdtd_derive_materials(const bvfdtd_material *table, int32_t n, double f0, float *out) {
+    if (!out) return BVFDTD_EINVAL;
+    std::vector<Derived> d;
+    const int rc = derive_materials(table, n, f0, d);
+    if (rc) return rc;
+    for (int m = 0; m < n; ++m) {
+        const double v[8] = {d[m].rho, d[m].piR, d[m].muR, d[m].tauP, d[m].tauS, d[m].piU, d[m].muU, d[m].cU};
+        for (int q = 0; q < 8; ++q) out[8 * m + q] = (float)v[q];
+    }
+    return BVFDTD_OK;
+}
+
+int bvfdtd_pml_profiles(int32_t n, int32_t pml, double dx, double dt, double f0, double pml_R,
+                        double c_ref, float *a_int, float *b_int, float *a_half, float *b_half) {
+    if (n < 1 || pml < 0 || 2 * pml > n || !(dx > 0) || !(dt > 0) || !(f0 > 0) || !(c_ref > 0) ||
+        !a_int || !b_int || !a_half || !b_half)
+        return BVFDTD_EINVAL;
+    if (pml_R == 0.0) pml_R = 1e-4;
+    if (!(pml_R > 0.0 && pml_R < 1.0)) return BVFDTD_EINVAL;
+    PmlAxis p;
+    pml_axis(n, pml, dx, dt, f0, pml_R, c_ref, p);
+    std::memcpy(a_int, p.a_int.data(), n * 4);
+    std::memcpy(b_int, p.b_int.data(), n * 4);
+    std::memcpy(a_half, p.a_half.data(), n * 4);
+    std::memcpy(b_half, p.b_half.data(), n * 4);
+    return BVFDTD_OK;
+}
+
+int bvfdtd_pml_mask(const bvfdtd_grid *g, uint8_t *mask) {
+    if (!grid_ok(g) || !mask) return BVFDTD_EINVAL;
+    const int P = g->pml;
+    size_t q = 0;
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                uint8_t m = 0;
+                if (i < P || i >= g->nx - P) m |= 1;
+                if (j < P || j >= g->ny - P) m |= 2;
+                if (k < P || k >= g->nz - P) m |= 4;
+                mask[q++] = m;
+            }
+    return BVFDTD_OK;
+}
+
+double bvfdtd_max_courant(const bvfdtd_material *table, int32_t n, double f0, double dt, double dx) {
+    std::vector<Derived> d;
+    const int rc = derive_materials(table, n, f0, d);
+    if (rc) return (double)rc;
+    if (!(dt > 0) || !(dx > 0)) return (double)BVFDTD_EINVAL;
+    return max_courant(d, dt, dx);
+}
+
+int bvfdtd_workspace_bytes(const bvfdtd_grid *grid, size_t *out_bytes) {
+    if (!grid_ok(grid) || !out_bytes) return BVFDTD_EINVAL;
+    *out_bytes = make_wsmap(make_layout(*grid)).total;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double dt,
+                  const bvfdtd_material *table, int32_t n_materials, const uint8_t *index_map,
+                  const bvfdtd_opts *opts, void *d_workspace, size_t workspace_bytes,
+                  void *cuda_stream) {
+    if (!out) return BVFDTD_EINVAL;
+    *out = nullptr;
+    if (!grid_ok(grid) || !table || !index_map || !opts || !d_workspace) return BVFDTD_EINVAL;
+    if (!(dx > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dt)) return BVFDTD_EINVAL;
+    if (!(opts->f0 > 0.0) || opts->reserved != 0) return BVFDTD_EINVAL;
+    double R = opts->pml_R == 0.0 ? 1e-4 : opts->pml_R;
+    if (!(R > 0.0 && R < 1.0)) return BVFDTD_EINVAL;
+    if (((uintptr_t)d_workspace & 255) != 0) return BVFDTD_EINVAL;
+
+    bvfdtd_ctx *c = new (std::nothrow) bvfdtd_ctx;
+    if (!c) return BVFDTD_ENOMEM;
+    struct Guard { bvfdtd_ctx *c; ~Guard() { delete c; } } guard{c};
+
+    int rc = derive_materials(table, n_materials, opts->f0, c->derived);
+    if (rc) return rc;
+    if (max_courant(c->derived, dt, dx) > 0.494) return BVFDTD_ESTABILITY;
+    const size_t cells = (size_t)grid->nx * grid->ny * grid->nz;
+    for (size_t q = 0; q < cells; ++q)
+        if (index_map[q] >= n_materials) return BVFDTD_EINVAL;
+
+    c->L = make_layout(*grid);
+    c->W = make_wsmap(c->L);
+    if (workspace_bytes < c->W.total) return BVFDTD_ENOMEM;
+    c->ws = (char *)d_workspace;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->dx = dx; c->dt = dt; c->opts = *opts; c->opts.pml_R = R; c->n_materials = n_materials;
+    const Layout &L = c->L;
+
+    // S0 tables
+    std::vector<KRow> rows;
+    kernel_rows(c->derived, dt, opts->f0, rows);
+    rows.resize(256, rows[0]);
+    double c_ref = 0.0;
+    for (int m = 0; m < n_materials; ++m) c_ref = std::max(c_ref, table[m].cL);
+    const int dims[3] = {L.nx, L.ny, L.nz};
+    std::vector<float> prof;
+    for (int a = 0; a < 3; ++a) {
+        pml_axis(dims[a], L.P, dx, dt, opts->f0, R, c_ref, c->pml[a]);
+        for (const std::vector<float> *v : {&c->pml[a].a_int, &c->pml[a].b_int, &c->pml[a].a_half, &c->pml[a].b_half})
+            prof.insert(prof.end(), v->begin(), v->end());
+    }
+    // index map in the private layout, edges replicated (reading P2)
+    std::vector<uint8_t> mat((size_t)L.mat_bytes);
+    for (int k = 0; k <= L.nz; ++k) {
+        const int ks = std::min(k, L.nz - 1);
+        for (int j = 0; j < L.py; ++j) {
+            const int js = std::min(j, L.ny - 1);
+            const uint8_t *src = index_map + (size_t)L.nx * (js + (size_t)L.ny * ks);
+            uint8_t *dst = mat.data() + (size_t)L.px * j + (size_t)L.sz * k;
+            std::memcpy(dst, src, L.nx);
+            std::memset(dst + L.nx, src[L.nx - 1], L.px - L.nx);
+        }
+    }
+
+    // zero the whole workspace (state, sensors, psi; reading P9), then upload
+    CU(cudaMemsetAsync(c->ws, 0, c->W.total, c->stream));
+    CU(cudaMemcpyAsync(c->ws + c->W.mat, mat.data(), mat.size(), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->ws + c->W.rows, rows.data(), 256 * sizeof(KRow), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->ws + c->W.prof, prof.data(), prof.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));  // host staging buffers die at return
+
+    Params &p = c->prm;
+    p.nx = L.nx; p.ny = L.ny; p.nz = L.nz; p.P = L.P;
+    p.px = L.px; p.py = L.py; p.wx = L.wx; p.sz = L.sz; p.org = L.org;
+    for (int q = 0; q < NSTATE; ++q) p.f[q] = (float *)(c->ws + c->W.field[q]);
+    p.peak = (float *)(c->ws + c->W.peak);
+    p.sumsq = (float *)(c->ws + c->W.sumsq);
+    p.mat = (const uint8_t *)(c->ws + c->W.mat);
+    for (int q = 0; q < 18; ++q) p.psi[q] = (float *)(c->ws + c->W.psi[q]);
+    p.rows = (const KRow *)(c->ws + c->W.rows);
+    {
+        const float *base = (const float *)(c->ws + c->W.prof);
+        for (int a = 0; a < 3; ++a)
+            for (int q = 0; q < 4; ++q) { p.prof[a][q] = base; base += dims[a]; }
+    }
+    const double tau_sigma = 1.0 / (2.0 * 3.14159265358979323846 * opts->f0);
+    const double beta = dt / (2.0 * tau_sigma);
+    p.inv_dx = (float)(1.0 / dx);
+    p.dt = (float)dt;
+    p.half_dt = (float)(0.5 * dt);
+    p.A = (float)((1.0 - beta) / (1.0 + beta));
+    p.B = (float)(2.0 * beta / (1.0 + beta));
+
+    if (!(opts->flags & BVFDTD_FLAG_REFERENCE_KERNELS)) {
+        rc = tiled_plan_create(c->plan, c->L, c->prm);
+        if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
+    }
+    guard.c = nullptr;
+    *out = c;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_set_source(bvfdtd_ctx *c, int64_t n_src, const int64_t *cell, const float *amp,
+                      const float *delay_s, int32_t waveform, double f_src, int32_t n_cycles) {
+    if (!c || n_src < 0) return BVFDTD_EINVAL;
+    if (n_src > 0) {
+        if (!cell || !amp || !delay_s || !(f_src > 0.0) || n_cycles < 1 || (waveform != 0 && waveform != 1))
+            return BVFDTD_EINVAL;
+        const Layout &L = c->L;
+        const int64_t cells = (int64_t)L.nx * L.ny * L.nz;
+        std::vector<int64_t> sorted(cell, cell + n_src);
+        std::sort(sorted.begin(), sorted.end());
+        for (int64_t s = 0; s < n_src; ++s) {
+            const int64_t q = sorted[s];
+            if (q < 0 || q >= cells) return BVFDTD_EINVAL;
+            if (s && sorted[s - 1] == q) return BVFDTD_EINVAL;
+            const int i = (int)(q % L.nx), j = (int)((q / L.nx) % L.ny), k = (int)(q / ((int64_t)L.nx * L.ny));
+            const int P = L.P;
+            if (i < P || i >= L.nx - P || j < P || j >= L.ny - P || k < P || k >= L.nz - P) return BVFDTD_EINVAL;
+            if (!std::isfinite(amp[s]) || !std::isfinite(delay_s[s])) return BVFDTD_EINVAL;
+        }
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    if (c->d_cell) { cudaFree(c->d_cell); cudaFree(c->d_amp); cudaFree(c->d_delay); }
+    c->d_cell = nullptr; c->d_amp = c->d_delay = nullptr;
+    c->n_src = 0;
+    if (n_src > 0) {
+        CU(cudaMalloc(&c->d_cell, n_src * sizeof(long long)));
+        CU(cudaMalloc(&c->d_amp, n_src * 4));
+        CU(cudaMalloc(&c->d_delay, n_src * 4));
+        CU(cudaMemcpyAsync(c->d_cell, cell, n_src * 8, cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_amp, amp, n_src * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(cudaMemcpyAsync(c->d_delay, delay_s, n_src * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        c->n_src = n_src; c->waveform = waveform; c->f_src = f_src; c->n_cycles = n_cycles;
+    }
+    return BVFDTD_OK;
+}
+
+int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
+    if (!c || n < 0) return BVFDTD_EINVAL;
+    const Layout &L = c->L;
+    const bool ref = (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) != 0;
+    for (int64_t s = 0; s < n; ++s) {
+        const int64_t step = c->step;
+        const bool in_end = c->opts.sensor_end < 0 || step < c->opts.sensor_end;
+        Params p = c->prm;
+        p.do_peak = in_end && step >= c->opts.peak_begin;
+        p.do_rms = in_end && step >= c->opts.rms_begin;
+        const bool timed = c->timing && c->timed_steps < BVFDTD_MAX_TIMED_STEPS;
+        cudaEvent_t *ev = nullptr;
+        if (timed) {
+            if (c->ev.size() < (size_t)(c->timed_steps + 1) * 4) {
+                for (int q = 0; q < 4; ++q) { cudaEvent_t e; CU(cudaEventCreate(&e)); c->ev.push_back(e); }
+            }
+            ev = &c->ev[c->timed_steps * 4];
+            CU(cudaEventRecord(ev[0], c->stream));
+        }
+        if (c->n_src > 0) {
+            const int tb = 128;
+            k_inject<<<(unsigned)((c->n_src + tb - 1) / tb), tb, 0, c->stream>>>(
+                p, c->n_src, c->d_cell, c->d_amp, c->d_delay, c->waveform, c->f_src, c->n_cycles,
+                (double)step * c->dt);
+        }
+        if (timed) CU(cudaEventRecord(ev[1], c->stream));
+        if (ref) {
+            const dim3 b(32, 4, 2), g((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
+            k_velocity_ref<<<g, b, 0, c->stream>>>(p);
+            if (timed) CU(cudaEventRecord(ev[2], c->stream));
+            k_stress_ref<<<g, b, 0, c->stream>>>(p);
+        } else {
+            int rc = tiled_velocity(c->plan, p, c->stream);
+            if (rc) return cuda_fail(cudaGetLastError(), "tiled_velocity");
+            if (timed) CU(cudaEventRecord(ev[2], c->stream));
+            rc = tiled_stress(c->plan, p, c->stream);
+            if (rc) return cuda_fail(cudaGetLastError(), "tiled_stress");
+        }
+        if (timed) { CU(cudaEventRecord(ev[3], c->stream)); c->timed_steps++; }
+        if (p.do_rms) c->rms_count++;
+        c->step++;
+    }
+    CU(cudaGetLastError());
+    return BVFDTD_OK;
+}
+
+int64_t bvfdtd_step_index(const bvfdtd_ctx *c) { return c ? c->step : -1; }
+
+int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, int32_t dst_is_device) {
+    if (!c || !dst) return BVFDTD_EINVAL;
+    const size_t need = field_bytes(c, id);
+    if (need == 0 || dst_bytes != need) return BVFDTD_EINVAL;
+    const Layout &L = c->L;
+    const dim3 b(128), g = grid3(L);
+    float *scratch = (float *)(c->ws + c->W.scratch);
+    if (id == BVFDTD_F_DERIVED || id == BVFDTD_F_PML_PROFILES) {
+        if (dst_is_device) return BVFDTD_EINVAL;
+        float *o = (float *)dst;
+        if (id == BVFDTD_F_DERIVED) {
+            for (int m = 0; m < c->n_materials; ++m) {
+                const Derived &d = c->derived[m];
+                const double v[8] = {d.rho, d.piR, d.muR, d.tauP, d.tauS, d.piU, d.muU, d.cU};
+                for (int q = 0; q < 8; ++q) *o++ = (float)v[q];
+            }
+        } else {
+            for (int a = 0; a < 3; ++a)
+                for (const std::vector<float> *v : {&c->pml[a].a_int, &c->pml[a].b_int, &c->pml[a].a_half, &c->pml[a].b_half}) {
+                    std::memcpy(o, v->data(), v->size() * 4);
+                    o += v->size();
+                }
+        }
+        return BVFDTD_OK;
+    }
+    void *target = dst_is_device ? dst : (void *)scratch;
+    if (id < NSTATE) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.f[id], c->prm);
+    else if (id == BVFDTD_F_SUMSQ) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.sumsq, c->prm);
+    else if (id == BVFDTD_F_PRESSURE) k_pressure<<<g, b, 0, c->stream>>>((float *)target, c->prm);
+    else if (id == BVFDTD_F_MATERIAL) k_unpack_u8<<<g, b, 0, c->stream>>>((uint8_t *)target, c->prm.mat, c->prm);
+    else k_mask<<<g, b, 0, c->stream>>>((uint8_t *)target, c->prm);
+    CU(cudaGetLastError());
+    return deliver(c, dst, target, need, dst_is_device);
+}
+
+int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_bytes, int32_t src_is_device) {
+    if (!c || !src || id >= NSTATE) return BVFDTD_EINVAL;
+    if (src_bytes != field_bytes(c, id)) return BVFDTD_EINVAL;
+    const float *d_src = (const float *)src;
+    if (!src_is_device) {
+        float *scratch = (float *)(c->ws + c->W.scratch);
+        CU(cudaMemcpyAsync(scratch, src, src_bytes, cudaMemcpyHostToDevice, c->stream));
+        d_src = scratch;
+    }
+    k_pack<<<grid3(c->L), 128, 0, c->stream>>>(c->prm.f[id], d_src, c->prm, id <= VZ ? (int)id : -1);
+    CU(cudaGetLastError());
+    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));
+    return BVFDTD_OK;
+}
+
+int bvfdtd_read_peak_pressure(bvfdtd_ctx *c, float *peak, float *rms_amp, int32_t dst_is_device) {
+    if (!c) return BVFDTD_EINVAL;
+    const Layout &L = c->L;
+    const size_t bytes = (size_t)L.nx * L.ny * L.nz * 4;
+    float *scratch = (float *)(c->ws + c->W.scratch);
+    if (peak) {
+        float *target = dst_is_device ? peak : scratch;
+        k_unpack<<<grid3(L), 128, 0, c->stream>>>(target, c->prm.peak, c->prm);
+        CU(cudaGetLastError());
+        const int rc = deliver(c, peak, target, bytes, dst_is_device);
+        if (rc) return rc;
+    }
+    if (rms_amp) {
+        float *target = dst_is_device ? rms_amp : scratch;
+        const float toc = c->rms_count > 0 ? (float)(2.0 / (double)c->rms_count) : 0.0f;
+        k_rms_amp<<<grid3(L), 128, 0, c->stream>>>(target, c->prm, toc);
+        CU(cudaGetLastError());
+        const int rc = deliver(c, rms_amp, target, bytes, dst_is_device);
+        if (rc) return rc;
+    }
+    return BVFDTD_OK;
+}
+
+int bvfdtd_enable_kernel_timing(bvfdtd_ctx *c, int32_t on) {
+    if (!c) return BVFDTD_EINVAL;
+    c->timing = on != 0;
+    c->timed_steps = 0;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[3], int64_t launches[3]) {
+    if (!c || !ms || !launches) return BVFDTD_EINVAL;
+    CU(cudaStreamSynchronize(c->stream));
+    for (int q = 0; q < 3; ++q) { ms[q] = 0.0; launches[q] = 0; }
+    for (int64_t s = 0; s < c->timed_steps; ++s) {
+        cudaEvent_t *ev = &c->ev[s * 4];
+        for (int q = 0; q < 3; ++q) {
+            float t = 0.0f;
+            CU(cudaEventElapsedTime(&t, ev[q], ev[q + 1]));
+            ms[q] += t;
+            launches[q] += 1;
+        }
+    }
+    if (c->n_src == 0) { ms[0] = 0.0; launches[0] = 0; }
+    c->timed_steps = 0;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_destroy(bvfdtd_ctx *c) {
+    if (!c) return BVFDTD_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    if (c->d_cell) { cudaFree(c->d_cell); cudaFree(c->d_amp); cudaFree(c->d_delay); }
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    tiled_plan_destroy(c->plan);
+    delete c;
+    return BVFDTD_OK;
+}
+
+}  // extern "C"
