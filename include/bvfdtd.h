@@ -68,9 +68,15 @@ typedef struct {
 } bvfdtd_material;
 
 enum { /* bvfdtd_opts.flags */
-    BVFDTD_FLAG_REFERENCE_KERNELS = 1 /* debug: run the one-thread-per-cell kernels instead of
-                                         the tiled TMA kernels (same arithmetic, same results up
-                                         to fp32 rounding order) */
+    BVFDTD_FLAG_REFERENCE_KERNELS = 1, /* debug: run the one-thread-per-cell kernels instead of
+                                          the tiled TMA kernels (same arithmetic, same results up
+                                          to fp32 rounding order) */
+    BVFDTD_FLAG_DENSE = 2              /* sweep every array everywhere: do not skip the shear
+                                          stresses / memory variables of tile-planes in which they
+                                          are identically zero (all-fluid or lossless regions,
+                                          DESIGN.md section 6).  Results are the same either way;
+                                          bvfdtd_write_fields of a shear stress or a memory variable
+                                          selects this mode by itself. */
 };
 
 typedef struct {

@@ -22,6 +22,7 @@ FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "sxy", "sxz", "syz",
 FIELD_ID = {n: i for i, n in enumerate(FIELDS)}
 FIELD_ID.update(p=15, material=16, pml_mask=17, derived=18, pml_profiles=19, sumsq=20)
 FLAG_REFERENCE_KERNELS = 1
+FLAG_DENSE = 2
 
 OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 

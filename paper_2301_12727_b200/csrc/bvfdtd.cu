@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -51,7 +52,13 @@ Layout make_layout(const bvfdtd_grid &g) {
     L.org = 2 * L.sz + 2 * L.px + 32;
     L.field_floats = round_up(L.org + L.sz * (g.nz + 2) + 2 * L.px + 32, 64);
     L.mat_bytes = round_up(L.sz * (g.nz + 1), 256);
-    L.wx = (int)round_up(2 * g.pml, 4);
+    L.xp4 = (int)round_up(g.pml, 4);
+    L.xhb = (g.nx - g.pml) & ~3;
+    L.xph = (int)round_up(g.nx - L.xhb, 4);
+    L.wx = L.xp4 + L.xph;
+    L.ntx = (g.nx + Cfg::TX - 1) / Cfg::TX;
+    L.nty = (g.ny + Cfg::TY - 1) / Cfg::TY;
+    L.flag_words = round_up((long long)L.ntx * L.nty * (g.nz + 4), 64);
     L.psi_floats[0] = round_up((long long)L.wx * g.ny * g.nz, 64);
     L.psi_floats[1] = round_up((long long)L.px * (2 * g.pml) * g.nz, 64);
     L.psi_floats[2] = round_up((long long)L.px * g.ny * (2 * g.pml), 64);
@@ -61,7 +68,7 @@ Layout make_layout(const bvfdtd_grid &g) {
 
 // Offsets (bytes) of every region of the caller's workspace.
 struct WsMap {
-    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, total;
+    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, flagsV, flagsS, total;
 };
 
 WsMap make_wsmap(const Layout &L) {
@@ -77,6 +84,8 @@ WsMap make_wsmap(const Layout &L) {
         for (int t = 0; t < 6; ++t) w.psi[a * 6 + t] = take(L.psi_floats[a] * 4);
     w.rows = take(256 * sizeof(KRow));
     w.prof = take((size_t)4 * (L.nx + L.ny + L.nz) * 4);
+    w.flagsV = take((size_t)L.flag_words * 4);
+    w.flagsS = take((size_t)L.flag_words * 4);
     w.total = off;
     return w;
 }
@@ -104,6 +113,7 @@ struct bvfdtd_ctx {
     double f_src = 0;
     // tiled-kernel plan (tensor maps etc.)
     TiledPlan plan;
+    bool dense = false;   // tile-class skipping off (BVFDTD_FLAG_DENSE, or a shear / memory field was written)
     // kernel timing
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -324,6 +334,9 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     Params &p = c->prm;
     p.nx = L.nx; p.ny = L.ny; p.nz = L.nz; p.P = L.P;
     p.px = L.px; p.py = L.py; p.wx = L.wx; p.sz = L.sz; p.org = L.org;
+    p.xp4 = L.xp4; p.xhb = L.xhb; p.xph = L.xph; p.ntx = L.ntx; p.nty = L.nty;
+    p.flagsV = (const uint32_t *)(c->ws + c->W.flagsV);
+    p.flagsS = (const uint32_t *)(c->ws + c->W.flagsS);
     for (int q = 0; q < NSTATE; ++q) p.f[q] = (float *)(c->ws + c->W.field[q]);
     p.peak = (float *)(c->ws + c->W.peak);
     p.sumsq = (float *)(c->ws + c->W.sumsq);
@@ -344,8 +357,18 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     p.B = (float)(2.0 * beta / (1.0 + beta));
 
     if (!(opts->flags & BVFDTD_FLAG_REFERENCE_KERNELS)) {
-        rc = tiled_plan_create(c->plan, c->L, c->prm);
+        char *psi_base[3];
+        long long psi_stride[3];
+        for (int a = 0; a < 3; ++a) {
+            psi_base[a] = c->ws + c->W.psi[a * 6];
+            psi_stride[a] = (long long)(c->W.psi[a * 6 + 1] - c->W.psi[a * 6]);
+        }
+        rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
+        c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;
+        tiled_flags(c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(c->stream));
     }
     guard.c = nullptr;
     *out = c;
@@ -483,6 +506,13 @@ int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_
     }
     k_pack<<<grid3(c->L), 128, 0, c->stream>>>(c->prm.f[id], d_src, c->prm, id <= VZ ? (int)id : -1);
     CU(cudaGetLastError());
+    if (id >= SXY && !c->dense && !(c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS)) {
+        // a caller-supplied shear stress or memory variable may be non-zero where the tile-class
+        // flags assume it is identically zero: switch this context to the dense sweep
+        c->dense = true;
+        tiled_flags(c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), true, c->stream);
+        CU(cudaGetLastError());
+    }
     if (!src_is_device) CU(cudaStreamSynchronize(c->stream));
     return BVFDTD_OK;
 }

@@ -23,13 +23,19 @@ struct Layout {
     long long org;            // offset of cell (0,0,0) inside a field allocation (floats)
     long long field_floats;   // floats per field allocation (multiple of 64)
     long long mat_bytes;      // index map: px * py * (nz + 1) bytes, edges replicated (P2)
-    int wx;                   // x pitch of the x-slab psi arrays = round_up(2P, 4)
+    int xp4, xhb, xph;        // x-slab psi: low slab at compact [0, xp4), xp4 = round_up(P, 4); high slab
+                              // at xp4 + (i - xhb), xhb = floor4(nx - P), width xph = round_up(nx - xhb, 4)
+    int wx;                   // x pitch of the x-slab psi arrays = xp4 + xph
     long long psi_floats[3];  // floats per psi array of axis x, y, z
+    int ntx, nty;             // x-y tiles of the tiled kernels
+    long long flag_words;     // uint32 words per flag table: ntx * nty * (nz + 4)
 };
 
 struct Params {
     int nx, ny, nz, P;
     int px, py, wx;
+    int xp4, xhb, xph;     // x-slab compact index: i < P ? i : xp4 + (i - xhb)
+    int ntx, nty;
     long long sz, org;
     float *f[NSTATE];
     float *peak, *sumsq;
@@ -39,6 +45,17 @@ struct Params {
     const float *prof[3][4];  // per axis: a_int, b_int, a_half, b_half
     float inv_dx, dt, half_dt, A, B;
     int do_peak, do_rms;
+    // tile-class flags: one word per (tile, plane + 2), planes -2..nz+1
+    const uint32_t *flagsV, *flagsS;
+};
+
+// tile-class flag bits
+enum : uint32_t {
+    TF_XY = 1u,    // stress: some xy shear node of the tile-plane has four solid cells
+    TF_XZ = 2u,    //         ... xz ...
+    TF_YZ = 4u,    //         ... yz ...
+    TF_RII = 8u,   // stress: some cell of the tile-plane is lossy (r_ii can be non-zero)
+    // velocity: the same three bits, taken over the halo-extended region the pass reads
 };
 
 }  // namespace bvfdtd

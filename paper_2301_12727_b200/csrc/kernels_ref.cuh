@@ -38,7 +38,7 @@ __device__ __forceinline__ SlabIdx slab_index(const Params &p, int i, int j, int
     s.in[0] = (i < P) || (i >= p.nx - P);
     s.in[1] = (j < P) || (j >= p.ny - P);
     s.in[2] = (k < P) || (k >= p.nz - P);
-    const int ix = i < P ? i : i - (p.nx - 2 * P);
+    const int ix = i < P ? i : p.xp4 + (i - p.xhb);
     const int jy = j < P ? j : j - (p.ny - 2 * P);
     const int kz = k < P ? k : k - (p.nz - 2 * P);
     s.q[0] = ix + (long long)p.wx * (j + (long long)p.ny * k);

@@ -2,10 +2,12 @@
 //
 // One CTA owns a TX x TY tile of the x-y plane and marches a chunk of z-planes.  A producer warp
 // (one elected lane) issues cp.async.bulk.tensor box loads for the planes of iteration m into a
-// ring of NS shared-memory stages (mbarrier full/empty pairs); NC = (TX/4)*TY consumer threads
-// each own 4 consecutive x-cells of one row (float4) and keep the z-direction stencil windows and
-// the x-y partial sums of the not-yet-finished planes in registers (a sliding window), so every
-// array plane is fetched from L2/HBM exactly once per CTA (plus the x-y halo of the box):
+// ring of shared-memory stages (mbarrier full/empty pairs); NC = (TX/4)*TY consumer threads each
+// own 4 consecutive x-cells of one row (float4) and keep the z-direction stencil windows and the
+// x-y partial sums of the not-yet-finished planes in registers (a sliding window), so every array
+// plane is fetched from L2/HBM exactly once per CTA (plus the x-y halo of the box).  Consumers read
+// shared memory only and write their results with 16-byte global stores: EVERY global read of the
+// hot loop, including the C-PML memory variables psi and the material indices, is a TMA prefetch.
 //
 //   velocity pass  (S2, Eq. 1 rows 1-3): iteration m loads sxx,syy,sxy,sxz,syz,szz at plane m and
 //       the old vx,vy (plane m-1), vz (plane m-2); it forms the x-y derivative sums of plane m,
@@ -17,9 +19,13 @@
 //
 // Out-of-grid reads: the private layout keeps zero gaps around every field (device_params.hpp)
 // and TMA zero-fills boxes that leave the allocation, so the zero ghost of reading P4 needs no
-// branch.  PML (reading P5): CTAs / planes that touch a slab take the psi branches (block- or
-// iteration-uniform tests, per-cell predicates inside); psi itself is read-modify-written with
-// plain global accesses because only slab cells touch it.
+// branch.
+//
+// Tile-class flags: per (tile, plane) words say whether any shear node of
+// kind xy / xz / yz has four solid cells and whether any cell is lossy.  Where a kind has no solid
+// node its stress and memory variable are identically zero (mu_h = 0, reading P2; zero initial
+// state, P9), so producer and consumers skip its loads, arithmetic and stores.  Both sides derive
+// the same per-iteration load plan from the same flag words (vel_plan / str_plan below).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -33,9 +39,11 @@ namespace bvfdtd {
 // ------------------------------------------------------------------------------------------
 // configuration
 // ------------------------------------------------------------------------------------------
-template <int TX_, int TY_, int NS_>
+constexpr int MAX_STAGES = 4;
+
+template <int TX_, int TY_>
 struct TileCfg {
-    static constexpr int TX = TX_, TY = TY_, NS = NS_;
+    static constexpr int TX = TX_, TY = TY_;
     static constexpr int NC = (TX / 4) * TY;            // consumer threads
     static constexpr int NT = NC + 32;                  // + producer warp
     static constexpr int AX = TX + 8, BY = TY + 4;      // halo box extents
@@ -45,30 +53,32 @@ struct TileCfg {
     static constexpr int D_BYTES = TX * TY * 4;         // plain tile
     static constexpr int MX = TX + 16, MY = TY + 1;     // material box (bytes)
     static constexpr int M_BYTES = (MX * MY + 127) / 128 * 128;
-    static constexpr int MR = NS + 3;                   // material ring of the stress pass
-    // velocity stage: sxx A, syy B, sxy C, sxz A, syz B, szz D, vx vy vz D, mat
-    static constexpr int V_SXX = 0, V_SYY = V_SXX + A_BYTES, V_SXY = V_SYY + B_BYTES,
-                         V_SXZ = V_SXY + C_BYTES, V_SYZ = V_SXZ + A_BYTES, V_SZZ = V_SYZ + B_BYTES,
-                         V_VX = V_SZZ + D_BYTES, V_VY = V_VX + D_BYTES, V_VZ = V_VY + D_BYTES,
-                         V_MAT = V_VZ + D_BYTES, V_STAGE = V_MAT + M_BYTES;
-    // stress stage: vx vy vz C, 12 sigma/r D, peak, sumsq D
-    static constexpr int S_V = 0, S_SR = 3 * C_BYTES, S_PEAK = S_SR + 12 * D_BYTES,
-                         S_SUMSQ = S_PEAK + D_BYTES, S_STAGE = S_SUMSQ + D_BYTES;
-    static constexpr int V_SMEM = NS * V_STAGE + 256 * 4 + 2 * NS * 8 + 128;
-    static constexpr int S_SMEM = NS * S_STAGE + MR * M_BYTES + 256 * 32 + 2 * NS * 8 + 128;
     static_assert(A_BYTES % 128 == 0 && B_BYTES % 128 == 0 && C_BYTES % 128 == 0 && D_BYTES % 128 == 0, "TMA alignment");
+    static_assert(NC % 32 == 0, "whole consumer warps");
 };
 
-using Cfg = TileCfg<64, 8, 2>;
+using Cfg = TileCfg<64, 8>;
 
 struct TiledMaps {
     CUtensorMap boxA, boxB, boxC, boxD;   // 4-D (x, y, z+2, field) fp32 maps over the 17 grid arrays
     CUtensorMap mat;                      // 3-D uint8 map over the index map
+    CUtensorMap psx, psy, psz;            // 4-D (x, y, z, array) maps over the slab-compact psi arrays
+};
+
+// Shared-memory plan of one pipeline stage (byte offsets inside the stage), fixed per context.
+struct StagePlan {
+    int psx, psy, psz;     // first psi slot of each axis (3 slots per axis)
+    int xb;                // bytes of one x-psi box (low or high slab); one slot = 2 boxes
+    int wxb;               // x-psi box width in floats
+    int bytes;             // stage size (multiple of 128)
+    int ns;                // pipeline stages
+    int smem;              // dynamic shared memory of the launch
 };
 
 struct TiledPlan {
     TiledMaps maps;
-    int chunks = 1, nzc = 0;
+    StagePlan sv, ss;
+    int chunks_v = 1, nzc_v = 0, chunks_s = 1, nzc_s = 0;
     bool ready = false;
 };
 
@@ -92,7 +102,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
         "{\n"
         ".reg .pred P1;\n"
         "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, 0x989680;\n"
         "@P1 bra DONE;\n"
         "bra LAB_WAIT;\n"
         "DONE:\n"
@@ -113,215 +123,362 @@ __device__ __forceinline__ void prefetch_tmap(const CUtensorMap *m) {
 }
 
 // ------------------------------------------------------------------------------------------
-// small device helpers
+// packed arithmetic on a thread's four x-consecutive cells (FADD2 / FMUL2 / FFMA2 on sm_100)
 // ------------------------------------------------------------------------------------------
-#define TC1 1.125f
-#define TC2 (-1.0f / 24.0f)
-
-__device__ __forceinline__ float4 lds4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
-
-// 12 consecutive x values around the thread's 4 cells: a[4..7] are its own cells i0..i0+3
-struct Row12 {
-    float a[12];
+struct Q4 {
+    float2 a, b;   // cells (0,1) and (2,3)
 };
-__device__ __forceinline__ Row12 load_row12(const float *row_own) {   // row_own -> own float4
-    Row12 r;
-    const float4 L = lds4(row_own - 4), O = lds4(row_own), R = lds4(row_own + 4);
-    r.a[0] = L.x; r.a[1] = L.y; r.a[2] = L.z; r.a[3] = L.w;
-    r.a[4] = O.x; r.a[5] = O.y; r.a[6] = O.z; r.a[7] = O.w;
-    r.a[8] = R.x; r.a[9] = R.y; r.a[10] = R.z; r.a[11] = R.w;
+__device__ __forceinline__ Q4 q_ld(const float *p) {
+    const float4 v = *reinterpret_cast<const float4 *>(p);
+    Q4 q; q.a = make_float2(v.x, v.y); q.b = make_float2(v.z, v.w); return q;
+}
+__device__ __forceinline__ Q4 q_set(float s) { Q4 q; q.a = make_float2(s, s); q.b = q.a; return q; }
+__device__ __forceinline__ Q4 q_make(float x, float y, float z, float w) { Q4 q; q.a = make_float2(x, y); q.b = make_float2(z, w); return q; }
+__device__ __forceinline__ float2 f2neg(float2 v) { return make_float2(-v.x, -v.y); }
+__device__ __forceinline__ Q4 q_add(Q4 x, Q4 y) { Q4 q; q.a = __fadd2_rn(x.a, y.a); q.b = __fadd2_rn(x.b, y.b); return q; }
+__device__ __forceinline__ Q4 q_sub(Q4 x, Q4 y) { Q4 q; q.a = __fadd2_rn(x.a, f2neg(y.a)); q.b = __fadd2_rn(x.b, f2neg(y.b)); return q; }
+__device__ __forceinline__ Q4 q_mul(Q4 x, Q4 y) { Q4 q; q.a = __fmul2_rn(x.a, y.a); q.b = __fmul2_rn(x.b, y.b); return q; }
+__device__ __forceinline__ Q4 q_muls(Q4 x, float s) { const float2 t = make_float2(s, s); Q4 q; q.a = __fmul2_rn(x.a, t); q.b = __fmul2_rn(x.b, t); return q; }
+__device__ __forceinline__ Q4 q_fma(Q4 x, Q4 y, Q4 z) { Q4 q; q.a = __ffma2_rn(x.a, y.a, z.a); q.b = __ffma2_rn(x.b, y.b, z.b); return q; }
+__device__ __forceinline__ Q4 q_fmas(float s, Q4 y, Q4 z) { const float2 t = make_float2(s, s); Q4 q; q.a = __ffma2_rn(t, y.a, z.a); q.b = __ffma2_rn(t, y.b, z.b); return q; }
+// x - y*z
+__device__ __forceinline__ Q4 q_fnma(Q4 y, Q4 z, Q4 x) { Q4 q; q.a = __ffma2_rn(f2neg(y.a), z.a, x.a); q.b = __ffma2_rn(f2neg(y.b), z.b, x.b); return q; }
+__device__ __forceinline__ float q_get(const Q4 &q, int c) { return c == 0 ? q.a.x : c == 1 ? q.a.y : c == 2 ? q.b.x : q.b.y; }
+__device__ __forceinline__ void q_st(float *g, const Q4 &q) { *reinterpret_cast<float4 *>(g) = make_float4(q.a.x, q.a.y, q.b.x, q.b.y); }
+// store the first nv (1..4) cells only: partial quad at the ragged x edge
+__device__ __forceinline__ void q_st_n(float *g, const Q4 &q, int nv) {
+    if (nv >= 4) { q_st(g, q); return; }
+    g[0] = q.a.x;
+    if (nv > 1) g[1] = q.a.y;
+    if (nv > 2) g[2] = q.b.x;
+}
+
+// 4-point staggered difference from four values ordered along the axis (weights carry 1/dx):
+// c1 (b - a) + c2 (d - z)
+__device__ __forceinline__ Q4 q_d4(const Q4 &z, const Q4 &a, const Q4 &b, const Q4 &d, float c1, float c2) {
+    return q_fmas(c2, q_sub(d, z), q_muls(q_sub(b, a), c1));
+}
+// C-PML (reading P5): psi <- b psi + a D ; D <- D + psi.  psi_old comes from the TMA stage.
+__device__ __forceinline__ Q4 q_cpml(Q4 &d, const Q4 &psi_old, const Q4 &a, const Q4 &b) {
+    const Q4 pn = q_fma(b, psi_old, q_mul(a, d));
+    d = q_add(d, pn);
+    return pn;
+}
+
+// x-direction differences of a thread's four cells from f[-2..5] around its quad (scalar: the
+// operand pairs are misaligned for the packed forms).  f points at the own quad in shared memory.
+struct XRow { float f[8]; };   // f[0] = cell -2 ... f[7] = cell +5
+// D- (lands on the integer node): c1 (f(i)-f(i-1)) + c2 (f(i+1)-f(i-2)); needs cells -2..4
+__device__ __forceinline__ Q4 x_dminus(const float *own, float c1, float c2) {
+    const float2 l = *reinterpret_cast<const float2 *>(own - 2);
+    const float4 o = *reinterpret_cast<const float4 *>(own);
+    const float r = own[4];
+    return q_make(fmaf(c2, o.y - l.x, c1 * (o.x - l.y)), fmaf(c2, o.z - l.y, c1 * (o.y - o.x)),
+                  fmaf(c2, o.w - o.x, c1 * (o.z - o.y)), fmaf(c2, r - o.y, c1 * (o.w - o.z)));
+}
+// D+ (lands on the half node): c1 (f(i+1)-f(i)) + c2 (f(i+2)-f(i-1)); needs cells -1..5
+__device__ __forceinline__ Q4 x_dplus(const float *own, float c1, float c2) {
+    const float l = own[-1];
+    const float4 o = *reinterpret_cast<const float4 *>(own);
+    const float2 r = *reinterpret_cast<const float2 *>(own + 4);
+    return q_make(fmaf(c2, o.z - l, c1 * (o.y - o.x)), fmaf(c2, o.w - o.x, c1 * (o.z - o.y)),
+                  fmaf(c2, r.x - o.y, c1 * (o.w - o.z)), fmaf(c2, r.y - o.z, c1 * (r.x - o.w)));
+}
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
-// D+x at cell c (result on the half node): c1 (f(i+1)-f(i)) + c2 (f(i+2)-f(i-1))
-__device__ __forceinline__ float dpx(const Row12 &r, int c, float inv_dx) {
-    return (TC1 * (r.a[5 + c] - r.a[4 + c]) + TC2 * (r.a[6 + c] - r.a[3 + c])) * inv_dx;
-}
-// D-x at cell c (result on the integer node): c1 (f(i)-f(i-1)) + c2 (f(i+1)-f(i-2))
-__device__ __forceinline__ float dmx(const Row12 &r, int c, float inv_dx) {
-    return (TC1 * (r.a[4 + c] - r.a[3 + c]) + TC2 * (r.a[5 + c] - r.a[2 + c])) * inv_dx;
-}
-__device__ __forceinline__ float comp(const float4 &v, int c) { return c == 0 ? v.x : c == 1 ? v.y : c == 2 ? v.z : v.w; }
-// 4-point difference from four values ordered along the axis: c1 (b-a) + c2 (d-z)
-__device__ __forceinline__ float d4(float z, float a, float b, float d, float inv_dx) {
-    return (TC1 * (b - a) + TC2 * (d - z)) * inv_dx;
+// reciprocal with one Newton step (finite positive x)
+__device__ __forceinline__ float rcp_newton(float x) {
+    const float r = rcp_approx(x);
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
 }
 
-// per-thread PML bookkeeping for its 4 cells
-struct PmlCtx {
-    bool tile_x, row_y;     // this thread's cells can be in an x slab / its row is in a y slab
-    bool in_x[4];
-    int ix[4];              // slab-compact x index
-    int jy;                 // slab-compact y index
+// ------------------------------------------------------------------------------------------
+// per-thread geometry shared by both passes
+// ------------------------------------------------------------------------------------------
+template <class C>
+struct ThreadGeom {
+    int tx, ty, i0, j, nv;       // nv = valid cells of the quad (0 = inactive thread)
+    bool active;
+    bool in_x;                   // quad touches an x slab
+    bool row_y;                  // row in a y slab
+    int psx_off;                 // float offset of the quad inside an x-psi slot (low or high box)
+    long long gx, gy;            // global float offset of the quad inside an x-/y-psi array at plane 0
+    long long gz;                // ... inside a z-psi array at compact plane 0
+    long long gcell;             // global float offset of the quad inside a grid field at plane 0
+    float ay_i, by_i, ay_h, by_h;
 };
 
-__device__ __forceinline__ float psi_rmw(float *__restrict__ psi, long long q, float a, float b, float d) {
-    const float p = fmaf(b, psi[q], a * d);
-    psi[q] = p;
-    return d + p;
+template <class C>
+__device__ __forceinline__ ThreadGeom<C> make_geom(const Params &p, const StagePlan &sp, int tid, int x0, int y0) {
+    ThreadGeom<C> g;
+    g.tx = tid % (C::TX / 4); g.ty = tid / (C::TX / 4);
+    g.i0 = x0 + 4 * g.tx; g.j = y0 + g.ty;
+    g.active = (g.j < p.ny) && (g.i0 < p.nx);
+    g.nv = g.active ? min(4, p.nx - g.i0) : 0;
+    const int P = p.P;
+    const bool in_lo = g.active && P > 0 && g.i0 < P;
+    const bool in_hi = g.active && P > 0 && g.i0 >= p.xhb;
+    g.in_x = in_lo || in_hi;
+    // low box is loaded at compact x = x0, high box at compact x = xp4 + max(x0, xhb) - xhb
+    const int hi0 = max(x0, p.xhb);
+    g.psx_off = in_lo ? (g.ty * sp.wxb + (g.i0 - x0)) : (sp.xb / 4 + g.ty * sp.wxb + (g.i0 - hi0));
+    const int cx = in_lo ? g.i0 : p.xp4 + (g.i0 - p.xhb);
+    g.gx = cx + (long long)p.wx * g.j;
+    g.row_y = g.active && P > 0 && (g.j < P || g.j >= p.ny - P);
+    const int jy = g.j < P ? g.j : g.j - (p.ny - 2 * P);
+    g.gy = g.i0 + (long long)p.px * jy;
+    g.gz = g.i0 + (long long)p.px * g.j;
+    g.gcell = p.org + g.i0 + (long long)p.px * g.j;
+    g.ay_i = g.by_i = g.ay_h = g.by_h = 0.0f;
+    if (g.row_y) {
+        g.ay_i = __ldg(p.prof[1][0] + g.j); g.by_i = __ldg(p.prof[1][1] + g.j);
+        g.ay_h = __ldg(p.prof[1][2] + g.j); g.by_h = __ldg(p.prof[1][3] + g.j);
+    }
+    return g;
 }
+
+// x-slab profile coefficients of the tile columns, zero outside the slabs / the grid
+template <class C>
+__device__ __forceinline__ void fill_xprof(float *sprof, const Params &p, int x0, int tid) {
+    for (int q = tid; q < 4 * C::TX; q += C::NT) {
+        const int a = q / C::TX, c = q % C::TX, i = x0 + c;
+        const bool in = p.P > 0 && i < p.nx && (i < p.P || i >= p.nx - p.P);
+        sprof[q] = in ? __ldg(p.prof[0][a] + i) : 0.0f;
+    }
+}
+
+struct TileX {
+    bool lo, hi;       // the tile touches the low / high x slab
+    int cx_lo, cx_hi;  // compact x of the two boxes
+};
+template <class C>
+__device__ __forceinline__ TileX make_tilex(const Params &p, int x0) {
+    TileX t;
+    t.lo = p.P > 0 && x0 < p.P;
+    t.hi = p.P > 0 && x0 + C::TX > p.xhb && x0 < p.nx;
+    t.cx_lo = x0;
+    t.cx_hi = p.xp4 + max(x0, p.xhb) - p.xhb;
+    return t;
+}
+template <class C>
+__device__ __forceinline__ bool tile_in_y(const Params &p, int y0) { return p.P > 0 && (y0 < p.P || y0 + C::TY > p.ny - p.P); }
+template <class C>
+__device__ __forceinline__ int tile_jy0(const Params &p, int y0) { return y0 < p.P ? y0 : y0 - (p.ny - 2 * p.P); }
+__device__ __forceinline__ bool z_in_slab(const Params &p, int k) { return p.P > 0 && k >= 0 && k < p.nz && (k < p.P || k >= p.nz - p.P); }
+__device__ __forceinline__ int z_compact(const Params &p, int k) { return k < p.P ? k : k - (p.nz - 2 * p.P); }
 
 // ------------------------------------------------------------------------------------------
 // S2: velocity pass
 // ------------------------------------------------------------------------------------------
+// stage slots (bytes), fixed part
 template <class C>
-__global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p, const int nzc) {
-    extern __shared__ __align__(128) unsigned char smem[];
+struct VStage {
+    static constexpr int SXX = 0, SYY = SXX + C::A_BYTES, SZZ = SYY + C::B_BYTES, SXY = SZZ + C::D_BYTES,
+                         SXZ = SXY + C::C_BYTES, SYZ = SXZ + C::A_BYTES, VXO = SYZ + C::B_BYTES,
+                         VYO = VXO + C::D_BYTES, VZO = VYO + C::D_BYTES, MAT = VZO + C::D_BYTES,
+                         FIXED = MAT + C::M_BYTES;
+};
+
+// What iteration m of the velocity pass loads and computes: derived identically by producer and
+// consumers from the chunk range and the flag words of planes m-3..m.
+struct VelPlan {
+    bool in0, in1, in2;    // plane m / m-1 / m-2 inside the chunk
+    bool xy, xz, yz;       // plane m carries non-zero sxy / sxz / syz (in the halo-extended tile)
+    bool wxz, wyz;         // some plane of the z window m-3..m carries non-zero sxz / syz
+};
+__device__ __forceinline__ VelPlan vel_plan(int m, int kz0, int kz1, uint32_t fl, uint32_t &hist_xz, uint32_t &hist_yz) {
+    VelPlan v;
+    v.in0 = m >= kz0 && m < kz1;
+    v.in1 = m - 1 >= kz0 && m - 1 < kz1;
+    v.in2 = m - 2 >= kz0 && m - 2 < kz1;
+    v.xy = (fl & TF_XY) != 0;
+    v.xz = (fl & TF_XZ) != 0;
+    v.yz = (fl & TF_YZ) != 0;
+    hist_xz = ((hist_xz << 1) | (v.xz ? 1u : 0u)) & 15u;
+    hist_yz = ((hist_yz << 1) | (v.yz ? 1u : 0u)) & 15u;
+    v.wxz = hist_xz != 0;
+    v.wyz = hist_yz != 0;
+    return v;
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
+                                                             const int nzc, const StagePlan sp) {
+    using VS = VStage<C>;
+    extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
-    float *rho_tab = reinterpret_cast<float *>(smem + C::NS * C::V_STAGE);
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + C::NS * C::V_STAGE + 256 * 4);
-    uint64_t *empty = full + C::NS;
+    float *rho_tab = reinterpret_cast<float *>(smem + sp.ns * sp.bytes);
+    float *sprof = rho_tab + 256;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * C::TX);
+    uint64_t *empty = full + MAX_STAGES;
 
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
     const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
     const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
+    const uint32_t *flags = p.flagsV + (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2;
 
     for (int q = tid; q < 256; q += C::NT) rho_tab[q] = p.rows[q].rho;
+    fill_xprof<C>(sprof, p, x0, tid);
     if (tid == 0) {
-        for (int s = 0; s < C::NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NC / 32); }
+        for (int s = 0; s < sp.ns; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+
+    const TileX tX = make_tilex<C>(p, x0);
+    const bool tY = tile_in_y<C>(p, y0);
+    const int jy0 = tile_jy0<C>(p, y0);
 
     if (tid >= C::NC) {
         // ================= producer warp =================
         if (tid == C::NC) {
             prefetch_tmap(&maps.boxA); prefetch_tmap(&maps.boxB); prefetch_tmap(&maps.boxC);
             prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
+            if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
+            uint32_t hxz = 0, hyz = 0;
+            const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
             for (int m = m_begin; m < m_end; ++m) {
+                const VelPlan v = vel_plan(m, kz0, kz1, __ldg(flags + m), hxz, hyz);
                 mbar_wait(&empty[s], ph ^ 1);
-                unsigned char *st = stages + s * C::V_STAGE;
-                const bool ld_xy = (m - 1 >= kz0) && (m - 1 < kz1);
-                const bool ld_z = (m - 2 >= kz0) && (m - 2 < kz1);
-                uint32_t bytes = 2 * C::A_BYTES + 2 * C::B_BYTES + C::C_BYTES + C::D_BYTES + C::MX * C::MY;
-                if (ld_xy) bytes += 2 * C::D_BYTES;
-                if (ld_z) bytes += C::D_BYTES;
-                mbar_expect_tx(&full[s], bytes);
-                const int z = m + 2;
-                tma_load_4d(st + C::V_SXX, &maps.boxA, &full[s], x0 - 4, y0, z, SXX);
-                tma_load_4d(st + C::V_SYY, &maps.boxB, &full[s], x0, y0 - 1, z, SYY);
-                tma_load_4d(st + C::V_SXY, &maps.boxC, &full[s], x0 - 4, y0 - 2, z, SXY);
-                tma_load_4d(st + C::V_SXZ, &maps.boxA, &full[s], x0 - 4, y0, z, SXZ);
-                tma_load_4d(st + C::V_SYZ, &maps.boxB, &full[s], x0, y0 - 2, z, SYZ);
-                tma_load_4d(st + C::V_SZZ, &maps.boxD, &full[s], x0, y0, z, SZZ);
-                if (ld_xy) {
-                    tma_load_4d(st + C::V_VX, &maps.boxD, &full[s], x0, y0, z - 1, VX);
-                    tma_load_4d(st + C::V_VY, &maps.boxD, &full[s], x0, y0, z - 1, VY);
+                unsigned char *st = stages + s * sp.bytes;
+                uint64_t *bar = &full[s];
+                const bool zs1 = v.in1 && z_in_slab(p, m - 1), zs2 = v.in2 && z_in_slab(p, m - 2);
+                const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
+                uint32_t bytes = C::D_BYTES + C::MX * C::MY;                       // szz, mat
+                if (v.xz) bytes += C::A_BYTES;
+                if (v.yz) bytes += C::B_BYTES;
+                if (v.in0) {
+                    bytes += C::A_BYTES + C::B_BYTES + (v.xy ? C::C_BYTES : 0);
+                    bytes += nx_boxes * xbox * (1u + (v.xy ? 1u : 0u) + (v.xz ? 1u : 0u));
+                    if (tY) bytes += C::D_BYTES * (1u + (v.xy ? 1u : 0u) + (v.yz ? 1u : 0u));
                 }
-                if (ld_z) tma_load_4d(st + C::V_VZ, &maps.boxD, &full[s], x0, y0, z - 2, VZ);
-                tma_load_3d(st + C::V_MAT, &maps.mat, &full[s], x0, y0, m - 1);
-                if (++s == C::NS) { s = 0; ph ^= 1; }
+                if (v.in1) bytes += 2 * C::D_BYTES;
+                if (v.in2) bytes += C::D_BYTES;
+                if (zs1) bytes += C::D_BYTES * ((v.wxz ? 1u : 0u) + (v.wyz ? 1u : 0u));
+                if (zs2) bytes += C::D_BYTES;
+                mbar_expect_tx(bar, bytes);
+                const int z = m + 2;
+                tma_load_4d(st + VS::SZZ, &maps.boxD, bar, x0, y0, z, SZZ);
+                if (v.xz) tma_load_4d(st + VS::SXZ, &maps.boxA, bar, x0 - 4, y0, z, SXZ);
+                if (v.yz) tma_load_4d(st + VS::SYZ, &maps.boxB, bar, x0, y0 - 2, z, SYZ);
+                if (v.in0) {
+                    tma_load_4d(st + VS::SXX, &maps.boxA, bar, x0 - 4, y0, z, SXX);
+                    tma_load_4d(st + VS::SYY, &maps.boxB, bar, x0, y0 - 1, z, SYY);
+                    if (v.xy) tma_load_4d(st + VS::SXY, &maps.boxC, bar, x0 - 4, y0 - 2, z, SXY);
+                    // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
+                    const bool use[3] = {true, v.xy, v.xz};
+                    const bool usey[3] = {v.xy, true, v.yz};
+#pragma unroll
+                    for (int t = 0; t < 3; ++t) {
+                        if (use[t]) {
+                            unsigned char *d = st + sp.psx + t * 2 * sp.xb;
+                            if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, t);
+                            if (tX.hi) tma_load_4d(d + sp.xb, &maps.psx, bar, tX.cx_hi, y0, m, t);
+                        }
+                        if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, t);
+                    }
+                }
+                if (v.in1) {
+                    tma_load_4d(st + VS::VXO, &maps.boxD, bar, x0, y0, z - 1, VX);
+                    tma_load_4d(st + VS::VYO, &maps.boxD, bar, x0, y0, z - 1, VY);
+                }
+                if (v.in2) tma_load_4d(st + VS::VZO, &maps.boxD, bar, x0, y0, z - 2, VZ);
+                if (zs1) {
+                    const int kc = z_compact(p, m - 1);
+                    if (v.wxz) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, kc, 0);
+                    if (v.wyz) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, kc, 1);
+                }
+                if (zs2) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 2);
+                tma_load_3d(st + VS::MAT, &maps.mat, bar, x0, y0, m - 1);
+                if (++s == sp.ns) { s = 0; ph ^= 1; }
             }
         }
         return;
     }
 
     // ================= consumers =================
-    const int tx = tid % (C::TX / 4), ty = tid / (C::TX / 4);
-    const int i0 = x0 + 4 * tx, j = y0 + ty;
-    const bool row_ok = (j < p.ny) && (i0 < p.nx);   // the thread owns at least one cell
-    const int P = p.P;
-    const float inv_dx = p.inv_dx, dt = p.dt;
-    bool ok[4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) ok[c] = row_ok && (i0 + c < p.nx);
+    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
+    const int tx = g.tx, ty = g.ty;
+    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
+    const float dt2 = 2.0f * p.dt;
+    const bool wall_x = g.active && (p.nx - 1 >= g.i0) && (p.nx - 1 <= g.i0 + 3);   // quad holds cell nx-1 (P4)
+    const bool wall_y = g.j == p.ny - 1;
+    const Q4 zero = q_set(0.0f);
 
-    PmlCtx pc;
-    pc.tile_x = (P > 0) && (i0 < P || i0 + 3 >= p.nx - P);
-    pc.row_y = (P > 0) && (j < P || j >= p.ny - P) && row_ok;
-    pc.jy = j < P ? j : j - (p.ny - 2 * P);
+    Q4 wxz[4], wyz[4], wzz[4];                 // z windows: slot 3 = plane m ... slot 0 = plane m-3
+    Q4 pvx = zero, pvy = zero, pvz1 = zero, pvz2 = zero;   // x-y sums of planes m-1 (pvx, pvy, pvz1) and m-2 (pvz2)
+    float rho_prev[4] = {1.0f, 1.0f, 1.0f, 1.0f};          // rho of the thread's cells at plane m-2
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const int i = i0 + c;
-        pc.in_x[c] = pc.tile_x && ok[c] && (i < P || i >= p.nx - P);
-        pc.ix[c] = i < P ? i : i - (p.nx - 2 * P);
-    }
-
-    float wxz[4][4], wyz[4][4], wzz[4][4];   // z windows: slot 3 = plane m ... slot 0 = plane m-3
-    float pvx[4], pvy[4], pvz1[4], pvz2[4];  // x-y sums of planes m-1 (pvx, pvy, pvz1) and m-2 (pvz2)
-    float rho_prev[4];                        // rho of the thread's cells at plane m-2
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-#pragma unroll
-        for (int w = 0; w < 4; ++w) wxz[w][c] = wyz[w][c] = wzz[w][c] = 0.0f;
-        pvx[c] = pvy[c] = pvz1[c] = pvz2[c] = 0.0f;
-        rho_prev[c] = 1.0f;
-    }
+    for (int w = 0; w < 4; ++w) wxz[w] = wyz[w] = wzz[w] = zero;
 
     int s = 0; uint32_t ph = 0;
+    uint32_t hxz = 0, hyz = 0;
+    uint32_t fl_next = __ldg(flags + m_begin);
     for (int m = m_begin; m < m_end; ++m) {
+        const uint32_t fl = fl_next;
+        fl_next = __ldg(flags + min(m + 1, p.nz + 1));
+        const VelPlan v = vel_plan(m, kz0, kz1, fl, hxz, hyz);
         mbar_wait(&full[s], ph);
-        const unsigned char *st = stages + s * C::V_STAGE;
-        const float *sA_xx = reinterpret_cast<const float *>(st + C::V_SXX) + ty * C::AX + 4 + 4 * tx;
-        const float *sB_yy = reinterpret_cast<const float *>(st + C::V_SYY) + ty * C::TX + 4 * tx;
-        const float *sC_xy = reinterpret_cast<const float *>(st + C::V_SXY) + ty * C::AX + 4 + 4 * tx;
-        const float *sA_xz = reinterpret_cast<const float *>(st + C::V_SXZ) + ty * C::AX + 4 + 4 * tx;
-        const float *sB_yz = reinterpret_cast<const float *>(st + C::V_SYZ) + ty * C::TX + 4 * tx;
-        const float *sD = reinterpret_cast<const float *>(st + C::V_SZZ) + ty * C::TX + 4 * tx;
+        const unsigned char *st = stages + s * sp.bytes;
+        const int qoff = ty * C::TX + 4 * tx;             // own quad inside a D / B(row 0) box
+        const int aoff = ty * C::AX + 4 + 4 * tx;         // own quad inside an A / C(row 0) box
+        const float *sD = reinterpret_cast<const float *>(st + VS::SZZ) + qoff;
 
-        float nvx[4], nvy[4], nvz[4];
-        const bool plane_in = (m >= kz0) && (m < kz1);
-        float4 xz_own, yz_own;
-        {
-            const Row12 rxz = load_row12(sA_xz);
-            xz_own = make_float4(rxz.a[4], rxz.a[5], rxz.a[6], rxz.a[7]);
-            const float4 y0v = lds4(sB_yz), y1v = lds4(sB_yz + C::TX), y2v = lds4(sB_yz + 2 * C::TX), y3v = lds4(sB_yz + 3 * C::TX);
-            yz_own = y2v;
-            if (plane_in) {
-                const Row12 rxx = load_row12(sA_xx);
-                const Row12 rxy = load_row12(sC_xy + 2 * C::AX);
-                const float4 xy0 = lds4(sC_xy), xy1 = lds4(sC_xy + C::AX), xy3 = lds4(sC_xy + 3 * C::AX);
-                const float4 yy0 = lds4(sB_yy), yy1 = lds4(sB_yy + C::TX), yy2 = lds4(sB_yy + 2 * C::TX), yy3 = lds4(sB_yy + 3 * C::TX);
-                const bool zin = true;
-                (void)zin;
-                float ay_i = 0, by_i = 0, ay_h = 0, by_h = 0;
-                if (pc.row_y) {
-                    ay_i = __ldg(p.prof[1][0] + j); by_i = __ldg(p.prof[1][1] + j);
-                    ay_h = __ldg(p.prof[1][2] + j); by_h = __ldg(p.prof[1][3] + j);
-                }
+        // ---- z windows: slide and insert plane m ----
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    float dxx = dpx(rxx, c, inv_dx);                                             // D+x sxx -> vx
-                    float dxy_y = d4(comp(xy0, c), comp(xy1, c), rxy.a[4 + c], comp(xy3, c), inv_dx);   // D-y sxy -> vx
-                    float dxy_x = dmx(rxy, c, inv_dx);                                           // D-x sxy -> vy
-                    float dyy = d4(comp(yy0, c), comp(yy1, c), comp(yy2, c), comp(yy3, c), inv_dx);     // D+y syy -> vy
-                    float dxz = dmx(rxz, c, inv_dx);                                             // D-x sxz -> vz
-                    float dyz = d4(comp(y0v, c), comp(y1v, c), comp(y2v, c), comp(y3v, c), inv_dx);     // D-y syz -> vz
-                    if (pc.in_x[c]) {
-                        const int i = i0 + c;
-                        const long long q = pc.ix[c] + (long long)p.wx * (j + (long long)p.ny * m);
-                        dxx = psi_rmw(p.psi[0], q, __ldg(p.prof[0][2] + i), __ldg(p.prof[0][3] + i), dxx);
-                        dxy_x = psi_rmw(p.psi[1], q, __ldg(p.prof[0][0] + i), __ldg(p.prof[0][1] + i), dxy_x);
-                        dxz = psi_rmw(p.psi[2], q, __ldg(p.prof[0][0] + i), __ldg(p.prof[0][1] + i), dxz);
-                    }
-                    if (pc.row_y && ok[c]) {
-                        const long long q = (i0 + c) + (long long)p.px * (pc.jy + (long long)(2 * P) * m);
-                        dxy_y = psi_rmw(p.psi[6], q, ay_i, by_i, dxy_y);
-                        dyy = psi_rmw(p.psi[7], q, ay_h, by_h, dyy);
-                        dyz = psi_rmw(p.psi[8], q, ay_i, by_i, dyz);
-                    }
-                    nvx[c] = dxx + dxy_y;
-                    nvy[c] = dxy_x + dyy;
-                    nvz[c] = dxz + dyz;
-                }
-            } else {
-#pragma unroll
-                for (int c = 0; c < 4; ++c) nvx[c] = nvy[c] = nvz[c] = 0.0f;
+        for (int w = 0; w < 3; ++w) { wxz[w] = wxz[w + 1]; wyz[w] = wyz[w + 1]; wzz[w] = wzz[w + 1]; }
+        wzz[3] = q_ld(sD);
+        const float *sA_xz = reinterpret_cast<const float *>(st + VS::SXZ) + aoff;
+        const float *sB_yz = reinterpret_cast<const float *>(st + VS::SYZ) + qoff;     // row j-2
+        wxz[3] = v.xz ? q_ld(sA_xz) : zero;
+        wyz[3] = v.yz ? q_ld(sB_yz + 2 * C::TX) : zero;
+
+        // ---- x-y derivative sums of plane m ----
+        Q4 nvx = zero, nvy = zero, nvz = zero;
+        if (v.in0 && g.active) {
+            const float *sA_xx = reinterpret_cast<const float *>(st + VS::SXX) + aoff;
+            const float *sB_yy = reinterpret_cast<const float *>(st + VS::SYY) + qoff;   // row j-1
+            Q4 dxx = x_dplus(sA_xx, c1, c2);                                             // D+x sxx -> vx
+            Q4 dyy = q_d4(q_ld(sB_yy), q_ld(sB_yy + C::TX), q_ld(sB_yy + 2 * C::TX), q_ld(sB_yy + 3 * C::TX), c1, c2);   // D+y syy -> vy
+            Q4 dxy_y = zero, dxy_x = zero, dxz = zero, dyz = zero;
+            if (v.xy) {
+                const float *sC = reinterpret_cast<const float *>(st + VS::SXY) + aoff;  // row j-2
+                dxy_x = x_dminus(sC + 2 * C::AX, c1, c2);                                // D-x sxy -> vy
+                dxy_y = q_d4(q_ld(sC), q_ld(sC + C::AX), q_ld(sC + 2 * C::AX), q_ld(sC + 3 * C::AX), c1, c2);   // D-y sxy -> vx
             }
-        }
-        const float4 zz_own = lds4(sD);
-        // slide the z windows and insert plane m
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-#pragma unroll
-            for (int w = 0; w < 3; ++w) { wxz[w][c] = wxz[w + 1][c]; wyz[w][c] = wyz[w + 1][c]; wzz[w][c] = wzz[w + 1][c]; }
-            wxz[3][c] = comp(xz_own, c); wyz[3][c] = comp(yz_own, c); wzz[3][c] = comp(zz_own, c);
+            if (v.xz) dxz = x_dminus(sA_xz, c1, c2);                                     // D-x sxz -> vz
+            if (v.yz) dyz = q_d4(q_ld(sB_yz), q_ld(sB_yz + C::TX), q_ld(sB_yz + 2 * C::TX), q_ld(sB_yz + 3 * C::TX), c1, c2);   // D-y syz -> vz
+            if (g.in_x) {
+                const float *sp_x = sprof + 4 * tx;
+                const Q4 ai = q_ld(sp_x), bi = q_ld(sp_x + C::TX), ah = q_ld(sp_x + 2 * C::TX), bh = q_ld(sp_x + 3 * C::TX);
+                const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
+                const long long q = g.gx + (long long)p.wx * p.ny * m;
+                q_st(p.psi[0] + q, q_cpml(dxx, q_ld(ps), ah, bh));
+                if (v.xy) q_st(p.psi[1] + q, q_cpml(dxy_x, q_ld(ps + sp.xb / 2), ai, bi));
+                if (v.xz) q_st(p.psi[2] + q, q_cpml(dxz, q_ld(ps + sp.xb), ai, bi));
+            }
+            if (g.row_y) {
+                const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
+                const long long q = g.gy + (long long)p.px * (2 * p.P) * m;
+                const Q4 ai = q_set(g.ay_i), bi = q_set(g.by_i);
+                if (v.xy) q_st_n(p.psi[6] + q, q_cpml(dxy_y, q_ld(ps), ai, bi), g.nv);
+                q_st_n(p.psi[7] + q, q_cpml(dyy, q_ld(ps + C::D_BYTES / 4), q_set(g.ay_h), q_set(g.by_h)), g.nv);
+                if (v.yz) q_st_n(p.psi[8] + q, q_cpml(dyz, q_ld(ps + 2 * (C::D_BYTES / 4)), ai, bi), g.nv);
+            }
+            nvx = q_add(dxx, dxy_y);
+            nvy = q_add(dxy_x, dyy);
+            nvz = q_add(dxz, dyz);
         }
 
-        // material of plane m-1: rho at i0..i0+4 of row j and i0..i0+3 of row j+1
-        const unsigned char *mt = st + C::V_MAT + ty * C::MX + 4 * tx;
+        // ---- material of plane m-1: rho at i0..i0+4 of row j and i0..i0+3 of row j+1 ----
+        const unsigned char *mt = st + VS::MAT + ty * C::MX + 4 * tx;
         float rho_j[5], rho_j1[4];
         {
             const uint32_t w0 = *reinterpret_cast<const uint32_t *>(mt);
@@ -335,397 +492,464 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
         }
 
         const int k1 = m - 1, k2 = m - 2;
-        if (k1 >= kz0 && k1 < kz1 && row_ok) {
+        if (v.in1 && g.active) {
             // finish vx, vy at plane k1: D-z of sxz / syz over planes m-3..m
-            const float4 vxo = lds4(reinterpret_cast<const float *>(st + C::V_VX) + ty * C::TX + 4 * tx);
-            const float4 vyo = lds4(reinterpret_cast<const float *>(st + C::V_VY) + ty * C::TX + 4 * tx);
-            const bool zs = (P > 0) && (k1 < P || k1 >= p.nz - P);
-            float az = 0, bz = 0;
-            int kz = 0;
-            if (zs) { az = __ldg(p.prof[2][0] + k1); bz = __ldg(p.prof[2][1] + k1); kz = k1 < P ? k1 : k1 - (p.nz - 2 * P); }
-            float ox[4], oy[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                float dzx = d4(wxz[0][c], wxz[1][c], wxz[2][c], wxz[3][c], inv_dx);
-                float dzy = d4(wyz[0][c], wyz[1][c], wyz[2][c], wyz[3][c], inv_dx);
-                if (zs && ok[c]) {
-                    const long long q = (i0 + c) + (long long)p.px * (j + (long long)p.ny * kz);
-                    dzx = psi_rmw(p.psi[12], q, az, bz, dzx);
-                    dzy = psi_rmw(p.psi[13], q, az, bz, dzy);
-                }
-                const float rx = 0.5f * (rho_j[c] + rho_j[c + 1]);
-                const float ry = 0.5f * (rho_j[c] + rho_j1[c]);
-                const float nx_ = comp(vxo, c) + dt / rx * (pvx[c] + dzx);
-                const float ny_ = comp(vyo, c) + dt / ry * (pvy[c] + dzy);
-                ox[c] = (ok[c] && (i0 + c < p.nx - 1)) ? nx_ : 0.0f;
-                oy[c] = (ok[c] && (j < p.ny - 1)) ? ny_ : 0.0f;
+            Q4 sx = pvx, sy = pvy;
+            const bool zs = z_in_slab(p, k1);
+            float az = 0.0f, bz = 0.0f;
+            long long qz = 0;
+            if (zs) { az = __ldg(p.prof[2][0] + k1); bz = __ldg(p.prof[2][1] + k1); qz = g.gz + (long long)p.px * p.ny * z_compact(p, k1); }
+            if (v.wxz) {
+                Q4 dzx = q_d4(wxz[0], wxz[1], wxz[2], wxz[3], c1, c2);
+                if (zs) q_st_n(p.psi[12] + qz, q_cpml(dzx, q_ld(reinterpret_cast<const float *>(st + sp.psz) + qoff), q_set(az), q_set(bz)), g.nv);
+                sx = q_add(sx, dzx);
             }
-            const long long g = p.org + i0 + (long long)p.px * j + p.sz * k1;
-            *reinterpret_cast<float4 *>(p.f[VX] + g) = make_float4(ox[0], ox[1], ox[2], ox[3]);
-            *reinterpret_cast<float4 *>(p.f[VY] + g) = make_float4(oy[0], oy[1], oy[2], oy[3]);
+            if (v.wyz) {
+                Q4 dzy = q_d4(wyz[0], wyz[1], wyz[2], wyz[3], c1, c2);
+                if (zs) q_st_n(p.psi[13] + qz, q_cpml(dzy, q_ld(reinterpret_cast<const float *>(st + sp.psz + C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
+                sy = q_add(sy, dzy);
+            }
+            const Q4 cx = q_make(dt2 * rcp_newton(rho_j[0] + rho_j[1]), dt2 * rcp_newton(rho_j[1] + rho_j[2]),
+                                 dt2 * rcp_newton(rho_j[2] + rho_j[3]), dt2 * rcp_newton(rho_j[3] + rho_j[4]));
+            const Q4 cy = q_make(dt2 * rcp_newton(rho_j[0] + rho_j1[0]), dt2 * rcp_newton(rho_j[1] + rho_j1[1]),
+                                 dt2 * rcp_newton(rho_j[2] + rho_j1[2]), dt2 * rcp_newton(rho_j[3] + rho_j1[3]));
+            Q4 ox = q_fma(cx, sx, q_ld(reinterpret_cast<const float *>(st + VS::VXO) + qoff));
+            Q4 oy = q_fma(cy, sy, q_ld(reinterpret_cast<const float *>(st + VS::VYO) + qoff));
+            if (wall_x) {
+                const int wc = p.nx - 1 - g.i0;
+                if (wc == 0) ox.a.x = 0.0f; else if (wc == 1) ox.a.y = 0.0f; else if (wc == 2) ox.b.x = 0.0f; else ox.b.y = 0.0f;
+            }
+            if (wall_y) oy = zero;
+            const long long gq = g.gcell + p.sz * k1;
+            q_st_n(p.f[VX] + gq, ox, g.nv);
+            q_st_n(p.f[VY] + gq, oy, g.nv);
         }
-        if (k2 >= kz0 && k2 < kz1 && row_ok) {
+        if (v.in2 && g.active) {
             // finish vz at plane k2: D+z of szz over planes m-3..m
-            const float4 vzo = lds4(reinterpret_cast<const float *>(st + C::V_VZ) + ty * C::TX + 4 * tx);
-            const bool zs = (P > 0) && (k2 < P || k2 >= p.nz - P);
-            float az = 0, bz = 0;
-            int kz = 0;
-            if (zs) { az = __ldg(p.prof[2][2] + k2); bz = __ldg(p.prof[2][3] + k2); kz = k2 < P ? k2 : k2 - (p.nz - 2 * P); }
-            float oz[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                float dzz = d4(wzz[0][c], wzz[1][c], wzz[2][c], wzz[3][c], inv_dx);
-                if (zs && ok[c]) {
-                    const long long q = (i0 + c) + (long long)p.px * (j + (long long)p.ny * kz);
-                    dzz = psi_rmw(p.psi[14], q, az, bz, dzz);
-                }
-                const float rz = 0.5f * (rho_prev[c] + rho_j[c]);
-                const float nz_ = comp(vzo, c) + dt / rz * (pvz2[c] + dzz);
-                oz[c] = (ok[c] && (k2 < p.nz - 1)) ? nz_ : 0.0f;
+            Q4 dzz = q_d4(wzz[0], wzz[1], wzz[2], wzz[3], c1, c2);
+            if (z_in_slab(p, k2)) {
+                const float az = __ldg(p.prof[2][2] + k2), bz = __ldg(p.prof[2][3] + k2);
+                const long long qz = g.gz + (long long)p.px * p.ny * z_compact(p, k2);
+                q_st_n(p.psi[14] + qz, q_cpml(dzz, q_ld(reinterpret_cast<const float *>(st + sp.psz + 2 * C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
             }
-            const long long g = p.org + i0 + (long long)p.px * j + p.sz * k2;
-            *reinterpret_cast<float4 *>(p.f[VZ] + g) = make_float4(oz[0], oz[1], oz[2], oz[3]);
+            const Q4 cz = q_make(dt2 * rcp_newton(rho_prev[0] + rho_j[0]), dt2 * rcp_newton(rho_prev[1] + rho_j[1]),
+                                 dt2 * rcp_newton(rho_prev[2] + rho_j[2]), dt2 * rcp_newton(rho_prev[3] + rho_j[3]));
+            Q4 oz = q_fma(cz, q_add(pvz2, dzz), q_ld(reinterpret_cast<const float *>(st + VS::VZO) + qoff));
+            if (k2 == p.nz - 1) oz = zero;
+            q_st_n(p.f[VZ] + g.gcell + p.sz * k2, oz, g.nv);
         }
+        pvz2 = pvz1; pvz1 = nvz; pvx = nvx; pvy = nvy;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            pvz2[c] = pvz1[c]; pvz1[c] = nvz[c]; pvx[c] = nvx[c]; pvy[c] = nvy[c];
-            rho_prev[c] = rho_j[c];
-        }
+        for (int c = 0; c < 4; ++c) rho_prev[c] = rho_j[c];
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&empty[s]);
-        if (++s == C::NS) { s = 0; ph ^= 1; }
+        if (++s == sp.ns) { s = 0; ph ^= 1; }
     }
 }
 
 // ------------------------------------------------------------------------------------------
 // S3 + S4: stress, memory variables, sensor
 // ------------------------------------------------------------------------------------------
-struct ShearMat {
-    float inv, ts;   // 1/mu_R (+inf for a fluid) and tau_s of one cell
+template <class C>
+struct SStage {
+    static constexpr int VXB = 0, VYB = C::C_BYTES, VZB = 2 * C::C_BYTES, SII = 3 * C::C_BYTES,
+                         RII = SII + 3 * C::D_BYTES, PEAK = RII + 3 * C::D_BYTES, SUMSQ = PEAK + C::D_BYTES,
+                         SXY = SUMSQ + C::D_BYTES, RXY = SXY + C::D_BYTES, SXZ = RXY + C::D_BYTES,
+                         RXZ = SXZ + C::D_BYTES, SYZ = RXZ + C::D_BYTES, RYZ = SYZ + C::D_BYTES,
+                         FIXED = RYZ + C::D_BYTES;
 };
 
+struct StrPlan {
+    bool in0, in1, in2;
+    bool xy0, xz0, yz0;    // plane m: finish sxy / form the D+x vz, D+y vz partials
+    bool rii1;             // plane m-1 has lossy cells
+    bool xz2, yz2;         // plane m-2: finish sxz / syz
+};
+// f0, f1, f2 = flag words of planes m, m-1, m-2
+__device__ __forceinline__ StrPlan str_plan(int m, int kz0, int kz1, uint32_t f0, uint32_t f1, uint32_t f2) {
+    StrPlan v;
+    v.in0 = m >= kz0 && m < kz1;
+    v.in1 = m - 1 >= kz0 && m - 1 < kz1;
+    v.in2 = m - 2 >= kz0 && m - 2 < kz1;
+    v.xy0 = v.in0 && (f0 & TF_XY);
+    v.xz0 = v.in0 && (f0 & TF_XZ);
+    v.yz0 = v.in0 && (f0 & TF_YZ);
+    v.rii1 = v.in1 && (f1 & TF_RII);
+    v.xz2 = v.in2 && (f2 & TF_XZ);
+    v.yz2 = v.in2 && (f2 & TF_YZ);
+    return v;
+}
+
+struct ShearCoef { float cU, cR; };   // dt mu_U,h and B mu_h tau_h of one shear node (readings P2, P3)
+__device__ __forceinline__ ShearCoef shear_coef(float2 a, float2 b, float2 c, float2 d, float dt, float B) {
+    // .x = 1/mu_R (+inf for a fluid: the harmonic mean becomes 0), .y = tau_s
+    const float mu_h = 4.0f * rcp_approx((a.x + b.x) + (c.x + d.x));
+    const float ts_h = 0.25f * ((a.y + b.y) + (c.y + d.y));
+    const float mt = mu_h * ts_h;
+    ShearCoef r; r.cU = dt * (mu_h + mt); r.cR = B * mt;
+    return r;
+}
+
 template <class C>
-__global__ void __launch_bounds__(C::NT, 2) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p, const int nzc) {
-    extern __shared__ __align__(128) unsigned char smem[];
+__global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
+                                                           const int nzc, const StagePlan sp) {
+    using SS = SStage<C>;
+    constexpr int DQ = C::D_BYTES / 4;
+    extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
-    unsigned char *mat_ring = smem + C::NS * C::S_STAGE;
-    KRow *tab = reinterpret_cast<KRow *>(mat_ring + C::MR * C::M_BYTES);
-    uint64_t *full = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(tab) + 256 * 32);
-    uint64_t *empty = full + C::NS;
+    const int MR = sp.ns + 3;                                   // material ring planes
+    unsigned char *mat_ring = smem + sp.ns * sp.bytes;
+    float4 *tabN = reinterpret_cast<float4 *>(mat_ring + MR * C::M_BYTES);   // eP, eS, bP, bS
+    float2 *tabS = reinterpret_cast<float2 *>(tabN + 256);                   // 1/mu_R (inf = fluid), tau_s
+    float *sprof = reinterpret_cast<float *>(tabS + 256);
+    uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * C::TX);
+    uint64_t *empty = full + MAX_STAGES;
 
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
     const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
     const int m_begin = kz0 - 2, m_end = kz1 + 2;
-    const bool sens = p.do_peak | p.do_rms;
+    const uint32_t *flags = p.flagsS + (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2;
+    const bool do_peak = p.do_peak != 0, do_rms = p.do_rms != 0;
 
     for (int q = tid; q < 256; q += C::NT) {
-        KRow r = p.rows[q];
-        if (r.solid == 0.0f) r.invMu = __int_as_float(0x7f800000);   // +inf: harmonic mean -> 0 (P2)
-        tab[q] = r;
+        const KRow r = p.rows[q];
+        tabN[q] = make_float4(r.eP, r.eS, r.bP, r.bS);
+        tabS[q] = make_float2(r.solid == 0.0f ? __int_as_float(0x7f800000) : r.invMu, r.tauS);
     }
+    fill_xprof<C>(sprof, p, x0, tid);
     if (tid == 0) {
-        for (int s = 0; s < C::NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NC / 32); }
+        for (int s = 0; s < sp.ns; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
 
+    const TileX tX = make_tilex<C>(p, x0);
+    const bool tY = tile_in_y<C>(p, y0);
+    const int jy0 = tile_jy0<C>(p, y0);
+
     if (tid >= C::NC) {
         if (tid == C::NC) {
             prefetch_tmap(&maps.boxC); prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
+            if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
-            int mr = ((m_begin % C::MR) + C::MR) % C::MR;
+            int mr = ((m_begin % MR) + MR) % MR;
+            uint32_t f1 = 0, f2 = 0;
+            const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
+            const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
             for (int m = m_begin; m < m_end; ++m) {
+                const uint32_t f0 = __ldg(flags + m);
+                const StrPlan v = str_plan(m, kz0, kz1, f0, f1, f2);
+                f2 = f1; f1 = f0;
                 mbar_wait(&empty[s], ph ^ 1);
-                unsigned char *st = stages + s * C::S_STAGE;
-                const bool in0 = (m >= kz0) && (m < kz1);
-                const bool in1 = (m - 1 >= kz0) && (m - 1 < kz1);
-                const bool in2 = (m - 2 >= kz0) && (m - 2 < kz1);
+                unsigned char *st = stages + s * sp.bytes;
+                uint64_t *bar = &full[s];
+                const bool zs1 = v.in1 && z_in_slab(p, m - 1), zs2 = v.in2 && z_in_slab(p, m - 2);
                 uint32_t bytes = 3 * C::C_BYTES + C::MX * C::MY;
-                if (in0) bytes += 2 * C::D_BYTES;
-                if (in1) bytes += 6 * C::D_BYTES + (p.do_peak ? C::D_BYTES : 0) + (p.do_rms ? C::D_BYTES : 0);
-                if (in2) bytes += 4 * C::D_BYTES;
-                mbar_expect_tx(&full[s], bytes);
+                if (v.in0) {
+                    bytes += nx_boxes * xbox * (1u + (v.xy0 ? 1u : 0u) + (v.xz0 ? 1u : 0u));
+                    if (tY) bytes += C::D_BYTES * (1u + (v.xy0 ? 1u : 0u) + (v.yz0 ? 1u : 0u));
+                }
+                if (v.xy0) bytes += 2 * C::D_BYTES;
+                if (v.in1) bytes += C::D_BYTES * (3u + (v.rii1 ? 3u : 0u) + (do_peak ? 1u : 0u) + (do_rms ? 1u : 0u) + (zs1 ? 1u : 0u));
+                if (v.xz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
+                if (v.yz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
+                mbar_expect_tx(bar, bytes);
                 const int z = m + 2;
-                tma_load_4d(st + C::S_V, &maps.boxC, &full[s], x0 - 4, y0 - 2, z, VX);
-                tma_load_4d(st + C::S_V + C::C_BYTES, &maps.boxC, &full[s], x0 - 4, y0 - 2, z, VY);
-                tma_load_4d(st + C::S_V + 2 * C::C_BYTES, &maps.boxC, &full[s], x0 - 4, y0 - 2, z, VZ);
-                unsigned char *sr = st + C::S_SR;
-                if (in1) {
-                    tma_load_4d(sr + 0 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, SXX);
-                    tma_load_4d(sr + 1 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, SYY);
-                    tma_load_4d(sr + 2 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, SZZ);
-                    tma_load_4d(sr + 3 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, RXX);
-                    tma_load_4d(sr + 4 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, RYY);
-                    tma_load_4d(sr + 5 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 1, RZZ);
-                    if (p.do_peak) tma_load_4d(st + C::S_PEAK, &maps.boxD, &full[s], x0, y0, z - 1, F_PEAK);
-                    if (p.do_rms) tma_load_4d(st + C::S_SUMSQ, &maps.boxD, &full[s], x0, y0, z - 1, F_SUMSQ);
+                tma_load_4d(st + SS::VXB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VX);
+                tma_load_4d(st + SS::VYB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VY);
+                tma_load_4d(st + SS::VZB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VZ);
+                if (v.in0) {
+                    // psi of the x-y derivatives of plane m: x terms 3 (D-x vx), 4 (D+x vy), 5 (D+x vz);
+                    // y terms 3 (D+y vx), 4 (D-y vy), 5 (D+y vz)
+                    const bool use[3] = {true, v.xy0, v.xz0};
+                    const bool usey[3] = {v.xy0, true, v.yz0};
+#pragma unroll
+                    for (int t = 0; t < 3; ++t) {
+                        if (use[t]) {
+                            unsigned char *d = st + sp.psx + t * 2 * sp.xb;
+                            if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, 3 + t);
+                            if (tX.hi) tma_load_4d(d + sp.xb, &maps.psx, bar, tX.cx_hi, y0, m, 3 + t);
+                        }
+                        if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, 3 + t);
+                    }
                 }
-                if (in0) {
-                    tma_load_4d(sr + 6 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z, SXY);
-                    tma_load_4d(sr + 7 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z, RXY);
+                if (v.xy0) {
+                    tma_load_4d(st + SS::SXY, &maps.boxD, bar, x0, y0, z, SXY);
+                    tma_load_4d(st + SS::RXY, &maps.boxD, bar, x0, y0, z, RXY);
                 }
-                if (in2) {
-                    tma_load_4d(sr + 8 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 2, SXZ);
-                    tma_load_4d(sr + 9 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 2, RXZ);
-                    tma_load_4d(sr + 10 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 2, SYZ);
-                    tma_load_4d(sr + 11 * C::D_BYTES, &maps.boxD, &full[s], x0, y0, z - 2, RYZ);
+                if (v.in1) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::SII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, SXX + q);
+                    if (v.rii1) {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::RII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, RXX + q);
+                    }
+                    if (do_peak) tma_load_4d(st + SS::PEAK, &maps.boxD, bar, x0, y0, z - 1, F_PEAK);
+                    if (do_rms) tma_load_4d(st + SS::SUMSQ, &maps.boxD, bar, x0, y0, z - 1, F_SUMSQ);
+                    if (zs1) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 1), 5);
                 }
-                tma_load_3d(mat_ring + mr * C::M_BYTES, &maps.mat, &full[s], x0, y0, m);
-                if (++mr == C::MR) mr = 0;
-                if (++s == C::NS) { s = 0; ph ^= 1; }
+                if (v.xz2) {
+                    tma_load_4d(st + SS::SXZ, &maps.boxD, bar, x0, y0, z - 2, SXZ);
+                    tma_load_4d(st + SS::RXZ, &maps.boxD, bar, x0, y0, z - 2, RXZ);
+                    if (zs2) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 3);
+                }
+                if (v.yz2) {
+                    tma_load_4d(st + SS::SYZ, &maps.boxD, bar, x0, y0, z - 2, SYZ);
+                    tma_load_4d(st + SS::RYZ, &maps.boxD, bar, x0, y0, z - 2, RYZ);
+                    if (zs2) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 4);
+                }
+                tma_load_3d(mat_ring + mr * C::M_BYTES, &maps.mat, bar, x0, y0, m);
+                if (++mr == MR) mr = 0;
+                if (++s == sp.ns) { s = 0; ph ^= 1; }
             }
         }
         return;
     }
 
     // ================= consumers =================
-    const int tx = tid % (C::TX / 4), ty = tid / (C::TX / 4);
-    const int i0 = x0 + 4 * tx, j = y0 + ty;
-    const bool row_ok = (j < p.ny) && (i0 < p.nx);   // the thread owns at least one cell
-    const int P = p.P;
-    const float inv_dx = p.inv_dx, dt = p.dt, hdt = p.half_dt, A = p.A, B = p.B;
-    bool ok[4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) ok[c] = row_ok && (i0 + c < p.nx);
+    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
+    const int tx = g.tx, ty = g.ty;
+    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
+    const float dt = p.dt, hdt = p.half_dt, A = p.A, B = p.B;
+    const Q4 zero = q_set(0.0f);
 
-    PmlCtx pc;
-    pc.tile_x = (P > 0) && (i0 < P || i0 + 3 >= p.nx - P);
-    pc.row_y = (P > 0) && (j < P || j >= p.ny - P) && row_ok;
-    pc.jy = j < P ? j : j - (p.ny - 2 * P);
+    Q4 wvx[4], wvy[4], wvz[4];     // z windows, slot 3 = plane m
+    Q4 nxx = zero, nyy = zero;     // vxx, vyy of plane m-1
+    Q4 dxz1 = zero, dxz2 = zero, dyz1 = zero, dyz2 = zero;   // D+x vz, D+y vz of planes m-1 and m-2
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const int i = i0 + c;
-        pc.in_x[c] = pc.tile_x && ok[c] && (i < P || i >= p.nx - P);
-        pc.ix[c] = i < P ? i : i - (p.nx - 2 * P);
-    }
-
-    float wvx[4][4], wvy[4][4], wvz[4][4];     // z windows, slot 3 = plane m
-    float nxx[4], nyy[4];                       // vxx, vyy of plane m-1
-    float dxz1[4], dxz2[4], dyz1[4], dyz2[4];   // D+x vz, D+y vz of planes m-1 and m-2
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-#pragma unroll
-        for (int w = 0; w < 4; ++w) wvx[w][c] = wvy[w][c] = wvz[w][c] = 0.0f;
-        nxx[c] = nyy[c] = dxz1[c] = dxz2[c] = dyz1[c] = dyz2[c] = 0.0f;
-    }
+    for (int w = 0; w < 4; ++w) wvx[w] = wvy[w] = wvz[w] = zero;
 
     int s = 0; uint32_t ph = 0;
-    int mr0 = ((m_begin % C::MR) + C::MR) % C::MR;   // ring slot of plane m
+    int mr0 = ((m_begin % MR) + MR) % MR;   // ring slot of plane m
+    uint32_t f1 = 0, f2 = 0;
+    uint32_t fl_next = __ldg(flags + m_begin);
     for (int m = m_begin; m < m_end; ++m) {
+        const uint32_t f0 = fl_next;
+        fl_next = __ldg(flags + min(m + 1, p.nz + 1));
+        const StrPlan v = str_plan(m, kz0, kz1, f0, f1, f2);
+        f2 = f1; f1 = f0;
         mbar_wait(&full[s], ph);
-        const unsigned char *st = stages + s * C::S_STAGE;
-        const float *cvx = reinterpret_cast<const float *>(st + C::S_V) + (ty + 2) * C::AX + 4 + 4 * tx;
+        const unsigned char *st = stages + s * sp.bytes;
+        const int qoff = ty * C::TX + 4 * tx;
+        const float *cvx = reinterpret_cast<const float *>(st + SS::VXB) + (ty + 2) * C::AX + 4 + 4 * tx;
         const float *cvy = cvx + C::C_BYTES / 4;
         const float *cvz = cvy + C::C_BYTES / 4;
-        const float *dbase = reinterpret_cast<const float *>(st + C::S_SR) + ty * C::TX + 4 * tx;
-        const int mr1 = mr0 == 0 ? C::MR - 1 : mr0 - 1;          // plane m-1
-        const int mr2 = mr1 == 0 ? C::MR - 1 : mr1 - 1;          // plane m-2
+        const float *dbase = reinterpret_cast<const float *>(st) + qoff;
+        const int mr1 = mr0 == 0 ? MR - 1 : mr0 - 1;          // plane m-1
+        const int mr2 = mr1 == 0 ? MR - 1 : mr1 - 1;          // plane m-2
         const unsigned char *mat0 = mat_ring + mr0 * C::M_BYTES + ty * C::MX + 4 * tx;
         const unsigned char *mat1 = mat_ring + mr1 * C::M_BYTES + ty * C::MX + 4 * tx;
         const unsigned char *mat2 = mat_ring + mr2 * C::M_BYTES + ty * C::MX + 4 * tx;
-        const bool in0 = (m >= kz0) && (m < kz1);
-        const long long gcell = p.org + i0 + (long long)p.px * j;
 
-        const Row12 rvx = load_row12(cvx), rvy = load_row12(cvy), rvz = load_row12(cvz);
-        float nvxx[4], nvyy[4], ndxz[4], ndyz[4];
-        if (in0) {
-            const float4 vxm = lds4(cvx - C::AX), vxp = lds4(cvx + C::AX), vxpp = lds4(cvx + 2 * C::AX);
-            const float4 vymm = lds4(cvy - 2 * C::AX), vym = lds4(cvy - C::AX), vyp = lds4(cvy + C::AX);
-            const float4 vzm = lds4(cvz - C::AX), vzp = lds4(cvz + C::AX), vzpp = lds4(cvz + 2 * C::AX);
-            const bool plane_ok = true;
-            float ay_i = 0, by_i = 0, ay_h = 0, by_h = 0;
-            if (pc.row_y) {
-                ay_i = __ldg(p.prof[1][0] + j); by_i = __ldg(p.prof[1][1] + j);
-                ay_h = __ldg(p.prof[1][2] + j); by_h = __ldg(p.prof[1][3] + j);
-            }
-            float gxy[4];
+        // ---- slide the z windows and insert plane m ----
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                float vxx = dmx(rvx, c, inv_dx);                                                    // D-x vx
-                float vyy = d4(comp(vymm, c), comp(vym, c), rvy.a[4 + c], comp(vyp, c), inv_dx);    // D-y vy
-                float vx_y = d4(comp(vxm, c), rvx.a[4 + c], comp(vxp, c), comp(vxpp, c), inv_dx);   // D+y vx
-                float vy_x = dpx(rvy, c, inv_dx);                                                   // D+x vy
-                float vz_x = dpx(rvz, c, inv_dx);                                                   // D+x vz
-                float vz_y = d4(comp(vzm, c), rvz.a[4 + c], comp(vzp, c), comp(vzpp, c), inv_dx);   // D+y vz
-                if (plane_ok) {
-                    if (pc.in_x[c]) {
-                        const int i = i0 + c;
-                        const long long q = pc.ix[c] + (long long)p.wx * (j + (long long)p.ny * m);
-                        const float ai = __ldg(p.prof[0][0] + i), bi = __ldg(p.prof[0][1] + i);
-                        const float ah = __ldg(p.prof[0][2] + i), bh = __ldg(p.prof[0][3] + i);
-                        vxx = psi_rmw(p.psi[3], q, ai, bi, vxx);
-                        vy_x = psi_rmw(p.psi[4], q, ah, bh, vy_x);
-                        vz_x = psi_rmw(p.psi[5], q, ah, bh, vz_x);
-                    }
-                    if (pc.row_y && ok[c]) {
-                        const long long q = (i0 + c) + (long long)p.px * (pc.jy + (long long)(2 * P) * m);
-                        vx_y = psi_rmw(p.psi[9], q, ay_h, by_h, vx_y);
-                        vyy = psi_rmw(p.psi[10], q, ay_i, by_i, vyy);
-                        vz_y = psi_rmw(p.psi[11], q, ay_h, by_h, vz_y);
-                    }
-                }
-                nvxx[c] = vxx; nvyy[c] = vyy; ndxz[c] = vz_x; ndyz[c] = vz_y;
-                gxy[c] = vx_y + vy_x;
+        for (int w = 0; w < 3; ++w) { wvx[w] = wvx[w + 1]; wvy[w] = wvy[w + 1]; wvz[w] = wvz[w + 1]; }
+        wvx[3] = q_ld(cvx); wvy[3] = q_ld(cvy); wvz[3] = q_ld(cvz);
+
+        Q4 nvxx = zero, nvyy = zero, ndxz = zero, ndyz = zero;
+        if (v.in0 && g.active) {
+            Q4 vxx = x_dminus(cvx, c1, c2);                                                           // D-x vx
+            Q4 vyy = q_d4(q_ld(cvy - 2 * C::AX), q_ld(cvy - C::AX), wvy[3], q_ld(cvy + C::AX), c1, c2);   // D-y vy
+            Q4 vx_y = zero, vy_x = zero, vz_x = zero, vz_y = zero;
+            if (v.xy0) {
+                vx_y = q_d4(q_ld(cvx - C::AX), wvx[3], q_ld(cvx + C::AX), q_ld(cvx + 2 * C::AX), c1, c2);   // D+y vx
+                vy_x = x_dplus(cvy, c1, c2);                                                          // D+x vy
             }
-            if (in0 && row_ok) {
+            if (v.xz0) vz_x = x_dplus(cvz, c1, c2);                                                   // D+x vz
+            if (v.yz0) vz_y = q_d4(q_ld(cvz - C::AX), wvz[3], q_ld(cvz + C::AX), q_ld(cvz + 2 * C::AX), c1, c2);   // D+y vz
+            if (g.in_x) {
+                const float *sp_x = sprof + 4 * tx;
+                const Q4 ah = q_ld(sp_x + 2 * C::TX), bh = q_ld(sp_x + 3 * C::TX);
+                const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
+                const long long q = g.gx + (long long)p.wx * p.ny * m;
+                q_st(p.psi[3] + q, q_cpml(vxx, q_ld(ps), q_ld(sp_x), q_ld(sp_x + C::TX)));
+                if (v.xy0) q_st(p.psi[4] + q, q_cpml(vy_x, q_ld(ps + sp.xb / 2), ah, bh));
+                if (v.xz0) q_st(p.psi[5] + q, q_cpml(vz_x, q_ld(ps + sp.xb), ah, bh));
+            }
+            if (g.row_y) {
+                const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
+                const long long q = g.gy + (long long)p.px * (2 * p.P) * m;
+                const Q4 ah = q_set(g.ay_h), bh = q_set(g.by_h);
+                if (v.xy0) q_st_n(p.psi[9] + q, q_cpml(vx_y, q_ld(ps), ah, bh), g.nv);
+                q_st_n(p.psi[10] + q, q_cpml(vyy, q_ld(ps + DQ), q_set(g.ay_i), q_set(g.by_i)), g.nv);
+                if (v.yz0) q_st_n(p.psi[11] + q, q_cpml(vz_y, q_ld(ps + 2 * DQ), ah, bh), g.nv);
+            }
+            nvxx = vxx; nvyy = vyy; ndxz = vz_x; ndyz = vz_y;
+            if (v.xy0) {
                 // finish sxy, rxy at plane m: material of the 4 cells (i..i+1, j..j+1, m)
-                const float4 so = lds4(dbase + 6 * (C::D_BYTES / 4)), ro = lds4(dbase + 7 * (C::D_BYTES / 4));
-                float inv_a[5], ts_a[5], inv_b[5], ts_b[5];
+                const Q4 gxy = q_add(vx_y, vy_x);
+                const Q4 so = q_ld(dbase + SS::SXY / 4), ro = q_ld(dbase + SS::RXY / 4);
+                float2 ma[5], mb[5];
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    const KRow &ra = tab[mat0[c]], &rb = tab[mat0[C::MX + c]];
-                    inv_a[c] = ra.invMu; ts_a[c] = ra.tauS; inv_b[c] = rb.invMu; ts_b[c] = rb.tauS;
-                }
+                for (int c = 0; c < 5; ++c) { ma[c] = tabS[mat0[c]]; mb[c] = tabS[mat0[C::MX + c]]; }
                 float os[4], orr[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    const float mu_h = 4.0f / ((inv_a[c] + inv_a[c + 1]) + (inv_b[c] + inv_b[c + 1]));
-                    const float ts_h = 0.25f * ((ts_a[c] + ts_a[c + 1]) + (ts_b[c] + ts_b[c + 1]));
-                    const float r0 = comp(ro, c);
-                    const float rn = fmaf(A, r0, -(B * (mu_h * ts_h) * gxy[c]));
-                    const float sn = comp(so, c) + (dt * (mu_h * (1.0f + ts_h)) * gxy[c] + hdt * (rn + r0));
-                    os[c] = ok[c] ? sn : 0.0f;
-                    orr[c] = ok[c] ? rn : 0.0f;
+                    const ShearCoef k = shear_coef(ma[c], ma[c + 1], mb[c], mb[c + 1], dt, B);
+                    const float r0 = q_get(ro, c), gg = q_get(gxy, c);
+                    const float rn = fmaf(A, r0, -(k.cR * gg));
+                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
+                    orr[c] = rn;
                 }
-                const long long g = gcell + p.sz * m;
-                *reinterpret_cast<float4 *>(p.f[SXY] + g) = make_float4(os[0], os[1], os[2], os[3]);
-                *reinterpret_cast<float4 *>(p.f[RXY] + g) = make_float4(orr[0], orr[1], orr[2], orr[3]);
+                const long long gq = g.gcell + p.sz * m;
+                q_st_n(p.f[SXY] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                q_st_n(p.f[RXY] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
             }
-        } else {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) nvxx[c] = nvyy[c] = ndxz[c] = ndyz[c] = 0.0f;
-        }
-        // slide the z windows and insert plane m
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-#pragma unroll
-            for (int w = 0; w < 3; ++w) { wvx[w][c] = wvx[w + 1][c]; wvy[w][c] = wvy[w + 1][c]; wvz[w][c] = wvz[w + 1][c]; }
-            wvx[3][c] = rvx.a[4 + c]; wvy[3][c] = rvy.a[4 + c]; wvz[3][c] = rvz.a[4 + c];
         }
 
         const int k1 = m - 1, k2 = m - 2;
-        if (k1 >= kz0 && k1 < kz1 && row_ok) {
+        if (v.in1 && g.active) {
             // finish the normal stresses, their memory variables and the sensor at plane k1
-            const bool zs = (P > 0) && (k1 < P || k1 >= p.nz - P);
-            float az = 0, bz = 0;
-            int kz = 0;
-            if (zs) { az = __ldg(p.prof[2][0] + k1); bz = __ldg(p.prof[2][1] + k1); kz = k1 < P ? k1 : k1 - (p.nz - 2 * P); }
-            const float4 s0 = lds4(dbase), s1 = lds4(dbase + (C::D_BYTES / 4)), s2 = lds4(dbase + 2 * (C::D_BYTES / 4));
-            const float4 r0v = lds4(dbase + 3 * (C::D_BYTES / 4)), r1v = lds4(dbase + 4 * (C::D_BYTES / 4)), r2v = lds4(dbase + 5 * (C::D_BYTES / 4));
-            float o[6][4], pr[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                float vzz = d4(wvz[0][c], wvz[1][c], wvz[2][c], wvz[3][c], inv_dx);   // D-z vz at k1
-                if (zs && ok[c]) {
-                    const long long q = (i0 + c) + (long long)p.px * (j + (long long)p.ny * kz);
-                    vzz = psi_rmw(p.psi[17], q, az, bz, vzz);
-                }
-                const KRow row = tab[mat1[c]];
-                const float th = nxx[c] + nyy[c] + vzz;
-                const float vii[3] = {nxx[c], nyy[c], vzz};
-                const float sold[3] = {comp(s0, c), comp(s1, c), comp(s2, c)};
-                const float rold[3] = {comp(r0v, c), comp(r1v, c), comp(r2v, c)};
-                float tr = 0.0f;
+            Q4 vzz = q_d4(wvz[0], wvz[1], wvz[2], wvz[3], c1, c2);   // D-z vz at k1
+            if (z_in_slab(p, k1)) {
+                const float az = __ldg(p.prof[2][0] + k1), bz = __ldg(p.prof[2][1] + k1);
+                const long long qz = g.gz + (long long)p.px * p.ny * z_compact(p, k1);
+                q_st_n(p.psi[17] + qz, q_cpml(vzz, q_ld(reinterpret_cast<const float *>(st + sp.psz + 2 * C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
+            }
+            const uint32_t mw = *reinterpret_cast<const uint32_t *>(mat1);
+            const float4 r0 = tabN[mw & 255u], r1 = tabN[(mw >> 8) & 255u], r2 = tabN[(mw >> 16) & 255u], r3 = tabN[mw >> 24];
+            const Q4 eP = q_make(r0.x, r1.x, r2.x, r3.x), eS = q_make(r0.y, r1.y, r2.y, r3.y);
+            const Q4 th = q_add(q_add(nxx, nyy), vzz);
+            const Q4 ePth = q_mul(eP, th);
+            const Q4 vii[3] = {nxx, nyy, vzz};
+            const long long gq = g.gcell + p.sz * k1;
+            Q4 tr = zero;
+            if (v.rii1) {
+                const Q4 bP = q_make(r0.z, r1.z, r2.z, r3.z), bS = q_make(r0.w, r1.w, r2.w, r3.w);
+                const Q4 bPth = q_mul(bP, th);
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
-                    const float oth = th - vii[q];
-                    const float eU = row.eP * th - row.eS * oth;
-                    const float eR = row.bP * th - row.bS * oth;
-                    const float rn = fmaf(A, rold[q], -eR);
-                    const float sn = sold[q] + (eU + hdt * (rn + rold[q]));
-                    o[q][c] = ok[c] ? sn : 0.0f;
-                    o[3 + q][c] = ok[c] ? rn : 0.0f;
-                    tr += o[q][c];
+                    const Q4 oth = q_sub(th, vii[q]);
+                    const Q4 eU = q_fnma(eS, oth, ePth);
+                    const Q4 eR = q_fnma(bS, oth, bPth);
+                    const Q4 rold = q_ld(dbase + SS::RII / 4 + q * DQ);
+                    const Q4 rn = q_sub(q_muls(rold, A), eR);
+                    const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), q_fmas(hdt, q_add(rn, rold), eU));
+                    q_st_n(p.f[SXX + q] + gq, sn, g.nv);
+                    q_st_n(p.f[RXX + q] + gq, rn, g.nv);
+                    tr = q_add(tr, sn);
                 }
-                pr[c] = (o[0][c] + o[1][c] + o[2][c]) * (-1.0f / 3.0f);
-                (void)tr;
-            }
-            const long long g = gcell + p.sz * k1;
+            } else {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                *reinterpret_cast<float4 *>(p.f[SXX + q] + g) = make_float4(o[q][0], o[q][1], o[q][2], o[q][3]);
-                *reinterpret_cast<float4 *>(p.f[RXX + q] + g) = make_float4(o[3 + q][0], o[3 + q][1], o[3 + q][2], o[3 + q][3]);
+                for (int q = 0; q < 3; ++q) {
+                    const Q4 eU = q_fnma(eS, q_sub(th, vii[q]), ePth);
+                    const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), eU);
+                    q_st_n(p.f[SXX + q] + gq, sn, g.nv);
+                    tr = q_add(tr, sn);
+                }
             }
-            if (sens) {
-                if (p.do_peak) {
-                    const float4 pk = lds4(reinterpret_cast<const float *>(st + C::S_PEAK) + ty * C::TX + 4 * tx);
-                    *reinterpret_cast<float4 *>(p.peak + g) = make_float4(fmaxf(pk.x, fabsf(pr[0])), fmaxf(pk.y, fabsf(pr[1])),
-                                                                          fmaxf(pk.z, fabsf(pr[2])), fmaxf(pk.w, fabsf(pr[3])));
+            if (do_peak | do_rms) {
+                const Q4 pr = q_muls(tr, -1.0f / 3.0f);
+                if (do_peak) {
+                    const Q4 pk = q_ld(dbase + SS::PEAK / 4);
+                    q_st_n(p.peak + gq, q_make(fmaxf(pk.a.x, fabsf(pr.a.x)), fmaxf(pk.a.y, fabsf(pr.a.y)),
+                                               fmaxf(pk.b.x, fabsf(pr.b.x)), fmaxf(pk.b.y, fabsf(pr.b.y))), g.nv);
                 }
-                if (p.do_rms) {
-                    const float4 sq = lds4(reinterpret_cast<const float *>(st + C::S_SUMSQ) + ty * C::TX + 4 * tx);
-                    *reinterpret_cast<float4 *>(p.sumsq + g) = make_float4(fmaf(pr[0], pr[0], sq.x), fmaf(pr[1], pr[1], sq.y),
-                                                                           fmaf(pr[2], pr[2], sq.z), fmaf(pr[3], pr[3], sq.w));
-                }
+                if (do_rms) q_st_n(p.sumsq + gq, q_fma(pr, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
             }
         }
-        if (k2 >= kz0 && k2 < kz1 && row_ok) {
+        if ((v.xz2 | v.yz2) && g.active) {
             // finish sxz, syz (+ r) at plane k2: D+z of vx, vy over planes m-3..m
-            const bool zs = (P > 0) && (k2 < P || k2 >= p.nz - P);
-            float az = 0, bz = 0;
-            int kz = 0;
-            if (zs) { az = __ldg(p.prof[2][2] + k2); bz = __ldg(p.prof[2][3] + k2); kz = k2 < P ? k2 : k2 - (p.nz - 2 * P); }
-            const float4 sxz_o = lds4(dbase + 8 * (C::D_BYTES / 4)), rxz_o = lds4(dbase + 9 * (C::D_BYTES / 4));
-            const float4 syz_o = lds4(dbase + 10 * (C::D_BYTES / 4)), ryz_o = lds4(dbase + 11 * (C::D_BYTES / 4));
+            const bool zs = z_in_slab(p, k2);
+            float az = 0.0f, bz = 0.0f;
+            long long qz = 0;
+            if (zs) { az = __ldg(p.prof[2][2] + k2); bz = __ldg(p.prof[2][3] + k2); qz = g.gz + (long long)p.px * p.ny * z_compact(p, k2); }
+            const long long gq = g.gcell + p.sz * k2;
             // materials: row j at planes k2 (mat2) and k2+1 (mat1), cells i0..i0+4; row j+1 cells i0..i0+3
-            float inv_2[5], ts_2[5], inv_1[5], ts_1[5], inv_2b[4], ts_2b[4], inv_1b[4], ts_1b[4];
+            float2 m2[5], m1[5];
 #pragma unroll
-            for (int c = 0; c < 5; ++c) {
-                const KRow &ra = tab[mat2[c]], &rb = tab[mat1[c]];
-                inv_2[c] = ra.invMu; ts_2[c] = ra.tauS; inv_1[c] = rb.invMu; ts_1[c] = rb.tauS;
-            }
+            for (int c = 0; c < 5; ++c) { m2[c] = tabS[mat2[c]]; m1[c] = tabS[mat1[c]]; }
+            if (v.xz2) {
+                Q4 vx_z = q_d4(wvx[0], wvx[1], wvx[2], wvx[3], c1, c2);   // D+z vx at k2
+                if (zs) q_st_n(p.psi[15] + qz, q_cpml(vx_z, q_ld(reinterpret_cast<const float *>(st + sp.psz) + qoff), q_set(az), q_set(bz)), g.nv);
+                const Q4 gg4 = q_add(vx_z, dxz2);
+                const Q4 so = q_ld(dbase + SS::SXZ / 4), ro = q_ld(dbase + SS::RXZ / 4);
+                float os[4], orr[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const KRow &ra = tab[mat2[C::MX + c]], &rb = tab[mat1[C::MX + c]];
-                inv_2b[c] = ra.invMu; ts_2b[c] = ra.tauS; inv_1b[c] = rb.invMu; ts_1b[c] = rb.tauS;
+                for (int c = 0; c < 4; ++c) {   // cells (i..i+1, j, k2..k2+1)
+                    const ShearCoef k = shear_coef(m2[c], m2[c + 1], m1[c], m1[c + 1], dt, B);
+                    const float r0 = q_get(ro, c), gg = q_get(gg4, c);
+                    const float rn = fmaf(A, r0, -(k.cR * gg));
+                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
+                    orr[c] = rn;
+                }
+                q_st_n(p.f[SXZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                q_st_n(p.f[RXZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
             }
-            float oxz[4], orxz[4], oyz[4], oryz[4];
+            if (v.yz2) {
+                Q4 vy_z = q_d4(wvy[0], wvy[1], wvy[2], wvy[3], c1, c2);   // D+z vy at k2
+                if (zs) q_st_n(p.psi[16] + qz, q_cpml(vy_z, q_ld(reinterpret_cast<const float *>(st + sp.psz + C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
+                const Q4 gg4 = q_add(vy_z, dyz2);
+                const Q4 so = q_ld(dbase + SS::SYZ / 4), ro = q_ld(dbase + SS::RYZ / 4);
+                float os[4], orr[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                float vx_z = d4(wvx[0][c], wvx[1][c], wvx[2][c], wvx[3][c], inv_dx);   // D+z vx at k2
-                float vy_z = d4(wvy[0][c], wvy[1][c], wvy[2][c], wvy[3][c], inv_dx);   // D+z vy at k2
-                if (zs && ok[c]) {
-                    const long long q = (i0 + c) + (long long)p.px * (j + (long long)p.ny * kz);
-                    vx_z = psi_rmw(p.psi[15], q, az, bz, vx_z);
-                    vy_z = psi_rmw(p.psi[16], q, az, bz, vy_z);
+                for (int c = 0; c < 4; ++c) {   // cells (i, j..j+1, k2..k2+1)
+                    const ShearCoef k = shear_coef(m2[c], tabS[mat2[C::MX + c]], m1[c], tabS[mat1[C::MX + c]], dt, B);
+                    const float r0 = q_get(ro, c), gg = q_get(gg4, c);
+                    const float rn = fmaf(A, r0, -(k.cR * gg));
+                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
+                    orr[c] = rn;
                 }
-                {   // sxz: cells (i..i+1, j, k2..k2+1)
-                    const float mu_h = 4.0f / ((inv_2[c] + inv_2[c + 1]) + (inv_1[c] + inv_1[c + 1]));
-                    const float ts_h = 0.25f * ((ts_2[c] + ts_2[c + 1]) + (ts_1[c] + ts_1[c + 1]));
-                    const float gg = vx_z + dxz2[c];
-                    const float r0 = comp(rxz_o, c);
-                    const float rn = fmaf(A, r0, -(B * (mu_h * ts_h) * gg));
-                    const float sn = comp(sxz_o, c) + (dt * (mu_h * (1.0f + ts_h)) * gg + hdt * (rn + r0));
-                    oxz[c] = ok[c] ? sn : 0.0f; orxz[c] = ok[c] ? rn : 0.0f;
-                }
-                {   // syz: cells (i, j..j+1, k2..k2+1)
-                    const float mu_h = 4.0f / ((inv_2[c] + inv_2b[c]) + (inv_1[c] + inv_1b[c]));
-                    const float ts_h = 0.25f * ((ts_2[c] + ts_2b[c]) + (ts_1[c] + ts_1b[c]));
-                    const float gg = vy_z + dyz2[c];
-                    const float r0 = comp(ryz_o, c);
-                    const float rn = fmaf(A, r0, -(B * (mu_h * ts_h) * gg));
-                    const float sn = comp(syz_o, c) + (dt * (mu_h * (1.0f + ts_h)) * gg + hdt * (rn + r0));
-                    oyz[c] = ok[c] ? sn : 0.0f; oryz[c] = ok[c] ? rn : 0.0f;
-                }
+                q_st_n(p.f[SYZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                q_st_n(p.f[RYZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
             }
-            const long long g = gcell + p.sz * k2;
-            *reinterpret_cast<float4 *>(p.f[SXZ] + g) = make_float4(oxz[0], oxz[1], oxz[2], oxz[3]);
-            *reinterpret_cast<float4 *>(p.f[RXZ] + g) = make_float4(orxz[0], orxz[1], orxz[2], orxz[3]);
-            *reinterpret_cast<float4 *>(p.f[SYZ] + g) = make_float4(oyz[0], oyz[1], oyz[2], oyz[3]);
-            *reinterpret_cast<float4 *>(p.f[RYZ] + g) = make_float4(oryz[0], oryz[1], oryz[2], oryz[3]);
         }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            nxx[c] = nvxx[c]; nyy[c] = nvyy[c];
-            dxz2[c] = dxz1[c]; dxz1[c] = ndxz[c];
-            dyz2[c] = dyz1[c]; dyz1[c] = ndyz[c];
-        }
+        nxx = nvxx; nyy = nvyy;
+        dxz2 = dxz1; dxz1 = ndxz;
+        dyz2 = dyz1; dyz1 = ndyz;
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&empty[s]);
-        if (++s == C::NS) { s = 0; ph ^= 1; }
-        if (++mr0 == C::MR) mr0 = 0;
+        if (++s == sp.ns) { s = 0; ph ^= 1; }
+        if (++mr0 == MR) mr0 = 0;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// S0 on the device: tile-class flags from the index map
+// ------------------------------------------------------------------------------------------
+// One CTA per (tile, plane).  solid(m) = mu_R > 0; a shear node is "solid" when its four cells are
+// (reading P2; out-of-grid neighbours are the replicated edge of the private index map).
+template <class C>
+__global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__restrict__ flagsV, uint32_t *__restrict__ flagsS, const int dense) {
+    __shared__ uint32_t sv, ss;
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, k = blockIdx.z;
+    if (threadIdx.x == 0) { sv = 0; ss = 0; }
+    __syncthreads();
+    uint32_t fv = 0, fs = 0;
+    if (dense) {
+        fv = TF_XY | TF_XZ | TF_YZ; fs = TF_XY | TF_XZ | TF_YZ | TF_RII;
+    } else {
+        constexpr int EX = C::TX + 4, EY = C::TY + 4;
+        for (int q = threadIdx.x; q < EX * EY; q += blockDim.x) {
+            const int i = x0 - 2 + q % EX, j = y0 - 2 + q / EX;
+            if (i < 0 || j < 0 || i >= p.nx || j >= p.ny) continue;
+            const uint8_t *mp = p.mat + i + (long long)p.px * j + p.sz * k;
+            const KRow r000 = p.rows[mp[0]];
+            const float s000 = r000.solid, s100 = p.rows[mp[1]].solid, s010 = p.rows[mp[p.px]].solid, s110 = p.rows[mp[p.px + 1]].solid;
+            const float s001 = p.rows[mp[p.sz]].solid, s101 = p.rows[mp[p.sz + 1]].solid, s011 = p.rows[mp[p.sz + p.px]].solid;
+            const bool nxy = s000 * s100 * s010 * s110 != 0.0f;
+            const bool nxz = s000 * s100 * s001 * s101 != 0.0f;
+            const bool nyz = s000 * s010 * s001 * s011 != 0.0f;
+            const bool inx = i >= x0 && i < x0 + C::TX, iny = j >= y0 && j < y0 + C::TY;
+            if (nxy) fv |= TF_XY;
+            if (nxz && iny) fv |= TF_XZ;
+            if (nyz && inx) fv |= TF_YZ;
+            if (inx && iny) {
+                if (nxy) fs |= TF_XY;
+                if (nxz) fs |= TF_XZ;
+                if (nyz) fs |= TF_YZ;
+                if (r000.bP != 0.0f || r000.bS != 0.0f) fs |= TF_RII;
+            }
+        }
+    }
+    if (fv) atomicOr(&sv, fv);
+    if (fs) atomicOr(&ss, fs);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const size_t o = (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2 + k;
+        flagsV[o] = sv; flagsS[o] = ss;
     }
 }
 
@@ -742,7 +966,25 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p) {
+inline int round128(int v) { return (v + 127) / 128 * 128; }
+
+// z chunks: fill the resident CTA slots in as few waves as possible
+inline void plan_chunks(const Layout &L, long long slots, int &chunks, int &nzc) {
+    const long long tiles = (long long)L.ntx * L.nty;
+    int best = 1;
+    double best_cost = 1e300;
+    for (int ch = 1; ch <= (L.nz + 7) / 8; ++ch) {
+        const int n = (L.nz + ch - 1) / ch;
+        const long long blocks = tiles * ((L.nz + n - 1) / n);
+        const double waves = (double)((blocks + slots - 1) / slots);
+        const double cost = waves * (n + 4);
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = ch; }
+    }
+    nzc = (L.nz + best - 1) / best;
+    chunks = (L.nz + nzc - 1) / nzc;
+}
+
+inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p, char *const psi_base[3], const long long psi_stride[3]) {
     using C = Cfg;
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -753,79 +995,125 @@ inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p) 
         return BVFDTD_ECUDA;
     }
     PFN_encodeTiled enc = (PFN_encodeTiled)fn;
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    auto encode = [&](CUtensorMap *m, CUtensorMapDataType ty, int rank, void *base, const cuuint64_t *gdim, const cuuint64_t *gstr,
+                      const cuuint32_t *box, const char *what) -> int {
+        CUresult r = enc(m, ty, rank, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled(%s) failed: %d", what, (int)r);
+            return BVFDTD_ECUDA;
+        }
+        return 0;
+    };
     // the 17 grid arrays (15 state + peak + sumsq) are laid out back to back at a constant stride
     const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
     for (int q = 0; q < NSTATE; ++q)
         if ((const char *)p.f[q] - (const char *)p.f[0] != fstride * q) return BVFDTD_EINVAL;
     if ((const char *)p.peak - (const char *)p.f[0] != fstride * F_PEAK) return BVFDTD_EINVAL;
     if ((const char *)p.sumsq - (const char *)p.f[0] != fstride * F_SUMSQ) return BVFDTD_EINVAL;
-    void *base = (void *)(p.f[0] + (L.org - 2 * L.sz));      // cell (0,0,-2)
-    const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), 17};
-    const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    struct { CUtensorMap *m; cuuint32_t bx, by; } boxes[4] = {
-        {&plan.maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&plan.maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
-        {&plan.maps.boxC, (cuuint32_t)C::AX, (cuuint32_t)C::BY}, {&plan.maps.boxD, (cuuint32_t)C::TX, (cuuint32_t)C::TY}};
-    for (auto &b : boxes) {
-        const cuuint32_t box[4] = {b.bx, b.by, 1, 1};
-        CUresult r = enc(b.m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) {
-            std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled(float box %ux%u) failed: %d", b.bx, b.by, (int)r);
-            return BVFDTD_ECUDA;
+    {
+        void *base = (void *)(p.f[0] + (L.org - 2 * L.sz));      // cell (0,0,-2)
+        const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), 17};
+        const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
+        struct { CUtensorMap *m; cuuint32_t bx, by; } boxes[4] = {
+            {&plan.maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&plan.maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
+            {&plan.maps.boxC, (cuuint32_t)C::AX, (cuuint32_t)C::BY}, {&plan.maps.boxD, (cuuint32_t)C::TX, (cuuint32_t)C::TY}};
+        for (auto &b : boxes) {
+            const cuuint32_t box[4] = {b.bx, b.by, 1, 1};
+            if (int rc = encode(b.m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, gdim, gstr, box, "field box")) return rc;
         }
     }
     {
         const cuuint64_t mdim[3] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 1)};
         const cuuint64_t mstr[2] = {(cuuint64_t)L.px, (cuuint64_t)L.sz};
         const cuuint32_t mbox[3] = {(cuuint32_t)C::MX, (cuuint32_t)C::MY, 1};
-        CUresult r = enc(&plan.maps.mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)p.mat, mdim, mstr, mbox, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) {
-            std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled(material box) failed: %d", (int)r);
-            return BVFDTD_ECUDA;
+        if (int rc = encode(&plan.maps.mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)p.mat, mdim, mstr, mbox, "material box")) return rc;
+    }
+    const int wxb = L.P > 0 ? std::min(L.xph, C::TX) : 4;
+    if (L.P > 0) {
+        {   // x slabs: (wx, ny, nz, 6)
+            const cuuint64_t d[4] = {(cuuint64_t)L.wx, (cuuint64_t)L.ny, (cuuint64_t)L.nz, 6};
+            const cuuint64_t s[3] = {(cuuint64_t)L.wx * 4, (cuuint64_t)L.wx * L.ny * 4, (cuuint64_t)psi_stride[0]};
+            const cuuint32_t b[4] = {(cuuint32_t)wxb, (cuuint32_t)C::TY, 1, 1};
+            if (int rc = encode(&plan.maps.psx, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[0], d, s, b, "psi x box")) return rc;
+        }
+        {   // y slabs: (px, 2P, nz, 6)
+            const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)(2 * L.P), (cuuint64_t)L.nz, 6};
+            const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * 2 * L.P * 4, (cuuint64_t)psi_stride[1]};
+            const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::TY, 1, 1};
+            if (int rc = encode(&plan.maps.psy, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[1], d, s, b, "psi y box")) return rc;
+        }
+        {   // z slabs: (px, ny, 2P, 6)
+            const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)L.ny, (cuuint64_t)(2 * L.P), 6};
+            const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * L.ny * 4, (cuuint64_t)psi_stride[2]};
+            const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::TY, 1, 1};
+            if (int rc = encode(&plan.maps.psz, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[2], d, s, b, "psi z box")) return rc;
         }
     }
-    e = cudaFuncSetAttribute(k_velocity_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::V_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::S_SMEM);
+    // stage plans
+    auto make_stage = [&](int fixed, int ns, int extra) {
+        StagePlan s;
+        s.wxb = wxb;
+        s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
+        s.psx = fixed;
+        s.psy = s.psx + 3 * 2 * s.xb;
+        s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
+        s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
+        s.ns = ns;
+        s.smem = ns * s.bytes + extra;
+        return s;
+    };
+    const int bar_bytes = 2 * MAX_STAGES * 8;
+    const int v_extra = 256 * 4 + 4 * C::TX * 4 + bar_bytes;
+    int dev = 0, sms = 148, smem_max = 227 * 1024;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const char *env_v = std::getenv("BVFDTD_NS_V"), *env_s = std::getenv("BVFDTD_NS_S");
+    int ns_v = env_v ? std::atoi(env_v) : 2, ns_s = env_s ? std::atoi(env_s) : 3;
+    ns_v = std::max(2, std::min(MAX_STAGES, ns_v));
+    ns_s = std::max(2, std::min(MAX_STAGES, ns_s));
+    plan.sv = make_stage(VStage<C>::FIXED, ns_v, v_extra);
+    auto s_extra = [&](int ns) { return (ns + 3) * C::M_BYTES + 256 * 16 + 256 * 8 + 4 * C::TX * 4 + bar_bytes; };
+    plan.ss = make_stage(SStage<C>::FIXED, ns_s, s_extra(ns_s));
+    while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage(SStage<C>::FIXED, plan.ss.ns - 1, s_extra(plan.ss.ns - 1));
+    while (plan.sv.smem > smem_max && plan.sv.ns > 2) plan.sv = make_stage(VStage<C>::FIXED, plan.sv.ns - 1, v_extra);
+    if (plan.ss.smem > smem_max || plan.sv.smem > smem_max) {
+        std::snprintf(tiled_err_buf(), 256, "pml %d needs %d bytes of shared memory per CTA (max %d)", L.P, plan.ss.smem, smem_max);
+        return BVFDTD_EINVAL;
+    }
+    e = cudaFuncSetAttribute(k_velocity_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
+    int occ_v = 1, occ_s = 1;
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<C>, C::NT, plan.sv.smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_stress_tiled<C>, C::NT, plan.ss.smem);
     if (e != cudaSuccess) {
-        std::snprintf(tiled_err_buf(), 256, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        std::snprintf(tiled_err_buf(), 256, "kernel attribute/occupancy query: %s", cudaGetErrorString(e));
         (void)cudaGetLastError();
         return BVFDTD_ECUDA;
     }
-    // z chunks: fill the resident CTA slots (2 per SM) in as few waves as possible
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long tiles = (long long)((L.nx + C::TX - 1) / C::TX) * ((L.ny + C::TY - 1) / C::TY);
-    const long long slots = 2LL * sms;
-    int best = 1;
-    double best_cost = 1e300;
-    for (int ch = 1; ch <= (L.nz + 7) / 8; ++ch) {
-        const int nzc = (L.nz + ch - 1) / ch;
-        const long long blocks = tiles * ((L.nz + nzc - 1) / nzc);
-        const double waves = (double)((blocks + slots - 1) / slots);
-        const double cost = waves * (nzc + 4);
-        if (cost < best_cost - 1e-9) { best_cost = cost; best = ch; }
-    }
-    plan.nzc = (L.nz + best - 1) / best;
-    plan.chunks = (L.nz + plan.nzc - 1) / plan.nzc;
+    plan_chunks(L, (long long)std::max(1, occ_v) * sms, plan.chunks_v, plan.nzc_v);
+    plan_chunks(L, (long long)std::max(1, occ_s) * sms, plan.chunks_s, plan.nzc_s);
+    if (std::getenv("BVFDTD_VERBOSE"))
+        std::fprintf(stderr, "[bvfdtd] velocity: ns %d stage %d smem %d occ %d chunks %d x %d planes; stress: ns %d stage %d smem %d occ %d chunks %d x %d planes\n",
+                     plan.sv.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.chunks_v, plan.nzc_v, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s,
+                     plan.chunks_s, plan.nzc_s);
     plan.ready = true;
     return 0;
 }
 
 inline void tiled_plan_destroy(TiledPlan &plan) { plan.ready = false; }
 
-inline dim3 tiled_grid(const TiledPlan &plan, const Params &p) {
-    return dim3((p.nx + Cfg::TX - 1) / Cfg::TX, (p.ny + Cfg::TY - 1) / Cfg::TY, plan.chunks);
+inline void tiled_flags(const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st) {
+    k_tile_flags<Cfg><<<dim3(p.ntx, p.nty, p.nz), 128, 0, st>>>(p, flagsV, flagsS, dense ? 1 : 0);
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_velocity_tiled<Cfg><<<tiled_grid(plan, p), Cfg::NT, Cfg::V_SMEM, st>>>(plan.maps, p, plan.nzc);
+    k_velocity_tiled<Cfg><<<dim3(p.ntx, p.nty, plan.chunks_v), Cfg::NT, plan.sv.smem, st>>>(plan.maps, p, plan.nzc_v, plan.sv);
     return 0;
 }
 inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_stress_tiled<Cfg><<<tiled_grid(plan, p), Cfg::NT, Cfg::S_SMEM, st>>>(plan.maps, p, plan.nzc);
+    k_stress_tiled<Cfg><<<dim3(p.ntx, p.nty, plan.chunks_s), Cfg::NT, plan.ss.smem, st>>>(plan.maps, p, plan.nzc_s, plan.ss);
     return 0;
 }
 

@@ -360,6 +360,38 @@ def random_domain(nx, ny, nz, pml, seed, n_mat=6, solid_fraction=0.5, lossy=True
                     n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
 
 
+def blocky_domain(nx, ny, nz, pml, seed, steps=20, waveform=1, f0=500e3, dx=1e-3 / 3.0) -> Workload:
+    """Mostly lossless water with a few box-shaped inclusions (lossy solids, one lossy fluid, one
+    lossless solid) whose faces are not aligned with the 64 x 8 tiles and of which one runs into
+    the PML slabs: the layout that exercises the tile-class skipping of the tiled kernels
+    (all-fluid tile-planes next to partly solid ones, lossless next to lossy)."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 3000 + seed))
+    table = np.array([WATER,
+                      (1900.0, 2800.0, 1500.0, 200.0, 200.0),     # lossy solid
+                      (1040.0, 1546.0, 0.0, 30.0, 0.0),           # lossy fluid
+                      (1700.0, 2500.0, 1300.0, 0.0, 0.0),         # lossless solid
+                      (2100.0, 3100.0, 1700.0, 80.0, 160.0)], dtype=np.float64)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    idx = np.zeros((nz, ny, nx), dtype=np.uint8)
+    dims = np.array([nz, ny, nx])
+    for b in range(6):
+        lo = np.array([rng.integers(0, max(1, d - 4)) for d in dims])
+        ext = np.array([rng.integers(2, max(3, d // 2)) for d in dims])
+        hi = np.minimum(dims, lo + ext)
+        idx[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] = 1 + b % 4
+    idx[:, :3, :] = np.where(idx[:, :3, :] == 0, 4, idx[:, :3, :]) if seed % 2 else idx[:, :3, :]
+    lo = pml
+    ci = rng.integers(lo, nx - lo, size=6)
+    cj = rng.integers(lo, ny - lo, size=6)
+    ck = rng.integers(lo, nz - lo, size=6)
+    cells = np.unique((ci + nx * (cj + ny * ck)).astype(np.int64))
+    amp = (0.5 + rng.random(cells.size)).astype(np.float32)
+    delay = (rng.random(cells.size) * 0.5 / f0).astype(np.float32)
+    return Workload(f"blocky_{nx}x{ny}x{nz}_p{pml}_s{seed}", nx, ny, nz, pml, dx, dt, f0, spp,
+                    steps, table, idx, cells, amp, delay, waveform=waveform, f_src=f0,
+                    n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
+
+
 def random_state(w: Workload, seed: int, scale_v: float = 1e-6) -> dict:
     """Seeded random state for single-pass parity tests: 3 v, 6 sigma, 6 r as float32 arrays
     shaped (nz, ny, nx) (values exactly representable in fp32 so both sides start equal)."""

@@ -83,7 +83,7 @@ def run_both(bv, w, steps=None, flags=0, state=None):
 # ---------------------------------------------------------------------------------------------
 # construction parity (bit-exact)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 def test_construction_bit_exact(bv, flags):
     w = wl.random_domain(37, 29, 41, 4, seed=1)
     sim = bv.Simulation.from_workload(w, flags=flags)
@@ -124,7 +124,7 @@ def test_write_read_round_trip(bv):
 # kernel-level parity: one full step from a seeded random state (v after the step checks S2 in
 # isolation, sigma/r check S3 given S2), on ragged grids that span several tiles
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 @pytest.mark.parametrize("dims,P", [((37, 29, 41), 4), ((72, 40, 24), 8), ((24, 24, 24), 0),
                                     ((131, 21, 19), 2), ((40, 70, 33), 12)])
 def test_single_step_random_state(bv, dims, P, flags):
@@ -138,7 +138,7 @@ def test_single_step_random_state(bv, dims, P, flags):
     sim.close()
 
 
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 @pytest.mark.parametrize("kind", ["all_fluid", "all_solid", "single_lossy_voxel", "lossless"])
 def test_degenerate_media(bv, kind, flags):
     w = wl.random_domain(36, 28, 30, 6, seed=20, lossy=(kind != "lossless"))
@@ -171,7 +171,7 @@ def test_degenerate_media(bv, kind, flags):
 # ---------------------------------------------------------------------------------------------
 # time-stepped parity with source, PML and sensors on small random domains
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 @pytest.mark.parametrize("dims,P,wave", [((45, 38, 50), 6, 0), ((64, 33, 37), 5, 1), ((30, 30, 30), 0, 0)])
 def test_stepped_random_domain(bv, dims, P, wave, flags):
     w = wl.random_domain(*dims, P, seed=30 + P, steps=120, waveform=wave)
@@ -182,6 +182,29 @@ def test_stepped_random_domain(bv, dims, P, wave, flags):
     compare_map(rms, o.get("rms_amp"))
     assert sim.step_index == 120
     sim.close()
+
+
+@pytest.mark.parametrize("dims,P,seed", [((150, 43, 38), 6, 1), ((70, 30, 61), 5, 2), ((64, 64, 40), 8, 3)])
+def test_tile_class_skipping(bv, dims, P, seed):
+    """Mostly-fluid, partly lossless domains: the default path skips the shear stresses and memory
+    variables of tile-planes where they are identically zero.  It must match the oracle AND be
+    bit-identical to the dense sweep (adding the skipped zeros changes nothing)."""
+    w = wl.blocky_domain(*dims, P, seed=seed, steps=60)
+    st = wl.random_state(w, 8)
+    st = {n: st[n] for n in ("vx", "vy", "vz", "sxx", "syy", "szz")}     # shear stresses and r start at 0
+    sim, o = run_both(bv, w, state=st)
+    compare_state(sim, o, rel=2e-5)
+    peak, rms = sim.read_peak_pressure()
+    compare_map(peak, o.get("peak"), rel=1e-4)
+    compare_map(rms, o.get("rms_amp"), rel=1e-4)
+    dense, _ = run_both(bv, w, state=st, flags=bv.FLAG_DENSE, steps=0)
+    dense.step(w.steps)
+    for n in bv.FIELDS:
+        assert np.array_equal(sim.read_fields(n), dense.read_fields(n)), n
+    pk2, rms2 = dense.read_peak_pressure()
+    assert np.array_equal(peak, pk2) and np.array_equal(rms, rms2)
+    sim.close()
+    dense.close()
 
 
 def test_sensor_windows(bv):
@@ -203,7 +226,7 @@ def test_sensor_windows(bv):
 # ---------------------------------------------------------------------------------------------
 # the configs of BASELINE.json
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2])
 def test_config0_full(bv, flags):
     w = wl.make(0)
     sim, o = run_both(bv, w, flags=flags)
