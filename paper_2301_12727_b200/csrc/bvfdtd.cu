@@ -39,7 +39,8 @@ bool grid_ok(const bvfdtd_grid *g) {
     if (!g || g->pml < 0) return false;
     const long long lim = 2LL * g->pml + 8;
     if (g->nx < lim || g->ny < lim || g->nz < lim) return false;
-    if ((long long)g->nx * g->ny * g->nz > (1LL << 40)) return false;
+    // the kernels address a field with 32-bit float offsets: keep a padded field under 2^31 floats
+    if ((long long)(g->nx + 34) * (g->ny + 2) * (g->nz + 6) >= (1LL << 31)) return false;
     return g->nx <= 65535 * 16 && g->ny <= 65535 && g->nz <= 65535;
 }
 
@@ -56,9 +57,12 @@ Layout make_layout(const bvfdtd_grid &g) {
     L.xhb = (g.nx - g.pml) & ~3;
     L.xph = (int)round_up(g.nx - L.xhb, 4);
     L.wx = L.xp4 + L.xph;
-    L.ntx = (g.nx + Cfg::TX - 1) / Cfg::TX;
-    L.nty = (g.ny + Cfg::TY - 1) / Cfg::TY;
-    L.flag_words = round_up((long long)L.ntx * L.nty * (g.nz + 4), 64);
+    L.ntxV = (g.nx + CfgV::TX - 1) / CfgV::TX;
+    L.ntyV = (g.ny + CfgV::TY - 1) / CfgV::TY;
+    L.ntxS = (g.nx + CfgS::TX - 1) / CfgS::TX;
+    L.ntyS = (g.ny + CfgS8::TY - 1) / CfgS8::TY;   // sized for the smaller stress tile; the plan fixes the real count
+    L.flag_wordsV = round_up((long long)L.ntxV * L.ntyV * (g.nz + 4), 64);
+    L.flag_wordsS = round_up((long long)L.ntxS * L.ntyS * (g.nz + 4), 64);
     L.psi_floats[0] = round_up((long long)L.wx * g.ny * g.nz, 64);
     L.psi_floats[1] = round_up((long long)L.px * (2 * g.pml) * g.nz, 64);
     L.psi_floats[2] = round_up((long long)L.px * g.ny * (2 * g.pml), 64);
@@ -84,8 +88,8 @@ WsMap make_wsmap(const Layout &L) {
         for (int t = 0; t < 6; ++t) w.psi[a * 6 + t] = take(L.psi_floats[a] * 4);
     w.rows = take(256 * sizeof(KRow));
     w.prof = take((size_t)4 * (L.nx + L.ny + L.nz) * 4);
-    w.flagsV = take((size_t)L.flag_words * 4);
-    w.flagsS = take((size_t)L.flag_words * 4);
+    w.flagsV = take((size_t)L.flag_wordsV * 4);
+    w.flagsS = take((size_t)L.flag_wordsS * 4);
     w.total = off;
     return w;
 }
@@ -334,7 +338,8 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     Params &p = c->prm;
     p.nx = L.nx; p.ny = L.ny; p.nz = L.nz; p.P = L.P;
     p.px = L.px; p.py = L.py; p.wx = L.wx; p.sz = L.sz; p.org = L.org;
-    p.xp4 = L.xp4; p.xhb = L.xhb; p.xph = L.xph; p.ntx = L.ntx; p.nty = L.nty;
+    p.xp4 = L.xp4; p.xhb = L.xhb; p.xph = L.xph;
+    p.ntxV = L.ntxV; p.ntyV = L.ntyV; p.ntxS = L.ntxS; p.ntyS = L.ntyS;
     p.flagsV = (const uint32_t *)(c->ws + c->W.flagsV);
     p.flagsS = (const uint32_t *)(c->ws + c->W.flagsS);
     for (int q = 0; q < NSTATE; ++q) p.f[q] = (float *)(c->ws + c->W.field[q]);
@@ -366,7 +371,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
         rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
         c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;
-        tiled_flags(c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);
+        tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(c->stream));
     }
@@ -510,7 +515,7 @@ int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_
         // a caller-supplied shear stress or memory variable may be non-zero where the tile-class
         // flags assume it is identically zero: switch this context to the dense sweep
         c->dense = true;
-        tiled_flags(c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), true, c->stream);
+        tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), true, c->stream);
         CU(cudaGetLastError());
     }
     if (!src_is_device) CU(cudaStreamSynchronize(c->stream));

@@ -27,15 +27,15 @@ struct Layout {
                               // at xp4 + (i - xhb), xhb = floor4(nx - P), width xph = round_up(nx - xhb, 4)
     int wx;                   // x pitch of the x-slab psi arrays = xp4 + xph
     long long psi_floats[3];  // floats per psi array of axis x, y, z
-    int ntx, nty;             // x-y tiles of the tiled kernels
-    long long flag_words;     // uint32 words per flag table: ntx * nty * (nz + 4)
+    int ntxV, ntyV, ntxS, ntyS;   // x-y tiles of the velocity / stress kernels
+    long long flag_wordsV, flag_wordsS;   // uint32 words per flag table: tiles * (nz + 4)
 };
 
 struct Params {
     int nx, ny, nz, P;
     int px, py, wx;
     int xp4, xhb, xph;     // x-slab compact index: i < P ? i : xp4 + (i - xhb)
-    int ntx, nty;
+    int ntxV, ntyV, ntxS, ntyS;
     long long sz, org;
     float *f[NSTATE];
     float *peak, *sumsq;

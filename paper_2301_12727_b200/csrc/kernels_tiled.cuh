@@ -57,7 +57,9 @@ struct TileCfg {
     static_assert(NC % 32 == 0, "whole consumer warps");
 };
 
-using Cfg = TileCfg<64, 8>;
+using CfgV = TileCfg<64, 8>;    // velocity pass: 4 consumer warps, 2 CTAs per SM
+using CfgS = TileCfg<64, 16>;   // stress pass: 8 consumer warps, 1 CTA per SM
+using CfgS8 = TileCfg<64, 8>;   // stress pass fallback when the 64 x 16 stages do not fit (very thick PML on a narrow grid)
 
 struct TiledMaps {
     CUtensorMap boxA, boxB, boxC, boxD;   // 4-D (x, y, z+2, field) fp32 maps over the 17 grid arrays
@@ -65,10 +67,22 @@ struct TiledMaps {
     CUtensorMap psx, psy, psz;            // 4-D (x, y, z, array) maps over the slab-compact psi arrays
 };
 
+// What the producer tells the consumers about one stage (written before the stage's barrier is
+// armed): the iteration's load/compute plan and the z-profile coefficients of the two planes the
+// iteration finishes (a, b at the integer node of plane m-1 and at the half node of plane m-2).
+struct StageHdr {
+    uint32_t ctrl, pad[3];
+    float az1, bz1, az2, bz2;
+};
+
 // Shared-memory plan of one pipeline stage (byte offsets inside the stage), fixed per context.
 struct StagePlan {
+    int hdr;               // per-stage header written by the producer (StageHdr)
     int psx, psy, psz;     // first psi slot of each axis (3 slots per axis)
-    int xb;                // bytes of one x-psi box (low or high slab); one slot = 2 boxes
+    int yb;                // bytes of one y- or z-psi box (= the tile's D box)
+    int xb;                // bytes of one x-psi box (low or high slab)
+    int xhi, xt;           // byte offset of the high-slab box inside a term slot (0 when no tile touches both
+                           // slabs), bytes of one term slot
     int wxb;               // x-psi box width in floats
     int bytes;             // stage size (multiple of 128)
     int ns;                // pipeline stages
@@ -76,8 +90,9 @@ struct StagePlan {
 };
 
 struct TiledPlan {
-    TiledMaps maps;
+    TiledMaps mv, ms;      // velocity / stress pass (their tiles differ)
     StagePlan sv, ss;
+    bool s16 = true;       // stress pass runs 64 x 16 tiles (else 64 x 8)
     int chunks_v = 1, nzc_v = 0, chunks_s = 1, nzc_s = 0;
     bool ready = false;
 };
@@ -196,6 +211,23 @@ __device__ __forceinline__ float rcp_newton(float x) {
     return fmaf(r, fmaf(-x, r, 1.0f), r);
 }
 
+// z-direction 4-point difference as an accumulator chain: when plane m arrives it is the last (+c2)
+// plane of one output, the +c1 plane of the next, the -c1 plane of the one after and the first
+// (-c2) plane of a new one.  Three accumulators per array replace a four-plane register window and
+// need no register moves.  The completed output is the D- difference at plane m-1 (array on half
+// nodes in z) or, equally, the D+ difference at plane m-2 (array on integer nodes in z).
+struct ZChain {
+    Q4 a1, a2, a3;
+};
+__device__ __forceinline__ void zc_clear(ZChain &c) { c.a1 = c.a2 = c.a3 = q_set(0.0f); }
+__device__ __forceinline__ Q4 zc_push(ZChain &c, const Q4 &f, float c1, float c2) {
+    const Q4 out = q_fmas(c2, f, c.a1);
+    c.a1 = q_fmas(c1, f, c.a2);
+    c.a2 = q_fmas(-c1, f, c.a3);
+    c.a3 = q_muls(f, -c2);
+    return out;
+}
+
 // ------------------------------------------------------------------------------------------
 // per-thread geometry shared by both passes
 // ------------------------------------------------------------------------------------------
@@ -206,9 +238,8 @@ struct ThreadGeom {
     bool in_x;                   // quad touches an x slab
     bool row_y;                  // row in a y slab
     int psx_off;                 // float offset of the quad inside an x-psi slot (low or high box)
-    long long gx, gy;            // global float offset of the quad inside an x-/y-psi array at plane 0
-    long long gz;                // ... inside a z-psi array at compact plane 0
-    long long gcell;             // global float offset of the quad inside a grid field at plane 0
+    uint32_t gx, gy, gz;         // float offset of the quad inside an x- / y- / z-psi array at (compact) plane 0
+    uint32_t gcell;              // float offset of the quad inside a grid field at plane 0
     float ay_i, by_i, ay_h, by_h;
 };
 
@@ -225,14 +256,14 @@ __device__ __forceinline__ ThreadGeom<C> make_geom(const Params &p, const StageP
     g.in_x = in_lo || in_hi;
     // low box is loaded at compact x = x0, high box at compact x = xp4 + max(x0, xhb) - xhb
     const int hi0 = max(x0, p.xhb);
-    g.psx_off = in_lo ? (g.ty * sp.wxb + (g.i0 - x0)) : (sp.xb / 4 + g.ty * sp.wxb + (g.i0 - hi0));
+    g.psx_off = in_lo ? (g.ty * sp.wxb + (g.i0 - x0)) : (sp.xhi / 4 + g.ty * sp.wxb + (g.i0 - hi0));
     const int cx = in_lo ? g.i0 : p.xp4 + (g.i0 - p.xhb);
-    g.gx = cx + (long long)p.wx * g.j;
+    g.gx = (uint32_t)(cx + p.wx * g.j);
     g.row_y = g.active && P > 0 && (g.j < P || g.j >= p.ny - P);
     const int jy = g.j < P ? g.j : g.j - (p.ny - 2 * P);
-    g.gy = g.i0 + (long long)p.px * jy;
-    g.gz = g.i0 + (long long)p.px * g.j;
-    g.gcell = p.org + g.i0 + (long long)p.px * g.j;
+    g.gy = (uint32_t)(g.i0 + p.px * jy);
+    g.gz = (uint32_t)(g.i0 + p.px * g.j);
+    g.gcell = (uint32_t)(p.org + g.i0 + (long long)p.px * g.j);
     g.ay_i = g.by_i = g.ay_h = g.by_h = 0.0f;
     if (g.row_y) {
         g.ay_i = __ldg(p.prof[1][0] + g.j); g.by_i = __ldg(p.prof[1][1] + g.j);
@@ -271,6 +302,12 @@ __device__ __forceinline__ int tile_jy0(const Params &p, int y0) { return y0 < p
 __device__ __forceinline__ bool z_in_slab(const Params &p, int k) { return p.P > 0 && k >= 0 && k < p.nz && (k < p.P || k >= p.nz - p.P); }
 __device__ __forceinline__ int z_compact(const Params &p, int k) { return k < p.P ? k : k - (p.nz - 2 * p.P); }
 
+// the store of a quad: EDGE CTAs may hold partial quads (nx % 4 != 0)
+template <bool EDGE>
+__device__ __forceinline__ void q_store(float *g, const Q4 &q, int nv) {
+    if (EDGE) q_st_n(g, q, nv); else q_st(g, q);
+}
+
 // ------------------------------------------------------------------------------------------
 // S2: velocity pass
 // ------------------------------------------------------------------------------------------
@@ -283,26 +320,153 @@ struct VStage {
                          FIXED = MAT + C::M_BYTES;
 };
 
-// What iteration m of the velocity pass loads and computes: derived identically by producer and
-// consumers from the chunk range and the flag words of planes m-3..m.
-struct VelPlan {
-    bool in0, in1, in2;    // plane m / m-1 / m-2 inside the chunk
-    bool xy, xz, yz;       // plane m carries non-zero sxy / sxz / syz (in the halo-extended tile)
-    bool wxz, wyz;         // some plane of the z window m-3..m carries non-zero sxz / syz
+// control word of one velocity iteration (StageHdr::ctrl)
+enum : uint32_t {
+    VC_IN0 = 1u, VC_IN1 = 2u, VC_IN2 = 4u,   // plane m / m-1 / m-2 inside the chunk
+    VC_XY = 8u, VC_XZ = 16u, VC_YZ = 32u,    // plane m carries non-zero sxy / sxz / syz (halo-extended tile)
+    VC_WXZ = 64u, VC_WYZ = 128u,             // some plane of m-3..m carries non-zero sxz / syz
+    VC_ZS1 = 256u, VC_ZS2 = 512u             // plane m-1 / m-2 lies in a z slab (and inside the chunk)
 };
-__device__ __forceinline__ VelPlan vel_plan(int m, int kz0, int kz1, uint32_t fl, uint32_t &hist_xz, uint32_t &hist_yz) {
-    VelPlan v;
-    v.in0 = m >= kz0 && m < kz1;
-    v.in1 = m - 1 >= kz0 && m - 1 < kz1;
-    v.in2 = m - 2 >= kz0 && m - 2 < kz1;
-    v.xy = (fl & TF_XY) != 0;
-    v.xz = (fl & TF_XZ) != 0;
-    v.yz = (fl & TF_YZ) != 0;
-    hist_xz = ((hist_xz << 1) | (v.xz ? 1u : 0u)) & 15u;
-    hist_yz = ((hist_yz << 1) | (v.yz ? 1u : 0u)) & 15u;
-    v.wxz = hist_xz != 0;
-    v.wyz = hist_yz != 0;
-    return v;
+
+template <class C, bool EDGE>
+__device__ __forceinline__ void velocity_consume(const Params &p, const StagePlan &sp, unsigned char *stages, const float *rho_tab,
+                                                 const float *sprof, uint64_t *full, uint64_t *empty, int tid, int x0, int y0,
+                                                 int m_begin, int m_end) {
+    using VS = VStage<C>;
+    constexpr int DQ = C::D_BYTES / 4;
+    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
+    const int tx = g.tx, ty = g.ty;
+    const bool active = EDGE ? g.active : true;
+    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
+    const float dt2 = 2.0f * p.dt;
+    const bool wall_x = EDGE && g.active && (p.nx - 1 >= g.i0) && (p.nx - 1 <= g.i0 + 3);   // quad holds cell nx-1 (P4)
+    const bool wall_y = EDGE && g.j == p.ny - 1;
+    const Q4 zero = q_set(0.0f);
+    const int qoff = ty * C::TX + 4 * tx;             // own quad inside a D / B(row 0) box
+    const int aoff = ty * C::AX + 4 + 4 * tx;         // own quad inside an A / C(row 0) box
+    const uint32_t zstride = (uint32_t)(p.px * p.ny);
+
+    ZChain zxz, zyz, zzz;                             // D-z sxz, D-z syz (finish at m-1), D+z szz (finish at m-2)
+    zc_clear(zxz); zc_clear(zyz); zc_clear(zzz);
+    Q4 pvx = zero, pvy = zero, pvz1 = zero, pvz2 = zero;   // x-y sums of planes m-1 (pvx, pvy, pvz1) and m-2 (pvz2)
+    float rho_prev[4] = {1.0f, 1.0f, 1.0f, 1.0f};          // rho of the thread's cells at plane m-2
+
+    uint32_t goff = g.gcell + (uint32_t)(p.sz * m_begin);              // field offset of the quad at plane m
+    uint32_t gxo = g.gx + (uint32_t)(p.wx * p.ny) * (uint32_t)m_begin; // x-psi offset at plane m
+    uint32_t gyo = g.gy + (uint32_t)(p.px * 2 * p.P) * (uint32_t)m_begin;
+    int s = 0; uint32_t ph = 0;
+    for (int m = m_begin; m < m_end; ++m) {
+        mbar_wait(&full[s], ph);
+        const unsigned char *st = stages + s * sp.bytes;
+        const StageHdr *hdr = reinterpret_cast<const StageHdr *>(st + sp.hdr);
+        const uint32_t ctrl = hdr->ctrl;
+        if (active) {
+            const float *sA_xz = reinterpret_cast<const float *>(st + VS::SXZ) + aoff;
+            const float *sB_yz = reinterpret_cast<const float *>(st + VS::SYZ) + qoff;     // row j-2
+            const float *psz = reinterpret_cast<const float *>(st + sp.psz) + qoff;
+            // ---- z chains: push plane m ----
+            Q4 dzz = zc_push(zzz, q_ld(reinterpret_cast<const float *>(st + VS::SZZ) + qoff), c1, c2);
+            Q4 dzx = zero, dzy = zero;
+            if (ctrl & VC_WXZ) dzx = zc_push(zxz, (ctrl & VC_XZ) ? q_ld(sA_xz) : zero, c1, c2);
+            if (ctrl & VC_WYZ) dzy = zc_push(zyz, (ctrl & VC_YZ) ? q_ld(sB_yz + 2 * C::TX) : zero, c1, c2);
+
+            // ---- material of plane m-1: rho at i0..i0+4 of row j and i0..i0+3 of row j+1 ----
+            const unsigned char *mt = st + VS::MAT + ty * C::MX + 4 * tx;
+            float rho_j[5], rho_j1[4];
+            {
+                const uint32_t w0 = *reinterpret_cast<const uint32_t *>(mt);
+                const uint32_t w1 = *reinterpret_cast<const uint32_t *>(mt + C::MX);
+                rho_j[4] = rho_tab[mt[4]];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    rho_j[c] = rho_tab[(w0 >> (8 * c)) & 255u];
+                    rho_j1[c] = rho_tab[(w1 >> (8 * c)) & 255u];
+                }
+            }
+            if (ctrl & VC_IN1) {
+                // finish vx, vy at plane m-1
+                if (ctrl & VC_ZS1) {
+                    const uint32_t qz = g.gz + zstride * (uint32_t)z_compact(p, m - 1);
+                    const Q4 az = q_set(hdr->az1), bz = q_set(hdr->bz1);
+                    if (ctrl & VC_WXZ) q_store<EDGE>(p.psi[12] + qz, q_cpml(dzx, q_ld(psz), az, bz), g.nv);
+                    if (ctrl & VC_WYZ) q_store<EDGE>(p.psi[13] + qz, q_cpml(dzy, q_ld(psz + DQ), az, bz), g.nv);
+                }
+                const Q4 cx = q_make(dt2 * rcp_newton(rho_j[0] + rho_j[1]), dt2 * rcp_newton(rho_j[1] + rho_j[2]),
+                                     dt2 * rcp_newton(rho_j[2] + rho_j[3]), dt2 * rcp_newton(rho_j[3] + rho_j[4]));
+                const Q4 cy = q_make(dt2 * rcp_newton(rho_j[0] + rho_j1[0]), dt2 * rcp_newton(rho_j[1] + rho_j1[1]),
+                                     dt2 * rcp_newton(rho_j[2] + rho_j1[2]), dt2 * rcp_newton(rho_j[3] + rho_j1[3]));
+                Q4 ox = q_fma(cx, q_add(pvx, dzx), q_ld(reinterpret_cast<const float *>(st + VS::VXO) + qoff));
+                Q4 oy = q_fma(cy, q_add(pvy, dzy), q_ld(reinterpret_cast<const float *>(st + VS::VYO) + qoff));
+                if (EDGE) {
+                    if (wall_x) {
+                        const int wc = p.nx - 1 - g.i0;
+                        if (wc == 0) ox.a.x = 0.0f; else if (wc == 1) ox.a.y = 0.0f; else if (wc == 2) ox.b.x = 0.0f; else ox.b.y = 0.0f;
+                    }
+                    if (wall_y) oy = zero;
+                }
+                const uint32_t gq = goff - (uint32_t)p.sz;
+                q_store<EDGE>(p.f[VX] + gq, ox, g.nv);
+                q_store<EDGE>(p.f[VY] + gq, oy, g.nv);
+            }
+            if (ctrl & VC_IN2) {
+                // finish vz at plane m-2
+                if (ctrl & VC_ZS2) {
+                    const uint32_t qz = g.gz + zstride * (uint32_t)z_compact(p, m - 2);
+                    q_store<EDGE>(p.psi[14] + qz, q_cpml(dzz, q_ld(psz + 2 * DQ), q_set(hdr->az2), q_set(hdr->bz2)), g.nv);
+                }
+                const Q4 cz = q_make(dt2 * rcp_newton(rho_prev[0] + rho_j[0]), dt2 * rcp_newton(rho_prev[1] + rho_j[1]),
+                                     dt2 * rcp_newton(rho_prev[2] + rho_j[2]), dt2 * rcp_newton(rho_prev[3] + rho_j[3]));
+                Q4 oz = q_fma(cz, q_add(pvz2, dzz), q_ld(reinterpret_cast<const float *>(st + VS::VZO) + qoff));
+                if (m - 2 == p.nz - 1) oz = zero;
+                q_store<EDGE>(p.f[VZ] + (goff - 2u * (uint32_t)p.sz), oz, g.nv);
+            }
+            pvz2 = pvz1;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) rho_prev[c] = rho_j[c];
+
+            // ---- x-y derivative sums of plane m ----
+            if (ctrl & VC_IN0) {
+                const float *sA_xx = reinterpret_cast<const float *>(st + VS::SXX) + aoff;
+                const float *sB_yy = reinterpret_cast<const float *>(st + VS::SYY) + qoff;   // row j-1
+                Q4 dxx = x_dplus(sA_xx, c1, c2);                                             // D+x sxx -> vx
+                Q4 dyy = q_d4(q_ld(sB_yy), q_ld(sB_yy + C::TX), q_ld(sB_yy + 2 * C::TX), q_ld(sB_yy + 3 * C::TX), c1, c2);   // D+y syy -> vy
+                Q4 dxy_y = zero, dxy_x = zero, dxz = zero, dyz = zero;
+                if (ctrl & VC_XY) {
+                    const float *sC = reinterpret_cast<const float *>(st + VS::SXY) + aoff;  // row j-2
+                    dxy_x = x_dminus(sC + 2 * C::AX, c1, c2);                                // D-x sxy -> vy
+                    dxy_y = q_d4(q_ld(sC), q_ld(sC + C::AX), q_ld(sC + 2 * C::AX), q_ld(sC + 3 * C::AX), c1, c2);   // D-y sxy -> vx
+                }
+                if (ctrl & VC_XZ) dxz = x_dminus(sA_xz, c1, c2);                             // D-x sxz -> vz
+                if (ctrl & VC_YZ) dyz = q_d4(q_ld(sB_yz), q_ld(sB_yz + C::TX), q_ld(sB_yz + 2 * C::TX), q_ld(sB_yz + 3 * C::TX), c1, c2);   // D-y syz -> vz
+                if (g.in_x) {
+                    const float *sp_x = sprof + 4 * tx;
+                    const Q4 ai = q_ld(sp_x), bi = q_ld(sp_x + C::TX);
+                    const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
+                    q_st(p.psi[0] + gxo, q_cpml(dxx, q_ld(ps), q_ld(sp_x + 2 * C::TX), q_ld(sp_x + 3 * C::TX)));
+                    if (ctrl & VC_XY) q_st(p.psi[1] + gxo, q_cpml(dxy_x, q_ld(ps + sp.xt / 4), ai, bi));
+                    if (ctrl & VC_XZ) q_st(p.psi[2] + gxo, q_cpml(dxz, q_ld(ps + sp.xt / 2), ai, bi));
+                }
+                if (g.row_y) {
+                    const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
+                    const Q4 ai = q_set(g.ay_i), bi = q_set(g.by_i);
+                    if (ctrl & VC_XY) q_store<EDGE>(p.psi[6] + gyo, q_cpml(dxy_y, q_ld(ps), ai, bi), g.nv);
+                    q_store<EDGE>(p.psi[7] + gyo, q_cpml(dyy, q_ld(ps + DQ), q_set(g.ay_h), q_set(g.by_h)), g.nv);
+                    if (ctrl & VC_YZ) q_store<EDGE>(p.psi[8] + gyo, q_cpml(dyz, q_ld(ps + 2 * DQ), ai, bi), g.nv);
+                }
+                pvx = q_add(dxx, dxy_y);
+                pvy = q_add(dxy_x, dyy);
+                pvz1 = q_add(dxz, dyz);
+            } else {
+                pvx = pvy = pvz1 = zero;
+            }
+        }
+        goff += (uint32_t)p.sz;
+        gxo += (uint32_t)(p.wx * p.ny);
+        gyo += (uint32_t)(p.px * 2 * p.P);
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&empty[s]);
+        if (++s == sp.ns) { s = 0; ph ^= 1; }
+    }
 }
 
 template <class C>
@@ -320,7 +484,6 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
     const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
     const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
-    const uint32_t *flags = p.flagsV + (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2;
 
     for (int q = tid; q < 256; q += C::NT) rho_tab[q] = p.rows[q].rho;
     fill_xprof<C>(sprof, p, x0, tid);
@@ -331,69 +494,84 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
     }
     __syncthreads();
 
-    const TileX tX = make_tilex<C>(p, x0);
-    const bool tY = tile_in_y<C>(p, y0);
-    const int jy0 = tile_jy0<C>(p, y0);
-
     if (tid >= C::NC) {
         // ================= producer warp =================
         if (tid == C::NC) {
+            const uint32_t *flags = p.flagsV + (size_t)(blockIdx.x + p.ntxV * blockIdx.y) * (p.nz + 4) + 2;
+            const TileX tX = make_tilex<C>(p, x0);
+            const bool tY = tile_in_y<C>(p, y0);
+            const int jy0 = tile_jy0<C>(p, y0);
             prefetch_tmap(&maps.boxA); prefetch_tmap(&maps.boxB); prefetch_tmap(&maps.boxC);
             prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
             uint32_t hxz = 0, hyz = 0;
             const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
+            const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
+            uint32_t fl_next = __ldg(flags + m_begin);
             for (int m = m_begin; m < m_end; ++m) {
-                const VelPlan v = vel_plan(m, kz0, kz1, __ldg(flags + m), hxz, hyz);
+                const uint32_t fl = fl_next;
+                fl_next = __ldg(flags + min(m + 1, p.nz + 1));
+                const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
+                const bool xy = (fl & TF_XY) != 0, xz = (fl & TF_XZ) != 0, yz = (fl & TF_YZ) != 0;
+                hxz = ((hxz << 1) | (xz ? 1u : 0u)) & 15u;
+                hyz = ((hyz << 1) | (yz ? 1u : 0u)) & 15u;
+                const bool wxz = hxz != 0, wyz = hyz != 0;
+                const bool zs1 = in1 && z_in_slab(p, m - 1), zs2 = in2 && z_in_slab(p, m - 2);
+                StageHdr h;
+                h.ctrl = (in0 ? VC_IN0 : 0u) | (in1 ? VC_IN1 : 0u) | (in2 ? VC_IN2 : 0u) | (xy ? VC_XY : 0u) | (xz ? VC_XZ : 0u) |
+                         (yz ? VC_YZ : 0u) | (wxz ? VC_WXZ : 0u) | (wyz ? VC_WYZ : 0u) | (zs1 ? VC_ZS1 : 0u) | (zs2 ? VC_ZS2 : 0u);
+                h.az1 = h.bz1 = h.az2 = h.bz2 = 0.0f;
+                if (zs1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
+                if (zs2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
                 mbar_wait(&empty[s], ph ^ 1);
                 unsigned char *st = stages + s * sp.bytes;
                 uint64_t *bar = &full[s];
-                const bool zs1 = v.in1 && z_in_slab(p, m - 1), zs2 = v.in2 && z_in_slab(p, m - 2);
-                const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
+                StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
+                hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
                 uint32_t bytes = C::D_BYTES + C::MX * C::MY;                       // szz, mat
-                if (v.xz) bytes += C::A_BYTES;
-                if (v.yz) bytes += C::B_BYTES;
-                if (v.in0) {
-                    bytes += C::A_BYTES + C::B_BYTES + (v.xy ? C::C_BYTES : 0);
-                    bytes += nx_boxes * xbox * (1u + (v.xy ? 1u : 0u) + (v.xz ? 1u : 0u));
-                    if (tY) bytes += C::D_BYTES * (1u + (v.xy ? 1u : 0u) + (v.yz ? 1u : 0u));
+                if (xz) bytes += C::A_BYTES;
+                if (yz) bytes += C::B_BYTES;
+                if (in0) {
+                    bytes += C::A_BYTES + C::B_BYTES + (xy ? C::C_BYTES : 0);
+                    bytes += nx_boxes * xbox * (1u + (xy ? 1u : 0u) + (xz ? 1u : 0u));
+                    if (tY) bytes += C::D_BYTES * (1u + (xy ? 1u : 0u) + (yz ? 1u : 0u));
                 }
-                if (v.in1) bytes += 2 * C::D_BYTES;
-                if (v.in2) bytes += C::D_BYTES;
-                if (zs1) bytes += C::D_BYTES * ((v.wxz ? 1u : 0u) + (v.wyz ? 1u : 0u));
+                if (in1) bytes += 2 * C::D_BYTES;
+                if (in2) bytes += C::D_BYTES;
+                if (zs1) bytes += C::D_BYTES * ((wxz ? 1u : 0u) + (wyz ? 1u : 0u));
                 if (zs2) bytes += C::D_BYTES;
                 mbar_expect_tx(bar, bytes);
                 const int z = m + 2;
                 tma_load_4d(st + VS::SZZ, &maps.boxD, bar, x0, y0, z, SZZ);
-                if (v.xz) tma_load_4d(st + VS::SXZ, &maps.boxA, bar, x0 - 4, y0, z, SXZ);
-                if (v.yz) tma_load_4d(st + VS::SYZ, &maps.boxB, bar, x0, y0 - 2, z, SYZ);
-                if (v.in0) {
+                if (xz) tma_load_4d(st + VS::SXZ, &maps.boxA, bar, x0 - 4, y0, z, SXZ);
+                if (yz) tma_load_4d(st + VS::SYZ, &maps.boxB, bar, x0, y0 - 2, z, SYZ);
+                if (in0) {
                     tma_load_4d(st + VS::SXX, &maps.boxA, bar, x0 - 4, y0, z, SXX);
                     tma_load_4d(st + VS::SYY, &maps.boxB, bar, x0, y0 - 1, z, SYY);
-                    if (v.xy) tma_load_4d(st + VS::SXY, &maps.boxC, bar, x0 - 4, y0 - 2, z, SXY);
+                    if (xy) tma_load_4d(st + VS::SXY, &maps.boxC, bar, x0 - 4, y0 - 2, z, SXY);
                     // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
-                    const bool use[3] = {true, v.xy, v.xz};
-                    const bool usey[3] = {v.xy, true, v.yz};
+                    const bool use[3] = {true, xy, xz};
+                    const bool usey[3] = {xy, true, yz};
 #pragma unroll
                     for (int t = 0; t < 3; ++t) {
                         if (use[t]) {
-                            unsigned char *d = st + sp.psx + t * 2 * sp.xb;
+                            unsigned char *d = st + sp.psx + t * sp.xt;
                             if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, t);
-                            if (tX.hi) tma_load_4d(d + sp.xb, &maps.psx, bar, tX.cx_hi, y0, m, t);
+                            if (tX.hi) tma_load_4d(d + sp.xhi, &maps.psx, bar, tX.cx_hi, y0, m, t);
                         }
                         if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, t);
                     }
                 }
-                if (v.in1) {
+                if (in1) {
                     tma_load_4d(st + VS::VXO, &maps.boxD, bar, x0, y0, z - 1, VX);
                     tma_load_4d(st + VS::VYO, &maps.boxD, bar, x0, y0, z - 1, VY);
                 }
-                if (v.in2) tma_load_4d(st + VS::VZO, &maps.boxD, bar, x0, y0, z - 2, VZ);
+                if (in2) tma_load_4d(st + VS::VZO, &maps.boxD, bar, x0, y0, z - 2, VZ);
                 if (zs1) {
                     const int kc = z_compact(p, m - 1);
-                    if (v.wxz) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, kc, 0);
-                    if (v.wyz) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, kc, 1);
+                    if (wxz) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, kc, 0);
+                    if (wyz) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, kc, 1);
                 }
                 if (zs2) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 2);
                 tma_load_3d(st + VS::MAT, &maps.mat, bar, x0, y0, m - 1);
@@ -404,147 +582,9 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
     }
 
     // ================= consumers =================
-    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
-    const int tx = g.tx, ty = g.ty;
-    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
-    const float dt2 = 2.0f * p.dt;
-    const bool wall_x = g.active && (p.nx - 1 >= g.i0) && (p.nx - 1 <= g.i0 + 3);   // quad holds cell nx-1 (P4)
-    const bool wall_y = g.j == p.ny - 1;
-    const Q4 zero = q_set(0.0f);
-
-    Q4 wxz[4], wyz[4], wzz[4];                 // z windows: slot 3 = plane m ... slot 0 = plane m-3
-    Q4 pvx = zero, pvy = zero, pvz1 = zero, pvz2 = zero;   // x-y sums of planes m-1 (pvx, pvy, pvz1) and m-2 (pvz2)
-    float rho_prev[4] = {1.0f, 1.0f, 1.0f, 1.0f};          // rho of the thread's cells at plane m-2
-#pragma unroll
-    for (int w = 0; w < 4; ++w) wxz[w] = wyz[w] = wzz[w] = zero;
-
-    int s = 0; uint32_t ph = 0;
-    uint32_t hxz = 0, hyz = 0;
-    uint32_t fl_next = __ldg(flags + m_begin);
-    for (int m = m_begin; m < m_end; ++m) {
-        const uint32_t fl = fl_next;
-        fl_next = __ldg(flags + min(m + 1, p.nz + 1));
-        const VelPlan v = vel_plan(m, kz0, kz1, fl, hxz, hyz);
-        mbar_wait(&full[s], ph);
-        const unsigned char *st = stages + s * sp.bytes;
-        const int qoff = ty * C::TX + 4 * tx;             // own quad inside a D / B(row 0) box
-        const int aoff = ty * C::AX + 4 + 4 * tx;         // own quad inside an A / C(row 0) box
-        const float *sD = reinterpret_cast<const float *>(st + VS::SZZ) + qoff;
-
-        // ---- z windows: slide and insert plane m ----
-#pragma unroll
-        for (int w = 0; w < 3; ++w) { wxz[w] = wxz[w + 1]; wyz[w] = wyz[w + 1]; wzz[w] = wzz[w + 1]; }
-        wzz[3] = q_ld(sD);
-        const float *sA_xz = reinterpret_cast<const float *>(st + VS::SXZ) + aoff;
-        const float *sB_yz = reinterpret_cast<const float *>(st + VS::SYZ) + qoff;     // row j-2
-        wxz[3] = v.xz ? q_ld(sA_xz) : zero;
-        wyz[3] = v.yz ? q_ld(sB_yz + 2 * C::TX) : zero;
-
-        // ---- x-y derivative sums of plane m ----
-        Q4 nvx = zero, nvy = zero, nvz = zero;
-        if (v.in0 && g.active) {
-            const float *sA_xx = reinterpret_cast<const float *>(st + VS::SXX) + aoff;
-            const float *sB_yy = reinterpret_cast<const float *>(st + VS::SYY) + qoff;   // row j-1
-            Q4 dxx = x_dplus(sA_xx, c1, c2);                                             // D+x sxx -> vx
-            Q4 dyy = q_d4(q_ld(sB_yy), q_ld(sB_yy + C::TX), q_ld(sB_yy + 2 * C::TX), q_ld(sB_yy + 3 * C::TX), c1, c2);   // D+y syy -> vy
-            Q4 dxy_y = zero, dxy_x = zero, dxz = zero, dyz = zero;
-            if (v.xy) {
-                const float *sC = reinterpret_cast<const float *>(st + VS::SXY) + aoff;  // row j-2
-                dxy_x = x_dminus(sC + 2 * C::AX, c1, c2);                                // D-x sxy -> vy
-                dxy_y = q_d4(q_ld(sC), q_ld(sC + C::AX), q_ld(sC + 2 * C::AX), q_ld(sC + 3 * C::AX), c1, c2);   // D-y sxy -> vx
-            }
-            if (v.xz) dxz = x_dminus(sA_xz, c1, c2);                                     // D-x sxz -> vz
-            if (v.yz) dyz = q_d4(q_ld(sB_yz), q_ld(sB_yz + C::TX), q_ld(sB_yz + 2 * C::TX), q_ld(sB_yz + 3 * C::TX), c1, c2);   // D-y syz -> vz
-            if (g.in_x) {
-                const float *sp_x = sprof + 4 * tx;
-                const Q4 ai = q_ld(sp_x), bi = q_ld(sp_x + C::TX), ah = q_ld(sp_x + 2 * C::TX), bh = q_ld(sp_x + 3 * C::TX);
-                const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
-                const long long q = g.gx + (long long)p.wx * p.ny * m;
-                q_st(p.psi[0] + q, q_cpml(dxx, q_ld(ps), ah, bh));
-                if (v.xy) q_st(p.psi[1] + q, q_cpml(dxy_x, q_ld(ps + sp.xb / 2), ai, bi));
-                if (v.xz) q_st(p.psi[2] + q, q_cpml(dxz, q_ld(ps + sp.xb), ai, bi));
-            }
-            if (g.row_y) {
-                const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
-                const long long q = g.gy + (long long)p.px * (2 * p.P) * m;
-                const Q4 ai = q_set(g.ay_i), bi = q_set(g.by_i);
-                if (v.xy) q_st_n(p.psi[6] + q, q_cpml(dxy_y, q_ld(ps), ai, bi), g.nv);
-                q_st_n(p.psi[7] + q, q_cpml(dyy, q_ld(ps + C::D_BYTES / 4), q_set(g.ay_h), q_set(g.by_h)), g.nv);
-                if (v.yz) q_st_n(p.psi[8] + q, q_cpml(dyz, q_ld(ps + 2 * (C::D_BYTES / 4)), ai, bi), g.nv);
-            }
-            nvx = q_add(dxx, dxy_y);
-            nvy = q_add(dxy_x, dyy);
-            nvz = q_add(dxz, dyz);
-        }
-
-        // ---- material of plane m-1: rho at i0..i0+4 of row j and i0..i0+3 of row j+1 ----
-        const unsigned char *mt = st + VS::MAT + ty * C::MX + 4 * tx;
-        float rho_j[5], rho_j1[4];
-        {
-            const uint32_t w0 = *reinterpret_cast<const uint32_t *>(mt);
-            const uint32_t w1 = *reinterpret_cast<const uint32_t *>(mt + C::MX);
-            rho_j[4] = rho_tab[mt[4]];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                rho_j[c] = rho_tab[(w0 >> (8 * c)) & 255u];
-                rho_j1[c] = rho_tab[(w1 >> (8 * c)) & 255u];
-            }
-        }
-
-        const int k1 = m - 1, k2 = m - 2;
-        if (v.in1 && g.active) {
-            // finish vx, vy at plane k1: D-z of sxz / syz over planes m-3..m
-            Q4 sx = pvx, sy = pvy;
-            const bool zs = z_in_slab(p, k1);
-            float az = 0.0f, bz = 0.0f;
-            long long qz = 0;
-            if (zs) { az = __ldg(p.prof[2][0] + k1); bz = __ldg(p.prof[2][1] + k1); qz = g.gz + (long long)p.px * p.ny * z_compact(p, k1); }
-            if (v.wxz) {
-                Q4 dzx = q_d4(wxz[0], wxz[1], wxz[2], wxz[3], c1, c2);
-                if (zs) q_st_n(p.psi[12] + qz, q_cpml(dzx, q_ld(reinterpret_cast<const float *>(st + sp.psz) + qoff), q_set(az), q_set(bz)), g.nv);
-                sx = q_add(sx, dzx);
-            }
-            if (v.wyz) {
-                Q4 dzy = q_d4(wyz[0], wyz[1], wyz[2], wyz[3], c1, c2);
-                if (zs) q_st_n(p.psi[13] + qz, q_cpml(dzy, q_ld(reinterpret_cast<const float *>(st + sp.psz + C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
-                sy = q_add(sy, dzy);
-            }
-            const Q4 cx = q_make(dt2 * rcp_newton(rho_j[0] + rho_j[1]), dt2 * rcp_newton(rho_j[1] + rho_j[2]),
-                                 dt2 * rcp_newton(rho_j[2] + rho_j[3]), dt2 * rcp_newton(rho_j[3] + rho_j[4]));
-            const Q4 cy = q_make(dt2 * rcp_newton(rho_j[0] + rho_j1[0]), dt2 * rcp_newton(rho_j[1] + rho_j1[1]),
-                                 dt2 * rcp_newton(rho_j[2] + rho_j1[2]), dt2 * rcp_newton(rho_j[3] + rho_j1[3]));
-            Q4 ox = q_fma(cx, sx, q_ld(reinterpret_cast<const float *>(st + VS::VXO) + qoff));
-            Q4 oy = q_fma(cy, sy, q_ld(reinterpret_cast<const float *>(st + VS::VYO) + qoff));
-            if (wall_x) {
-                const int wc = p.nx - 1 - g.i0;
-                if (wc == 0) ox.a.x = 0.0f; else if (wc == 1) ox.a.y = 0.0f; else if (wc == 2) ox.b.x = 0.0f; else ox.b.y = 0.0f;
-            }
-            if (wall_y) oy = zero;
-            const long long gq = g.gcell + p.sz * k1;
-            q_st_n(p.f[VX] + gq, ox, g.nv);
-            q_st_n(p.f[VY] + gq, oy, g.nv);
-        }
-        if (v.in2 && g.active) {
-            // finish vz at plane k2: D+z of szz over planes m-3..m
-            Q4 dzz = q_d4(wzz[0], wzz[1], wzz[2], wzz[3], c1, c2);
-            if (z_in_slab(p, k2)) {
-                const float az = __ldg(p.prof[2][2] + k2), bz = __ldg(p.prof[2][3] + k2);
-                const long long qz = g.gz + (long long)p.px * p.ny * z_compact(p, k2);
-                q_st_n(p.psi[14] + qz, q_cpml(dzz, q_ld(reinterpret_cast<const float *>(st + sp.psz + 2 * C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
-            }
-            const Q4 cz = q_make(dt2 * rcp_newton(rho_prev[0] + rho_j[0]), dt2 * rcp_newton(rho_prev[1] + rho_j[1]),
-                                 dt2 * rcp_newton(rho_prev[2] + rho_j[2]), dt2 * rcp_newton(rho_prev[3] + rho_j[3]));
-            Q4 oz = q_fma(cz, q_add(pvz2, dzz), q_ld(reinterpret_cast<const float *>(st + VS::VZO) + qoff));
-            if (k2 == p.nz - 1) oz = zero;
-            q_st_n(p.f[VZ] + g.gcell + p.sz * k2, oz, g.nv);
-        }
-        pvz2 = pvz1; pvz1 = nvz; pvx = nvx; pvy = nvy;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) rho_prev[c] = rho_j[c];
-        __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty[s]);
-        if (++s == sp.ns) { s = 0; ph ^= 1; }
-    }
+    const bool edge = (x0 + C::TX >= p.nx) || (y0 + C::TY >= p.ny);
+    if (edge) velocity_consume<C, true>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
+    else velocity_consume<C, false>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -559,26 +599,15 @@ struct SStage {
                          FIXED = RYZ + C::D_BYTES;
 };
 
-struct StrPlan {
-    bool in0, in1, in2;
-    bool xy0, xz0, yz0;    // plane m: finish sxy / form the D+x vz, D+y vz partials
-    bool rii1;             // plane m-1 has lossy cells
-    bool xz2, yz2;         // plane m-2: finish sxz / syz
+// control word of one stress iteration (StageHdr::ctrl)
+enum : uint32_t {
+    SC_IN0 = 1u, SC_IN1 = 2u, SC_IN2 = 4u,
+    SC_XY0 = 8u, SC_XZ0 = 16u, SC_YZ0 = 32u,   // plane m: finish sxy / form the D+x vz, D+y vz partials
+    SC_RII1 = 64u,                             // plane m-1 has lossy cells
+    SC_XZ2 = 128u, SC_YZ2 = 256u,              // plane m-2: finish sxz / syz
+    SC_ZS1 = 512u, SC_ZS2 = 1024u,             // plane m-1 / m-2 lies in a z slab (and inside the chunk)
+    SC_PEAK = 2048u, SC_RMS = 4096u
 };
-// f0, f1, f2 = flag words of planes m, m-1, m-2
-__device__ __forceinline__ StrPlan str_plan(int m, int kz0, int kz1, uint32_t f0, uint32_t f1, uint32_t f2) {
-    StrPlan v;
-    v.in0 = m >= kz0 && m < kz1;
-    v.in1 = m - 1 >= kz0 && m - 1 < kz1;
-    v.in2 = m - 2 >= kz0 && m - 2 < kz1;
-    v.xy0 = v.in0 && (f0 & TF_XY);
-    v.xz0 = v.in0 && (f0 & TF_XZ);
-    v.yz0 = v.in0 && (f0 & TF_YZ);
-    v.rii1 = v.in1 && (f1 & TF_RII);
-    v.xz2 = v.in2 && (f2 & TF_XZ);
-    v.yz2 = v.in2 && (f2 & TF_YZ);
-    return v;
-}
 
 struct ShearCoef { float cU, cR; };   // dt mu_U,h and B mu_h tau_h of one shear node (readings P2, P3)
 __device__ __forceinline__ ShearCoef shear_coef(float2 a, float2 b, float2 c, float2 d, float dt, float B) {
@@ -589,12 +618,202 @@ __device__ __forceinline__ ShearCoef shear_coef(float2 a, float2 b, float2 c, fl
     ShearCoef r; r.cU = dt * (mu_h + mt); r.cR = B * mt;
     return r;
 }
+// one shear node: r' = A r - cR g ; s' = s + cU g + dt/2 (r' + r)
+__device__ __forceinline__ void shear_update(const ShearCoef &k, float g, float s0, float r0, float A, float hdt, float &sn, float &rn) {
+    rn = fmaf(A, r0, -(k.cR * g));
+    sn = s0 + fmaf(k.cU, g, hdt * (rn + r0));
+}
+
+template <class C, bool EDGE>
+__device__ __forceinline__ void stress_consume(const Params &p, const StagePlan &sp, unsigned char *stages, unsigned char *mat_ring,
+                                               const int MR, const float4 *tabN, const float2 *tabS, const float *sprof,
+                                               uint64_t *full, uint64_t *empty, int tid, int x0, int y0, int m_begin, int m_end) {
+    using SS = SStage<C>;
+    constexpr int DQ = C::D_BYTES / 4;
+    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
+    const int tx = g.tx, ty = g.ty;
+    const bool active = EDGE ? g.active : true;
+    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
+    const float dt = p.dt, hdt = p.half_dt, A = p.A, B = p.B;
+    const Q4 zero = q_set(0.0f);
+    const int qoff = ty * C::TX + 4 * tx;
+    const int coff = (ty + 2) * C::AX + 4 + 4 * tx;    // own quad inside a C box
+    const int moff = ty * C::MX + 4 * tx;
+    const uint32_t zstride = (uint32_t)(p.px * p.ny);
+
+    ZChain zvx, zvy, zvz;          // D+z vx, D+z vy (finish at m-2), D-z vz (finish at m-1)
+    zc_clear(zvx); zc_clear(zvy); zc_clear(zvz);
+    Q4 nxx = zero, nyy = zero;     // vxx, vyy of plane m-1
+    Q4 dxz1 = zero, dxz2 = zero, dyz1 = zero, dyz2 = zero;   // D+x vz, D+y vz of planes m-1 and m-2
+
+    uint32_t goff = g.gcell + (uint32_t)(p.sz * m_begin);
+    uint32_t gxo = g.gx + (uint32_t)(p.wx * p.ny) * (uint32_t)m_begin;
+    uint32_t gyo = g.gy + (uint32_t)(p.px * 2 * p.P) * (uint32_t)m_begin;
+    int s = 0; uint32_t ph = 0;
+    int mr0 = ((m_begin % MR) + MR) % MR;   // ring slot of plane m
+    for (int m = m_begin; m < m_end; ++m) {
+        mbar_wait(&full[s], ph);
+        const unsigned char *st = stages + s * sp.bytes;
+        const StageHdr *hdr = reinterpret_cast<const StageHdr *>(st + sp.hdr);
+        const uint32_t ctrl = hdr->ctrl;
+        const int mr1 = mr0 == 0 ? MR - 1 : mr0 - 1;          // plane m-1
+        const int mr2 = mr1 == 0 ? MR - 1 : mr1 - 1;          // plane m-2
+        if (active) {
+            const float *cvx = reinterpret_cast<const float *>(st + SS::VXB) + coff;
+            const float *cvy = cvx + C::C_BYTES / 4;
+            const float *cvz = cvy + C::C_BYTES / 4;
+            const float *dbase = reinterpret_cast<const float *>(st) + qoff;
+            const float *psz = reinterpret_cast<const float *>(st + sp.psz) + qoff;
+            const unsigned char *mat0 = mat_ring + mr0 * C::M_BYTES + moff;
+            const unsigned char *mat1 = mat_ring + mr1 * C::M_BYTES + moff;
+            const unsigned char *mat2 = mat_ring + mr2 * C::M_BYTES + moff;
+
+            // ---- z chains: push plane m ----
+            const Q4 fvx = q_ld(cvx), fvy = q_ld(cvy), fvz = q_ld(cvz);
+            Q4 vzz = zc_push(zvz, fvz, c1, c2);     // D-z vz at m-1
+            Q4 vx_z = zc_push(zvx, fvx, c1, c2);    // D+z vx at m-2
+            Q4 vy_z = zc_push(zvy, fvy, c1, c2);    // D+z vy at m-2
+
+            if (ctrl & SC_IN1) {
+                // finish the normal stresses, their memory variables and the sensor at plane m-1
+                if (ctrl & SC_ZS1) {
+                    const uint32_t qz = g.gz + zstride * (uint32_t)z_compact(p, m - 1);
+                    q_store<EDGE>(p.psi[17] + qz, q_cpml(vzz, q_ld(psz + 2 * DQ), q_set(hdr->az1), q_set(hdr->bz1)), g.nv);
+                }
+                const uint32_t mw = *reinterpret_cast<const uint32_t *>(mat1);
+                const float4 r0 = tabN[mw & 255u], r1 = tabN[(mw >> 8) & 255u], r2 = tabN[(mw >> 16) & 255u], r3 = tabN[mw >> 24];
+                const Q4 eP = q_make(r0.x, r1.x, r2.x, r3.x), eS = q_make(r0.y, r1.y, r2.y, r3.y);
+                const Q4 th = q_add(q_add(nxx, nyy), vzz);
+                const Q4 ePth = q_mul(eP, th);
+                const Q4 vii[3] = {nxx, nyy, vzz};
+                const uint32_t gq = goff - (uint32_t)p.sz;
+                Q4 tr = zero;
+                if (ctrl & SC_RII1) {
+                    const Q4 bP = q_make(r0.z, r1.z, r2.z, r3.z), bS = q_make(r0.w, r1.w, r2.w, r3.w);
+                    const Q4 bPth = q_mul(bP, th);
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        const Q4 oth = q_sub(th, vii[q]);
+                        const Q4 eU = q_fnma(eS, oth, ePth);
+                        const Q4 eR = q_fnma(bS, oth, bPth);
+                        const Q4 rold = q_ld(dbase + SS::RII / 4 + q * DQ);
+                        const Q4 rn = q_sub(q_muls(rold, A), eR);
+                        const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), q_fmas(hdt, q_add(rn, rold), eU));
+                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        q_store<EDGE>(p.f[RXX + q] + gq, rn, g.nv);
+                        tr = q_add(tr, sn);
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        const Q4 eU = q_fnma(eS, q_sub(th, vii[q]), ePth);
+                        const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), eU);
+                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        tr = q_add(tr, sn);
+                    }
+                }
+                if (ctrl & (SC_PEAK | SC_RMS)) {
+                    const Q4 pr = q_muls(tr, -1.0f / 3.0f);
+                    if (ctrl & SC_PEAK) {
+                        const Q4 pk = q_ld(dbase + SS::PEAK / 4);
+                        q_store<EDGE>(p.peak + gq, q_make(fmaxf(pk.a.x, fabsf(pr.a.x)), fmaxf(pk.a.y, fabsf(pr.a.y)),
+                                                          fmaxf(pk.b.x, fabsf(pr.b.x)), fmaxf(pk.b.y, fabsf(pr.b.y))), g.nv);
+                    }
+                    if (ctrl & SC_RMS) q_store<EDGE>(p.sumsq + gq, q_fma(pr, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
+                }
+            }
+            if (ctrl & (SC_XZ2 | SC_YZ2)) {
+                // finish sxz, syz (+ r) at plane m-2
+                const uint32_t qz = g.gz + zstride * (uint32_t)z_compact(p, m - 2);
+                const Q4 az = q_set(hdr->az2), bz = q_set(hdr->bz2);
+                const uint32_t gq = goff - 2u * (uint32_t)p.sz;
+                // materials: row j at planes m-2 (mat2) and m-1 (mat1), cells i0..i0+4; row j+1 cells i0..i0+3
+                float2 m2[5], m1[5];
+#pragma unroll
+                for (int c = 0; c < 5; ++c) { m2[c] = tabS[mat2[c]]; m1[c] = tabS[mat1[c]]; }
+                if (ctrl & SC_XZ2) {
+                    if (ctrl & SC_ZS2) q_store<EDGE>(p.psi[15] + qz, q_cpml(vx_z, q_ld(psz), az, bz), g.nv);
+                    const Q4 gg4 = q_add(vx_z, dxz2);
+                    const Q4 so = q_ld(dbase + SS::SXZ / 4), ro = q_ld(dbase + SS::RXZ / 4);
+                    float os[4], orr[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)   // cells (i..i+1, j, k..k+1)
+                        shear_update(shear_coef(m2[c], m2[c + 1], m1[c], m1[c + 1], dt, B), q_get(gg4, c), q_get(so, c), q_get(ro, c), A, hdt, os[c], orr[c]);
+                    q_store<EDGE>(p.f[SXZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                    q_store<EDGE>(p.f[RXZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
+                }
+                if (ctrl & SC_YZ2) {
+                    if (ctrl & SC_ZS2) q_store<EDGE>(p.psi[16] + qz, q_cpml(vy_z, q_ld(psz + DQ), az, bz), g.nv);
+                    const Q4 gg4 = q_add(vy_z, dyz2);
+                    const Q4 so = q_ld(dbase + SS::SYZ / 4), ro = q_ld(dbase + SS::RYZ / 4);
+                    float os[4], orr[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)   // cells (i, j..j+1, k..k+1)
+                        shear_update(shear_coef(m2[c], tabS[mat2[C::MX + c]], m1[c], tabS[mat1[C::MX + c]], dt, B), q_get(gg4, c), q_get(so, c),
+                                     q_get(ro, c), A, hdt, os[c], orr[c]);
+                    q_store<EDGE>(p.f[SYZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                    q_store<EDGE>(p.f[RYZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
+                }
+            }
+            dxz2 = dxz1; dyz2 = dyz1;
+
+            // ---- x-y derivatives of plane m ----
+            if (ctrl & SC_IN0) {
+                Q4 vxx = x_dminus(cvx, c1, c2);                                                       // D-x vx
+                Q4 vyy = q_d4(q_ld(cvy - 2 * C::AX), q_ld(cvy - C::AX), fvy, q_ld(cvy + C::AX), c1, c2);  // D-y vy
+                Q4 vx_y = zero, vy_x = zero, vz_x = zero, vz_y = zero;
+                if (ctrl & SC_XY0) {
+                    vx_y = q_d4(q_ld(cvx - C::AX), fvx, q_ld(cvx + C::AX), q_ld(cvx + 2 * C::AX), c1, c2);   // D+y vx
+                    vy_x = x_dplus(cvy, c1, c2);                                                      // D+x vy
+                }
+                if (ctrl & SC_XZ0) vz_x = x_dplus(cvz, c1, c2);                                       // D+x vz
+                if (ctrl & SC_YZ0) vz_y = q_d4(q_ld(cvz - C::AX), fvz, q_ld(cvz + C::AX), q_ld(cvz + 2 * C::AX), c1, c2);   // D+y vz
+                if (g.in_x) {
+                    const float *sp_x = sprof + 4 * tx;
+                    const Q4 ah = q_ld(sp_x + 2 * C::TX), bh = q_ld(sp_x + 3 * C::TX);
+                    const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
+                    q_st(p.psi[3] + gxo, q_cpml(vxx, q_ld(ps), q_ld(sp_x), q_ld(sp_x + C::TX)));
+                    if (ctrl & SC_XY0) q_st(p.psi[4] + gxo, q_cpml(vy_x, q_ld(ps + sp.xt / 4), ah, bh));
+                    if (ctrl & SC_XZ0) q_st(p.psi[5] + gxo, q_cpml(vz_x, q_ld(ps + sp.xt / 2), ah, bh));
+                }
+                if (g.row_y) {
+                    const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
+                    const Q4 ah = q_set(g.ay_h), bh = q_set(g.by_h);
+                    if (ctrl & SC_XY0) q_store<EDGE>(p.psi[9] + gyo, q_cpml(vx_y, q_ld(ps), ah, bh), g.nv);
+                    q_store<EDGE>(p.psi[10] + gyo, q_cpml(vyy, q_ld(ps + DQ), q_set(g.ay_i), q_set(g.by_i)), g.nv);
+                    if (ctrl & SC_YZ0) q_store<EDGE>(p.psi[11] + gyo, q_cpml(vz_y, q_ld(ps + 2 * DQ), ah, bh), g.nv);
+                }
+                nxx = vxx; nyy = vyy; dxz1 = vz_x; dyz1 = vz_y;
+                if (ctrl & SC_XY0) {
+                    // finish sxy, rxy at plane m: material of the 4 cells (i..i+1, j..j+1, m)
+                    const Q4 gxy = q_add(vx_y, vy_x);
+                    const Q4 so = q_ld(dbase + SS::SXY / 4), ro = q_ld(dbase + SS::RXY / 4);
+                    float2 ma[5], mb[5];
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) { ma[c] = tabS[mat0[c]]; mb[c] = tabS[mat0[C::MX + c]]; }
+                    float os[4], orr[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        shear_update(shear_coef(ma[c], ma[c + 1], mb[c], mb[c + 1], dt, B), q_get(gxy, c), q_get(so, c), q_get(ro, c), A, hdt, os[c], orr[c]);
+                    q_store<EDGE>(p.f[SXY] + goff, q_make(os[0], os[1], os[2], os[3]), g.nv);
+                    q_store<EDGE>(p.f[RXY] + goff, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
+                }
+            }
+        }
+        goff += (uint32_t)p.sz;
+        gxo += (uint32_t)(p.wx * p.ny);
+        gyo += (uint32_t)(p.px * 2 * p.P);
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&empty[s]);
+        if (++s == sp.ns) { s = 0; ph ^= 1; }
+        if (++mr0 == MR) mr0 = 0;
+    }
+}
 
 template <class C>
 __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
                                                            const int nzc, const StagePlan sp) {
     using SS = SStage<C>;
-    constexpr int DQ = C::D_BYTES / 4;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
     const int MR = sp.ns + 3;                                   // material ring planes
@@ -609,8 +828,6 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
     const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
     const int m_begin = kz0 - 2, m_end = kz1 + 2;
-    const uint32_t *flags = p.flagsS + (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2;
-    const bool do_peak = p.do_peak != 0, do_rms = p.do_rms != 0;
 
     for (int q = tid; q < 256; q += C::NT) {
         const KRow r = p.rows[q];
@@ -625,12 +842,13 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
     }
     __syncthreads();
 
-    const TileX tX = make_tilex<C>(p, x0);
-    const bool tY = tile_in_y<C>(p, y0);
-    const int jy0 = tile_jy0<C>(p, y0);
-
     if (tid >= C::NC) {
         if (tid == C::NC) {
+            const uint32_t *flags = p.flagsS + (size_t)(blockIdx.x + p.ntxS * blockIdx.y) * (p.nz + 4) + 2;
+            const bool do_peak = p.do_peak != 0, do_rms = p.do_rms != 0;
+            const TileX tX = make_tilex<C>(p, x0);
+            const bool tY = tile_in_y<C>(p, y0);
+            const int jy0 = tile_jy0<C>(p, y0);
             prefetch_tmap(&maps.boxC); prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
@@ -638,51 +856,65 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
             uint32_t f1 = 0, f2 = 0;
             const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
             const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
+            uint32_t fl_next = __ldg(flags + m_begin);
             for (int m = m_begin; m < m_end; ++m) {
-                const uint32_t f0 = __ldg(flags + m);
-                const StrPlan v = str_plan(m, kz0, kz1, f0, f1, f2);
+                const uint32_t f0 = fl_next;
+                fl_next = __ldg(flags + min(m + 1, p.nz + 1));
+                const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
+                const bool xy0 = in0 && (f0 & TF_XY), xz0 = in0 && (f0 & TF_XZ), yz0 = in0 && (f0 & TF_YZ);
+                const bool rii1 = in1 && (f1 & TF_RII);
+                const bool xz2 = in2 && (f2 & TF_XZ), yz2 = in2 && (f2 & TF_YZ);
                 f2 = f1; f1 = f0;
+                const bool zs1 = in1 && z_in_slab(p, m - 1), zs2 = in2 && z_in_slab(p, m - 2);
+                StageHdr h;
+                h.ctrl = (in0 ? SC_IN0 : 0u) | (in1 ? SC_IN1 : 0u) | (in2 ? SC_IN2 : 0u) | (xy0 ? SC_XY0 : 0u) | (xz0 ? SC_XZ0 : 0u) |
+                         (yz0 ? SC_YZ0 : 0u) | (rii1 ? SC_RII1 : 0u) | (xz2 ? SC_XZ2 : 0u) | (yz2 ? SC_YZ2 : 0u) | (zs1 ? SC_ZS1 : 0u) |
+                         (zs2 ? SC_ZS2 : 0u) | (do_peak ? SC_PEAK : 0u) | (do_rms ? SC_RMS : 0u);
+                h.az1 = h.bz1 = h.az2 = h.bz2 = 0.0f;
+                if (zs1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
+                if (zs2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
                 mbar_wait(&empty[s], ph ^ 1);
                 unsigned char *st = stages + s * sp.bytes;
                 uint64_t *bar = &full[s];
-                const bool zs1 = v.in1 && z_in_slab(p, m - 1), zs2 = v.in2 && z_in_slab(p, m - 2);
+                StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
+                hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
                 uint32_t bytes = 3 * C::C_BYTES + C::MX * C::MY;
-                if (v.in0) {
-                    bytes += nx_boxes * xbox * (1u + (v.xy0 ? 1u : 0u) + (v.xz0 ? 1u : 0u));
-                    if (tY) bytes += C::D_BYTES * (1u + (v.xy0 ? 1u : 0u) + (v.yz0 ? 1u : 0u));
+                if (in0) {
+                    bytes += nx_boxes * xbox * (1u + (xy0 ? 1u : 0u) + (xz0 ? 1u : 0u));
+                    if (tY) bytes += C::D_BYTES * (1u + (xy0 ? 1u : 0u) + (yz0 ? 1u : 0u));
                 }
-                if (v.xy0) bytes += 2 * C::D_BYTES;
-                if (v.in1) bytes += C::D_BYTES * (3u + (v.rii1 ? 3u : 0u) + (do_peak ? 1u : 0u) + (do_rms ? 1u : 0u) + (zs1 ? 1u : 0u));
-                if (v.xz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
-                if (v.yz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
+                if (xy0) bytes += 2 * C::D_BYTES;
+                if (in1) bytes += C::D_BYTES * (3u + (rii1 ? 3u : 0u) + (do_peak ? 1u : 0u) + (do_rms ? 1u : 0u) + (zs1 ? 1u : 0u));
+                if (xz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
+                if (yz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
                 mbar_expect_tx(bar, bytes);
                 const int z = m + 2;
                 tma_load_4d(st + SS::VXB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VX);
                 tma_load_4d(st + SS::VYB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VY);
                 tma_load_4d(st + SS::VZB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VZ);
-                if (v.in0) {
+                if (in0) {
                     // psi of the x-y derivatives of plane m: x terms 3 (D-x vx), 4 (D+x vy), 5 (D+x vz);
                     // y terms 3 (D+y vx), 4 (D-y vy), 5 (D+y vz)
-                    const bool use[3] = {true, v.xy0, v.xz0};
-                    const bool usey[3] = {v.xy0, true, v.yz0};
+                    const bool use[3] = {true, xy0, xz0};
+                    const bool usey[3] = {xy0, true, yz0};
 #pragma unroll
                     for (int t = 0; t < 3; ++t) {
                         if (use[t]) {
-                            unsigned char *d = st + sp.psx + t * 2 * sp.xb;
+                            unsigned char *d = st + sp.psx + t * sp.xt;
                             if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, 3 + t);
-                            if (tX.hi) tma_load_4d(d + sp.xb, &maps.psx, bar, tX.cx_hi, y0, m, 3 + t);
+                            if (tX.hi) tma_load_4d(d + sp.xhi, &maps.psx, bar, tX.cx_hi, y0, m, 3 + t);
                         }
                         if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, 3 + t);
                     }
                 }
-                if (v.xy0) {
+                if (xy0) {
                     tma_load_4d(st + SS::SXY, &maps.boxD, bar, x0, y0, z, SXY);
                     tma_load_4d(st + SS::RXY, &maps.boxD, bar, x0, y0, z, RXY);
                 }
-                if (v.in1) {
+                if (in1) {
 #pragma unroll
                     for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::SII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, SXX + q);
-                    if (v.rii1) {
+                    if (rii1) {
 #pragma unroll
                         for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::RII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, RXX + q);
                     }
@@ -690,12 +922,12 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
                     if (do_rms) tma_load_4d(st + SS::SUMSQ, &maps.boxD, bar, x0, y0, z - 1, F_SUMSQ);
                     if (zs1) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 1), 5);
                 }
-                if (v.xz2) {
+                if (xz2) {
                     tma_load_4d(st + SS::SXZ, &maps.boxD, bar, x0, y0, z - 2, SXZ);
                     tma_load_4d(st + SS::RXZ, &maps.boxD, bar, x0, y0, z - 2, RXZ);
                     if (zs2) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 3);
                 }
-                if (v.yz2) {
+                if (yz2) {
                     tma_load_4d(st + SS::SYZ, &maps.boxD, bar, x0, y0, z - 2, SYZ);
                     tma_load_4d(st + SS::RYZ, &maps.boxD, bar, x0, y0, z - 2, RYZ);
                     if (zs2) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 4);
@@ -709,201 +941,9 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
     }
 
     // ================= consumers =================
-    const ThreadGeom<C> g = make_geom<C>(p, sp, tid, x0, y0);
-    const int tx = g.tx, ty = g.ty;
-    const float c1 = 1.125f * p.inv_dx, c2 = (-1.0f / 24.0f) * p.inv_dx;
-    const float dt = p.dt, hdt = p.half_dt, A = p.A, B = p.B;
-    const Q4 zero = q_set(0.0f);
-
-    Q4 wvx[4], wvy[4], wvz[4];     // z windows, slot 3 = plane m
-    Q4 nxx = zero, nyy = zero;     // vxx, vyy of plane m-1
-    Q4 dxz1 = zero, dxz2 = zero, dyz1 = zero, dyz2 = zero;   // D+x vz, D+y vz of planes m-1 and m-2
-#pragma unroll
-    for (int w = 0; w < 4; ++w) wvx[w] = wvy[w] = wvz[w] = zero;
-
-    int s = 0; uint32_t ph = 0;
-    int mr0 = ((m_begin % MR) + MR) % MR;   // ring slot of plane m
-    uint32_t f1 = 0, f2 = 0;
-    uint32_t fl_next = __ldg(flags + m_begin);
-    for (int m = m_begin; m < m_end; ++m) {
-        const uint32_t f0 = fl_next;
-        fl_next = __ldg(flags + min(m + 1, p.nz + 1));
-        const StrPlan v = str_plan(m, kz0, kz1, f0, f1, f2);
-        f2 = f1; f1 = f0;
-        mbar_wait(&full[s], ph);
-        const unsigned char *st = stages + s * sp.bytes;
-        const int qoff = ty * C::TX + 4 * tx;
-        const float *cvx = reinterpret_cast<const float *>(st + SS::VXB) + (ty + 2) * C::AX + 4 + 4 * tx;
-        const float *cvy = cvx + C::C_BYTES / 4;
-        const float *cvz = cvy + C::C_BYTES / 4;
-        const float *dbase = reinterpret_cast<const float *>(st) + qoff;
-        const int mr1 = mr0 == 0 ? MR - 1 : mr0 - 1;          // plane m-1
-        const int mr2 = mr1 == 0 ? MR - 1 : mr1 - 1;          // plane m-2
-        const unsigned char *mat0 = mat_ring + mr0 * C::M_BYTES + ty * C::MX + 4 * tx;
-        const unsigned char *mat1 = mat_ring + mr1 * C::M_BYTES + ty * C::MX + 4 * tx;
-        const unsigned char *mat2 = mat_ring + mr2 * C::M_BYTES + ty * C::MX + 4 * tx;
-
-        // ---- slide the z windows and insert plane m ----
-#pragma unroll
-        for (int w = 0; w < 3; ++w) { wvx[w] = wvx[w + 1]; wvy[w] = wvy[w + 1]; wvz[w] = wvz[w + 1]; }
-        wvx[3] = q_ld(cvx); wvy[3] = q_ld(cvy); wvz[3] = q_ld(cvz);
-
-        Q4 nvxx = zero, nvyy = zero, ndxz = zero, ndyz = zero;
-        if (v.in0 && g.active) {
-            Q4 vxx = x_dminus(cvx, c1, c2);                                                           // D-x vx
-            Q4 vyy = q_d4(q_ld(cvy - 2 * C::AX), q_ld(cvy - C::AX), wvy[3], q_ld(cvy + C::AX), c1, c2);   // D-y vy
-            Q4 vx_y = zero, vy_x = zero, vz_x = zero, vz_y = zero;
-            if (v.xy0) {
-                vx_y = q_d4(q_ld(cvx - C::AX), wvx[3], q_ld(cvx + C::AX), q_ld(cvx + 2 * C::AX), c1, c2);   // D+y vx
-                vy_x = x_dplus(cvy, c1, c2);                                                          // D+x vy
-            }
-            if (v.xz0) vz_x = x_dplus(cvz, c1, c2);                                                   // D+x vz
-            if (v.yz0) vz_y = q_d4(q_ld(cvz - C::AX), wvz[3], q_ld(cvz + C::AX), q_ld(cvz + 2 * C::AX), c1, c2);   // D+y vz
-            if (g.in_x) {
-                const float *sp_x = sprof + 4 * tx;
-                const Q4 ah = q_ld(sp_x + 2 * C::TX), bh = q_ld(sp_x + 3 * C::TX);
-                const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
-                const long long q = g.gx + (long long)p.wx * p.ny * m;
-                q_st(p.psi[3] + q, q_cpml(vxx, q_ld(ps), q_ld(sp_x), q_ld(sp_x + C::TX)));
-                if (v.xy0) q_st(p.psi[4] + q, q_cpml(vy_x, q_ld(ps + sp.xb / 2), ah, bh));
-                if (v.xz0) q_st(p.psi[5] + q, q_cpml(vz_x, q_ld(ps + sp.xb), ah, bh));
-            }
-            if (g.row_y) {
-                const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
-                const long long q = g.gy + (long long)p.px * (2 * p.P) * m;
-                const Q4 ah = q_set(g.ay_h), bh = q_set(g.by_h);
-                if (v.xy0) q_st_n(p.psi[9] + q, q_cpml(vx_y, q_ld(ps), ah, bh), g.nv);
-                q_st_n(p.psi[10] + q, q_cpml(vyy, q_ld(ps + DQ), q_set(g.ay_i), q_set(g.by_i)), g.nv);
-                if (v.yz0) q_st_n(p.psi[11] + q, q_cpml(vz_y, q_ld(ps + 2 * DQ), ah, bh), g.nv);
-            }
-            nvxx = vxx; nvyy = vyy; ndxz = vz_x; ndyz = vz_y;
-            if (v.xy0) {
-                // finish sxy, rxy at plane m: material of the 4 cells (i..i+1, j..j+1, m)
-                const Q4 gxy = q_add(vx_y, vy_x);
-                const Q4 so = q_ld(dbase + SS::SXY / 4), ro = q_ld(dbase + SS::RXY / 4);
-                float2 ma[5], mb[5];
-#pragma unroll
-                for (int c = 0; c < 5; ++c) { ma[c] = tabS[mat0[c]]; mb[c] = tabS[mat0[C::MX + c]]; }
-                float os[4], orr[4];
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const ShearCoef k = shear_coef(ma[c], ma[c + 1], mb[c], mb[c + 1], dt, B);
-                    const float r0 = q_get(ro, c), gg = q_get(gxy, c);
-                    const float rn = fmaf(A, r0, -(k.cR * gg));
-                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
-                    orr[c] = rn;
-                }
-                const long long gq = g.gcell + p.sz * m;
-                q_st_n(p.f[SXY] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
-                q_st_n(p.f[RXY] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
-            }
-        }
-
-        const int k1 = m - 1, k2 = m - 2;
-        if (v.in1 && g.active) {
-            // finish the normal stresses, their memory variables and the sensor at plane k1
-            Q4 vzz = q_d4(wvz[0], wvz[1], wvz[2], wvz[3], c1, c2);   // D-z vz at k1
-            if (z_in_slab(p, k1)) {
-                const float az = __ldg(p.prof[2][0] + k1), bz = __ldg(p.prof[2][1] + k1);
-                const long long qz = g.gz + (long long)p.px * p.ny * z_compact(p, k1);
-                q_st_n(p.psi[17] + qz, q_cpml(vzz, q_ld(reinterpret_cast<const float *>(st + sp.psz + 2 * C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
-            }
-            const uint32_t mw = *reinterpret_cast<const uint32_t *>(mat1);
-            const float4 r0 = tabN[mw & 255u], r1 = tabN[(mw >> 8) & 255u], r2 = tabN[(mw >> 16) & 255u], r3 = tabN[mw >> 24];
-            const Q4 eP = q_make(r0.x, r1.x, r2.x, r3.x), eS = q_make(r0.y, r1.y, r2.y, r3.y);
-            const Q4 th = q_add(q_add(nxx, nyy), vzz);
-            const Q4 ePth = q_mul(eP, th);
-            const Q4 vii[3] = {nxx, nyy, vzz};
-            const long long gq = g.gcell + p.sz * k1;
-            Q4 tr = zero;
-            if (v.rii1) {
-                const Q4 bP = q_make(r0.z, r1.z, r2.z, r3.z), bS = q_make(r0.w, r1.w, r2.w, r3.w);
-                const Q4 bPth = q_mul(bP, th);
-#pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    const Q4 oth = q_sub(th, vii[q]);
-                    const Q4 eU = q_fnma(eS, oth, ePth);
-                    const Q4 eR = q_fnma(bS, oth, bPth);
-                    const Q4 rold = q_ld(dbase + SS::RII / 4 + q * DQ);
-                    const Q4 rn = q_sub(q_muls(rold, A), eR);
-                    const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), q_fmas(hdt, q_add(rn, rold), eU));
-                    q_st_n(p.f[SXX + q] + gq, sn, g.nv);
-                    q_st_n(p.f[RXX + q] + gq, rn, g.nv);
-                    tr = q_add(tr, sn);
-                }
-            } else {
-#pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    const Q4 eU = q_fnma(eS, q_sub(th, vii[q]), ePth);
-                    const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), eU);
-                    q_st_n(p.f[SXX + q] + gq, sn, g.nv);
-                    tr = q_add(tr, sn);
-                }
-            }
-            if (do_peak | do_rms) {
-                const Q4 pr = q_muls(tr, -1.0f / 3.0f);
-                if (do_peak) {
-                    const Q4 pk = q_ld(dbase + SS::PEAK / 4);
-                    q_st_n(p.peak + gq, q_make(fmaxf(pk.a.x, fabsf(pr.a.x)), fmaxf(pk.a.y, fabsf(pr.a.y)),
-                                               fmaxf(pk.b.x, fabsf(pr.b.x)), fmaxf(pk.b.y, fabsf(pr.b.y))), g.nv);
-                }
-                if (do_rms) q_st_n(p.sumsq + gq, q_fma(pr, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
-            }
-        }
-        if ((v.xz2 | v.yz2) && g.active) {
-            // finish sxz, syz (+ r) at plane k2: D+z of vx, vy over planes m-3..m
-            const bool zs = z_in_slab(p, k2);
-            float az = 0.0f, bz = 0.0f;
-            long long qz = 0;
-            if (zs) { az = __ldg(p.prof[2][2] + k2); bz = __ldg(p.prof[2][3] + k2); qz = g.gz + (long long)p.px * p.ny * z_compact(p, k2); }
-            const long long gq = g.gcell + p.sz * k2;
-            // materials: row j at planes k2 (mat2) and k2+1 (mat1), cells i0..i0+4; row j+1 cells i0..i0+3
-            float2 m2[5], m1[5];
-#pragma unroll
-            for (int c = 0; c < 5; ++c) { m2[c] = tabS[mat2[c]]; m1[c] = tabS[mat1[c]]; }
-            if (v.xz2) {
-                Q4 vx_z = q_d4(wvx[0], wvx[1], wvx[2], wvx[3], c1, c2);   // D+z vx at k2
-                if (zs) q_st_n(p.psi[15] + qz, q_cpml(vx_z, q_ld(reinterpret_cast<const float *>(st + sp.psz) + qoff), q_set(az), q_set(bz)), g.nv);
-                const Q4 gg4 = q_add(vx_z, dxz2);
-                const Q4 so = q_ld(dbase + SS::SXZ / 4), ro = q_ld(dbase + SS::RXZ / 4);
-                float os[4], orr[4];
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {   // cells (i..i+1, j, k2..k2+1)
-                    const ShearCoef k = shear_coef(m2[c], m2[c + 1], m1[c], m1[c + 1], dt, B);
-                    const float r0 = q_get(ro, c), gg = q_get(gg4, c);
-                    const float rn = fmaf(A, r0, -(k.cR * gg));
-                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
-                    orr[c] = rn;
-                }
-                q_st_n(p.f[SXZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
-                q_st_n(p.f[RXZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
-            }
-            if (v.yz2) {
-                Q4 vy_z = q_d4(wvy[0], wvy[1], wvy[2], wvy[3], c1, c2);   // D+z vy at k2
-                if (zs) q_st_n(p.psi[16] + qz, q_cpml(vy_z, q_ld(reinterpret_cast<const float *>(st + sp.psz + C::D_BYTES) + qoff), q_set(az), q_set(bz)), g.nv);
-                const Q4 gg4 = q_add(vy_z, dyz2);
-                const Q4 so = q_ld(dbase + SS::SYZ / 4), ro = q_ld(dbase + SS::RYZ / 4);
-                float os[4], orr[4];
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {   // cells (i, j..j+1, k2..k2+1)
-                    const ShearCoef k = shear_coef(m2[c], tabS[mat2[C::MX + c]], m1[c], tabS[mat1[C::MX + c]], dt, B);
-                    const float r0 = q_get(ro, c), gg = q_get(gg4, c);
-                    const float rn = fmaf(A, r0, -(k.cR * gg));
-                    os[c] = q_get(so, c) + fmaf(k.cU, gg, hdt * (rn + r0));
-                    orr[c] = rn;
-                }
-                q_st_n(p.f[SYZ] + gq, q_make(os[0], os[1], os[2], os[3]), g.nv);
-                q_st_n(p.f[RYZ] + gq, q_make(orr[0], orr[1], orr[2], orr[3]), g.nv);
-            }
-        }
-        nxx = nvxx; nyy = nvyy;
-        dxz2 = dxz1; dxz1 = ndxz;
-        dyz2 = dyz1; dyz1 = ndyz;
-        __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty[s]);
-        if (++s == sp.ns) { s = 0; ph ^= 1; }
-        if (++mr0 == MR) mr0 = 0;
-    }
+    const bool edge = (x0 + C::TX >= p.nx) || (y0 + C::TY >= p.ny);
+    if (edge) stress_consume<C, true>(p, sp, stages, mat_ring, MR, tabN, tabS, sprof, full, empty, tid, x0, y0, m_begin, m_end);
+    else stress_consume<C, false>(p, sp, stages, mat_ring, MR, tabN, tabS, sprof, full, empty, tid, x0, y0, m_begin, m_end);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -911,19 +951,21 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
 // ------------------------------------------------------------------------------------------
 // One CTA per (tile, plane).  solid(m) = mu_R > 0; a shear node is "solid" when its four cells are
 // (reading P2; out-of-grid neighbours are the replicated edge of the private index map).
+// pass 0: velocity flags (taken over the halo-extended tile the pass reads), pass 1: stress flags.
 template <class C>
-__global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__restrict__ flagsV, uint32_t *__restrict__ flagsS, const int dense) {
-    __shared__ uint32_t sv, ss;
+__global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__restrict__ flags, const int ntx, const int pass, const int dense) {
+    __shared__ uint32_t sf;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, k = blockIdx.z;
-    if (threadIdx.x == 0) { sv = 0; ss = 0; }
+    if (threadIdx.x == 0) sf = 0;
     __syncthreads();
-    uint32_t fv = 0, fs = 0;
+    uint32_t f = 0;
     if (dense) {
-        fv = TF_XY | TF_XZ | TF_YZ; fs = TF_XY | TF_XZ | TF_YZ | TF_RII;
+        f = pass == 0 ? (TF_XY | TF_XZ | TF_YZ) : (TF_XY | TF_XZ | TF_YZ | TF_RII);
     } else {
-        constexpr int EX = C::TX + 4, EY = C::TY + 4;
+        const int h = pass == 0 ? 2 : 0;
+        const int EX = C::TX + 2 * h, EY = C::TY + 2 * h;
         for (int q = threadIdx.x; q < EX * EY; q += blockDim.x) {
-            const int i = x0 - 2 + q % EX, j = y0 - 2 + q / EX;
+            const int i = x0 - h + q % EX, j = y0 - h + q / EX;
             if (i < 0 || j < 0 || i >= p.nx || j >= p.ny) continue;
             const uint8_t *mp = p.mat + i + (long long)p.px * j + p.sz * k;
             const KRow r000 = p.rows[mp[0]];
@@ -933,24 +975,15 @@ __global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__
             const bool nxz = s000 * s100 * s001 * s101 != 0.0f;
             const bool nyz = s000 * s010 * s001 * s011 != 0.0f;
             const bool inx = i >= x0 && i < x0 + C::TX, iny = j >= y0 && j < y0 + C::TY;
-            if (nxy) fv |= TF_XY;
-            if (nxz && iny) fv |= TF_XZ;
-            if (nyz && inx) fv |= TF_YZ;
-            if (inx && iny) {
-                if (nxy) fs |= TF_XY;
-                if (nxz) fs |= TF_XZ;
-                if (nyz) fs |= TF_YZ;
-                if (r000.bP != 0.0f || r000.bS != 0.0f) fs |= TF_RII;
-            }
+            if (nxy) f |= TF_XY;
+            if (nxz && iny) f |= TF_XZ;      // velocity reads sxz with an x halo only
+            if (nyz && inx) f |= TF_YZ;      // ... syz with a y halo only
+            if (pass == 1 && (r000.bP != 0.0f || r000.bS != 0.0f)) f |= TF_RII;
         }
     }
-    if (fv) atomicOr(&sv, fv);
-    if (fs) atomicOr(&ss, fs);
+    if (f) atomicOr(&sf, f);
     __syncthreads();
-    if (threadIdx.x == 0) {
-        const size_t o = (size_t)(blockIdx.x + p.ntx * blockIdx.y) * (p.nz + 4) + 2 + k;
-        flagsV[o] = sv; flagsS[o] = ss;
-    }
+    if (threadIdx.x == 0) flags[(size_t)(blockIdx.x + ntx * blockIdx.y) * (p.nz + 4) + 2 + k] = sf;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -968,33 +1001,26 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
 
 inline int round128(int v) { return (v + 127) / 128 * 128; }
 
-// z chunks: fill the resident CTA slots in as few waves as possible
-inline void plan_chunks(const Layout &L, long long slots, int &chunks, int &nzc) {
-    const long long tiles = (long long)L.ntx * L.nty;
+// z chunks: whole waves of resident CTAs cost (planes + 4 priming planes) each; half a wave is added
+// for the imbalance between all-fluid and partly solid tiles (measured on config 2: 14 chunks of 33
+// planes beat 3 chunks of 150 by 8 % in spite of the extra priming planes)
+inline void plan_chunks(int nz, long long tiles, long long slots, int &chunks, int &nzc) {
     int best = 1;
     double best_cost = 1e300;
-    for (int ch = 1; ch <= (L.nz + 7) / 8; ++ch) {
-        const int n = (L.nz + ch - 1) / ch;
-        const long long blocks = tiles * ((L.nz + n - 1) / n);
+    for (int ch = 1; ch <= (nz + 7) / 8; ++ch) {
+        const int n = (nz + ch - 1) / ch;
+        const long long blocks = tiles * ((nz + n - 1) / n);
         const double waves = (double)((blocks + slots - 1) / slots);
-        const double cost = waves * (n + 4);
+        const double cost = (waves + 0.5) * (n + 4);
         if (cost < best_cost - 1e-9) { best_cost = cost; best = ch; }
     }
-    nzc = (L.nz + best - 1) / best;
-    chunks = (L.nz + nzc - 1) / nzc;
+    nzc = (nz + best - 1) / best;
+    chunks = (nz + nzc - 1) / nzc;
 }
 
-inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p, char *const psi_base[3], const long long psi_stride[3]) {
-    using C = Cfg;
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-    if (e != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
-        std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled entry point unavailable (%s)", cudaGetErrorString(e));
-        (void)cudaGetLastError();
-        return BVFDTD_ECUDA;
-    }
-    PFN_encodeTiled enc = (PFN_encodeTiled)fn;
+template <class C>
+inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, const Params &p, char *const psi_base[3],
+                       const long long psi_stride[3], int wxb) {
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     auto encode = [&](CUtensorMap *m, CUtensorMapDataType ty, int rank, void *base, const cuuint64_t *gdim, const cuuint64_t *gstr,
                       const cuuint32_t *box, const char *what) -> int {
@@ -1006,19 +1032,14 @@ inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p, 
         }
         return 0;
     };
-    // the 17 grid arrays (15 state + peak + sumsq) are laid out back to back at a constant stride
     const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
-    for (int q = 0; q < NSTATE; ++q)
-        if ((const char *)p.f[q] - (const char *)p.f[0] != fstride * q) return BVFDTD_EINVAL;
-    if ((const char *)p.peak - (const char *)p.f[0] != fstride * F_PEAK) return BVFDTD_EINVAL;
-    if ((const char *)p.sumsq - (const char *)p.f[0] != fstride * F_SUMSQ) return BVFDTD_EINVAL;
     {
         void *base = (void *)(p.f[0] + (L.org - 2 * L.sz));      // cell (0,0,-2)
         const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), 17};
         const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
         struct { CUtensorMap *m; cuuint32_t bx, by; } boxes[4] = {
-            {&plan.maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&plan.maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
-            {&plan.maps.boxC, (cuuint32_t)C::AX, (cuuint32_t)C::BY}, {&plan.maps.boxD, (cuuint32_t)C::TX, (cuuint32_t)C::TY}};
+            {&maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
+            {&maps.boxC, (cuuint32_t)C::AX, (cuuint32_t)C::BY}, {&maps.boxD, (cuuint32_t)C::TX, (cuuint32_t)C::TY}};
         for (auto &b : boxes) {
             const cuuint32_t box[4] = {b.bx, b.by, 1, 1};
             if (int rc = encode(b.m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, gdim, gstr, box, "field box")) return rc;
@@ -1028,73 +1049,125 @@ inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p, 
         const cuuint64_t mdim[3] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 1)};
         const cuuint64_t mstr[2] = {(cuuint64_t)L.px, (cuuint64_t)L.sz};
         const cuuint32_t mbox[3] = {(cuuint32_t)C::MX, (cuuint32_t)C::MY, 1};
-        if (int rc = encode(&plan.maps.mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)p.mat, mdim, mstr, mbox, "material box")) return rc;
+        if (int rc = encode(&maps.mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)p.mat, mdim, mstr, mbox, "material box")) return rc;
     }
-    const int wxb = L.P > 0 ? std::min(L.xph, C::TX) : 4;
     if (L.P > 0) {
         {   // x slabs: (wx, ny, nz, 6)
             const cuuint64_t d[4] = {(cuuint64_t)L.wx, (cuuint64_t)L.ny, (cuuint64_t)L.nz, 6};
             const cuuint64_t s[3] = {(cuuint64_t)L.wx * 4, (cuuint64_t)L.wx * L.ny * 4, (cuuint64_t)psi_stride[0]};
             const cuuint32_t b[4] = {(cuuint32_t)wxb, (cuuint32_t)C::TY, 1, 1};
-            if (int rc = encode(&plan.maps.psx, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[0], d, s, b, "psi x box")) return rc;
+            if (int rc = encode(&maps.psx, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[0], d, s, b, "psi x box")) return rc;
         }
         {   // y slabs: (px, 2P, nz, 6)
             const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)(2 * L.P), (cuuint64_t)L.nz, 6};
             const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * 2 * L.P * 4, (cuuint64_t)psi_stride[1]};
             const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::TY, 1, 1};
-            if (int rc = encode(&plan.maps.psy, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[1], d, s, b, "psi y box")) return rc;
+            if (int rc = encode(&maps.psy, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[1], d, s, b, "psi y box")) return rc;
         }
         {   // z slabs: (px, ny, 2P, 6)
             const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)L.ny, (cuuint64_t)(2 * L.P), 6};
             const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * L.ny * 4, (cuuint64_t)psi_stride[2]};
             const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::TY, 1, 1};
-            if (int rc = encode(&plan.maps.psz, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[2], d, s, b, "psi z box")) return rc;
+            if (int rc = encode(&maps.psz, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[2], d, s, b, "psi z box")) return rc;
         }
     }
-    // stage plans
-    auto make_stage = [&](int fixed, int ns, int extra) {
-        StagePlan s;
-        s.wxb = wxb;
-        s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
-        s.psx = fixed;
-        s.psy = s.psx + 3 * 2 * s.xb;
-        s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
-        s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
-        s.ns = ns;
-        s.smem = ns * s.bytes + extra;
-        return s;
-    };
+    return 0;
+}
+
+template <class C>
+inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb) {
+    StagePlan s;
+    s.wxb = wxb;
+    s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
+    s.yb = C::D_BYTES;
+    s.hdr = fixed;
+    s.psx = s.hdr + 128;
+    // a tile touches both x slabs only on grids narrower than a tile + the slabs
+    const bool both = L.P > 0 && (C::TX > L.xhb || L.P > C::TX);
+    s.xhi = both ? s.xb : 0;
+    s.xt = both ? 2 * s.xb : s.xb;
+    s.psy = s.psx + 3 * s.xt;
+    s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
+    s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
+    s.ns = ns;
+    s.smem = ns * s.bytes + extra;
+    return s;
+}
+
+inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const psi_base[3], const long long psi_stride[3]) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled entry point unavailable (%s)", cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return BVFDTD_ECUDA;
+    }
+    PFN_encodeTiled enc = (PFN_encodeTiled)fn;
+    // the 17 grid arrays (15 state + peak + sumsq) are laid out back to back at a constant stride
+    const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
+    for (int q = 0; q < NSTATE; ++q)
+        if ((const char *)p.f[q] - (const char *)p.f[0] != fstride * q) return BVFDTD_EINVAL;
+    if ((const char *)p.peak - (const char *)p.f[0] != fstride * F_PEAK) return BVFDTD_EINVAL;
+    if ((const char *)p.sumsq - (const char *)p.f[0] != fstride * F_SUMSQ) return BVFDTD_EINVAL;
+    const int wxb = L.P > 0 ? std::min(L.xph, CfgV::TX) : 4;
+    if (int rc = encode_maps<CfgV>(enc, plan.mv, L, p, psi_base, psi_stride, wxb)) return rc;
+
     const int bar_bytes = 2 * MAX_STAGES * 8;
-    const int v_extra = 256 * 4 + 4 * C::TX * 4 + bar_bytes;
     int dev = 0, sms = 148, smem_max = 227 * 1024;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const char *env_v = std::getenv("BVFDTD_NS_V"), *env_s = std::getenv("BVFDTD_NS_S");
-    int ns_v = env_v ? std::atoi(env_v) : 2, ns_s = env_s ? std::atoi(env_s) : 3;
+    const char *env_v = std::getenv("BVFDTD_NS_V"), *env_s = std::getenv("BVFDTD_NS_S"), *env_ty = std::getenv("BVFDTD_STRESS_TY");
+    int ns_v = env_v ? std::atoi(env_v) : 3, ns_s = env_s ? std::atoi(env_s) : 0;
     ns_v = std::max(2, std::min(MAX_STAGES, ns_v));
-    ns_s = std::max(2, std::min(MAX_STAGES, ns_s));
-    plan.sv = make_stage(VStage<C>::FIXED, ns_v, v_extra);
-    auto s_extra = [&](int ns) { return (ns + 3) * C::M_BYTES + 256 * 16 + 256 * 8 + 4 * C::TX * 4 + bar_bytes; };
-    plan.ss = make_stage(SStage<C>::FIXED, ns_s, s_extra(ns_s));
-    while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage(SStage<C>::FIXED, plan.ss.ns - 1, s_extra(plan.ss.ns - 1));
-    while (plan.sv.smem > smem_max && plan.sv.ns > 2) plan.sv = make_stage(VStage<C>::FIXED, plan.sv.ns - 1, v_extra);
+    const int v_extra = 256 * 4 + 4 * CfgV::TX * 4 + bar_bytes;
+    plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, ns_v, v_extra, wxb);
+    while (plan.sv.smem > smem_max && plan.sv.ns > 2) plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb);
+    // stress pass: 64 x 16 tiles with 2 stages when they fit, else 64 x 8 tiles with up to 3 stages
+    auto s_extra16 = [&](int ns) { return (ns + 3) * CfgS::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS::TX * 4 + bar_bytes; };
+    auto s_extra8 = [&](int ns) { return (ns + 3) * CfgS8::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS8::TX * 4 + bar_bytes; };
+    plan.s16 = !(env_ty && std::atoi(env_ty) == 8);
+    if (plan.s16) {
+        const int ns = ns_s ? std::max(2, std::min(MAX_STAGES, ns_s)) : 2;
+        plan.ss = make_stage<CfgS>(L, SStage<CfgS>::FIXED, ns, s_extra16(ns), wxb);
+        while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage<CfgS>(L, SStage<CfgS>::FIXED, plan.ss.ns - 1, s_extra16(plan.ss.ns - 1), wxb);
+        if (plan.ss.smem > smem_max) plan.s16 = false;
+    }
+    if (!plan.s16) {
+        const int ns = ns_s ? std::max(2, std::min(MAX_STAGES, ns_s)) : 3;
+        plan.ss = make_stage<CfgS8>(L, SStage<CfgS8>::FIXED, ns, s_extra8(ns), wxb);
+        while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage<CfgS8>(L, SStage<CfgS8>::FIXED, plan.ss.ns - 1, s_extra8(plan.ss.ns - 1), wxb);
+    }
     if (plan.ss.smem > smem_max || plan.sv.smem > smem_max) {
         std::snprintf(tiled_err_buf(), 256, "pml %d needs %d bytes of shared memory per CTA (max %d)", L.P, plan.ss.smem, smem_max);
         return BVFDTD_EINVAL;
     }
-    e = cudaFuncSetAttribute(k_velocity_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
+    const int sty = plan.s16 ? CfgS::TY : CfgS8::TY;
+    L.ntxS = (L.nx + CfgS::TX - 1) / CfgS::TX;
+    L.ntyS = (L.ny + sty - 1) / sty;
+    p.ntxS = L.ntxS; p.ntyS = L.ntyS;
+    if (int rc = plan.s16 ? encode_maps<CfgS>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)
+                          : encode_maps<CfgS8>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)) return rc;
+    e = cudaFuncSetAttribute(k_velocity_tiled<CfgV>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
     int occ_v = 1, occ_s = 1;
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<C>, C::NT, plan.sv.smem);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_stress_tiled<C>, C::NT, plan.ss.smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV>, CfgV::NT, plan.sv.smem);
+    if (plan.s16) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<CfgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_stress_tiled<CfgS>, CfgS::NT, plan.ss.smem);
+    } else {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<CfgS8>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_stress_tiled<CfgS8>, CfgS8::NT, plan.ss.smem);
+    }
     if (e != cudaSuccess) {
         std::snprintf(tiled_err_buf(), 256, "kernel attribute/occupancy query: %s", cudaGetErrorString(e));
         (void)cudaGetLastError();
         return BVFDTD_ECUDA;
     }
-    plan_chunks(L, (long long)std::max(1, occ_v) * sms, plan.chunks_v, plan.nzc_v);
-    plan_chunks(L, (long long)std::max(1, occ_s) * sms, plan.chunks_s, plan.nzc_s);
+    plan_chunks(L.nz, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, plan.chunks_v, plan.nzc_v);
+    plan_chunks(L.nz, (long long)L.ntxS * L.ntyS, (long long)std::max(1, occ_s) * sms, plan.chunks_s, plan.nzc_s);
+    if (const char *c = std::getenv("BVFDTD_CHUNKS_V")) { plan.chunks_v = std::max(1, std::atoi(c)); plan.nzc_v = (L.nz + plan.chunks_v - 1) / plan.chunks_v; plan.chunks_v = (L.nz + plan.nzc_v - 1) / plan.nzc_v; }
+    if (const char *c = std::getenv("BVFDTD_CHUNKS_S")) { plan.chunks_s = std::max(1, std::atoi(c)); plan.nzc_s = (L.nz + plan.chunks_s - 1) / plan.chunks_s; plan.chunks_s = (L.nz + plan.nzc_s - 1) / plan.nzc_s; }
     if (std::getenv("BVFDTD_VERBOSE"))
         std::fprintf(stderr, "[bvfdtd] velocity: ns %d stage %d smem %d occ %d chunks %d x %d planes; stress: ns %d stage %d smem %d occ %d chunks %d x %d planes\n",
                      plan.sv.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.chunks_v, plan.nzc_v, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s,
@@ -1105,15 +1178,18 @@ inline int tiled_plan_create(TiledPlan &plan, const Layout &L, const Params &p, 
 
 inline void tiled_plan_destroy(TiledPlan &plan) { plan.ready = false; }
 
-inline void tiled_flags(const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st) {
-    k_tile_flags<Cfg><<<dim3(p.ntx, p.nty, p.nz), 128, 0, st>>>(p, flagsV, flagsS, dense ? 1 : 0);
+inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st) {
+    k_tile_flags<CfgV><<<dim3(p.ntxV, p.ntyV, p.nz), 128, 0, st>>>(p, flagsV, p.ntxV, 0, dense ? 1 : 0);
+    if (plan.s16) k_tile_flags<CfgS><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
+    else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_velocity_tiled<Cfg><<<dim3(p.ntx, p.nty, plan.chunks_v), Cfg::NT, plan.sv.smem, st>>>(plan.maps, p, plan.nzc_v, plan.sv);
+    k_velocity_tiled<CfgV><<<dim3(p.ntxV, p.ntyV, plan.chunks_v), CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.nzc_v, plan.sv);
     return 0;
 }
 inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_stress_tiled<Cfg><<<dim3(p.ntx, p.nty, plan.chunks_s), Cfg::NT, plan.ss.smem, st>>>(plan.maps, p, plan.nzc_s, plan.ss);
+    if (plan.s16) k_stress_tiled<CfgS><<<dim3(p.ntxS, p.ntyS, plan.chunks_s), CfgS::NT, plan.ss.smem, st>>>(plan.ms, p, plan.nzc_s, plan.ss);
+    else k_stress_tiled<CfgS8><<<dim3(p.ntxS, p.ntyS, plan.chunks_s), CfgS8::NT, plan.ss.smem, st>>>(plan.ms, p, plan.nzc_s, plan.ss);
     return 0;
 }
 

@@ -172,7 +172,8 @@ def test_degenerate_media(bv, kind, flags):
 # time-stepped parity with source, PML and sensors on small random domains
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("flags", [0, 1, 2])
-@pytest.mark.parametrize("dims,P,wave", [((45, 38, 50), 6, 0), ((64, 33, 37), 5, 1), ((30, 30, 30), 0, 0)])
+@pytest.mark.parametrize("dims,P,wave", [((45, 38, 50), 6, 0), ((64, 33, 37), 5, 1), ((30, 30, 30), 0, 0),
+                                         ((70, 57, 56), 24, 1)])
 def test_stepped_random_domain(bv, dims, P, wave, flags):
     w = wl.random_domain(*dims, P, seed=30 + P, steps=120, waveform=wave)
     sim, o = run_both(bv, w, flags=flags)
