@@ -293,6 +293,8 @@ def ours(args):
     w.steps = total
     w.rms_begin = max(0, total - 3 * w.spp) if args.config in (1, 2, 3) else -1
     flags = bv.FLAG_REFERENCE_KERNELS if args.reference_kernels else 0
+    if args.dense:
+        flags |= bv.FLAG_DENSE
 
     # ---- device-resident timing -----------------------------------------------------------
     sim = bv.Simulation.from_workload(w, flags=flags, device=dev)
@@ -363,7 +365,12 @@ def ours(args):
     step_bytes = vel_b + st_b
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak_gbs, "unit": "GB/s",
-                "frac": ach / peak_gbs if ach else None, "traffic": ncu_traffic_bytes(dom),
+                "frac": ach / peak_gbs if ach else None,
+                "traffic": ncu_traffic_bytes(dom) if (args.config == 2 and not args.dense and not args.reference_kernels) else None,
+                "bytes_definition": "B_dense of SURVEY.md 8(d): every array of every cell once per pass; the default "
+                                    "path moves fewer bytes where shear stresses / memory variables are identically "
+                                    "zero (traffic = ncu-measured DRAM bytes of the same kernel, profiles/traffic.md)",
+                "class_aware_min_bytes_per_step": w.min_bytes_per_cell_step(rms_frac=n_rms / K) * w.cells,
                 "peak_source": peak_src + ", burst copy figure", "algorithmic_bytes_per_launch": st_b,
                 "step": {"algorithmic_bytes": step_bytes, "achieved_gbs": step_gbs,
                          "frac_of_measured": step_gbs / peak_gbs, "frac_of_8TBs": step_gbs / 8000.0},
@@ -379,7 +386,8 @@ def ours(args):
                    "materials": int(w.table.shape[0]), "source_cells": int(w.src_cell.size),
                    "parallelism": f"replicas x{world} (no sharding)",
                    "l2": "state 2.4 GB per step >> 126 MB L2: inputs larger than L2, no flush",
-                   "kernels": "reference (one thread per cell)" if args.reference_kernels else "tiled",
+                   "kernels": "reference (one thread per cell)" if args.reference_kernels else
+                              ("tiled, dense sweep" if args.dense else "tiled, tile-class skipping"),
                    "result_finite_nonzero": finite},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d / total,
@@ -404,6 +412,8 @@ def main():
     ap.add_argument("--reference-kernels", action="store_true",
                     help="debug: time the one-thread-per-cell kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense", action="store_true",
+                    help="BVFDTD_FLAG_DENSE: sweep every array everywhere (no tile-class skipping)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

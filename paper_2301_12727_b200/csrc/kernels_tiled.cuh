@@ -86,6 +86,7 @@ struct StagePlan {
     int wxb;               // x-psi box width in floats
     int bytes;             // stage size (multiple of 128)
     int ns;                // pipeline stages
+    int pf;                // L2 prefetch distance in planes (0 = off)
     int smem;              // dynamic shared memory of the launch
 };
 
@@ -133,6 +134,32 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
         ::"r"(smem_u32(dst)), "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int x, int y, int z, int f) {
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(map), "r"(x), "r"(y), "r"(z), "r"(f) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *map, int x, int y, int z) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                 ::"l"(map), "r"(x), "r"(y), "r"(z) : "memory");
+}
+// One box: either a load into the stage (counting its bytes for the barrier) or, PF = true, an L2
+// prefetch of the same box for an iteration a few planes ahead.  The prefetch moves the DRAM latency
+// out of the shared-memory pipeline: L2 (126 MB) holds the bytes in flight, the stages only have to
+// cover the L2 -> SM hop.
+template <bool PF>
+struct Tma {
+    unsigned char *st;
+    uint64_t *bar;
+    uint32_t bytes;
+    __device__ __forceinline__ void box4(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z, int f) {
+        if (PF) tma_prefetch_4d(map, x, y, z, f);
+        else { tma_load_4d(st + off, map, bar, x, y, z, f); bytes += nbytes; }
+    }
+    __device__ __forceinline__ void box3(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z) {
+        if (PF) tma_prefetch_3d(map, x, y, z);
+        else { tma_load_3d(st + off, map, bar, x, y, z); bytes += nbytes; }
+    }
+};
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap *m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");
 }
@@ -328,6 +355,68 @@ enum : uint32_t {
     VC_ZS1 = 256u, VC_ZS2 = 512u             // plane m-1 / m-2 lies in a z slab (and inside the chunk)
 };
 
+// The loads of one velocity iteration m, derived from the chunk range and the flag words of planes
+// m-3..m (hist, 4 bits per plane, newest lowest).  The same routine issues the real loads and, a few
+// planes ahead, their L2 prefetches.
+template <class C>
+struct VelIssue {
+    const TiledMaps *maps; const Params *p; const StagePlan *sp;
+    TileX tX; bool tY; int jy0, x0, y0, kz0, kz1;
+    __device__ __forceinline__ uint32_t ctrl(int m, uint32_t hist) const {
+        const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
+        const uint32_t fl = hist & 15u, any = (hist | (hist >> 4) | (hist >> 8) | (hist >> 12)) & 15u;
+        uint32_t c = (in0 ? VC_IN0 : 0u) | (in1 ? VC_IN1 : 0u) | (in2 ? VC_IN2 : 0u);
+        if (fl & TF_XY) c |= VC_XY;
+        if (fl & TF_XZ) c |= VC_XZ;
+        if (fl & TF_YZ) c |= VC_YZ;
+        if (any & TF_XZ) c |= VC_WXZ;
+        if (any & TF_YZ) c |= VC_WYZ;
+        if (in1 && z_in_slab(*p, m - 1)) c |= VC_ZS1;
+        if (in2 && z_in_slab(*p, m - 2)) c |= VC_ZS2;
+        return c;
+    }
+    template <bool PF>
+    __device__ __forceinline__ void run(Tma<PF> &t, int m, uint32_t hist) const {
+        using VS = VStage<C>;
+        const uint32_t c = ctrl(m, hist);
+        const bool xy = c & VC_XY, xz = c & VC_XZ, yz = c & VC_YZ;
+        const uint32_t xbox = (uint32_t)sp->wxb * C::TY * 4;
+        const int z = m + 2;
+        t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, SZZ);
+        if (xz) t.box4(VS::SXZ, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXZ);
+        if (yz) t.box4(VS::SYZ, C::B_BYTES, &maps->boxB, x0, y0 - 2, z, SYZ);
+        if (c & VC_IN0) {
+            t.box4(VS::SXX, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXX);
+            t.box4(VS::SYY, C::B_BYTES, &maps->boxB, x0, y0 - 1, z, SYY);
+            if (xy) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, SXY);
+            // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
+            const bool use[3] = {true, xy, xz};
+            const bool usey[3] = {xy, true, yz};
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                if (use[q]) {
+                    const int d = sp->psx + q * sp->xt;
+                    if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, q);
+                    if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, q);
+                }
+                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, q);
+            }
+        }
+        if (c & VC_IN1) {
+            t.box4(VS::VXO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, VX);
+            t.box4(VS::VYO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, VY);
+        }
+        if (c & VC_IN2) t.box4(VS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, VZ);
+        if (c & VC_ZS1) {
+            const int kc = z_compact(*p, m - 1);
+            if (c & VC_WXZ) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, kc, 0);
+            if (c & VC_WYZ) t.box4(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, kc, 1);
+        }
+        if (c & VC_ZS2) t.box4(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 2);
+        t.box3(VS::MAT, C::MX * C::MY, &maps->mat, x0, y0, m - 1);
+    }
+};
+
 template <class C, bool EDGE>
 __device__ __forceinline__ void velocity_consume(const Params &p, const StagePlan &sp, unsigned char *stages, const float *rho_tab,
                                                  const float *sprof, uint64_t *full, uint64_t *empty, int tid, int x0, int y0,
@@ -498,83 +587,40 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
         // ================= producer warp =================
         if (tid == C::NC) {
             const uint32_t *flags = p.flagsV + (size_t)(blockIdx.x + p.ntxV * blockIdx.y) * (p.nz + 4) + 2;
-            const TileX tX = make_tilex<C>(p, x0);
-            const bool tY = tile_in_y<C>(p, y0);
-            const int jy0 = tile_jy0<C>(p, y0);
+            VelIssue<C> iss;
+            iss.maps = &maps; iss.p = &p; iss.sp = &sp;
+            iss.tX = make_tilex<C>(p, x0); iss.tY = tile_in_y<C>(p, y0); iss.jy0 = tile_jy0<C>(p, y0);
+            iss.x0 = x0; iss.y0 = y0; iss.kz0 = kz0; iss.kz1 = kz1;
             prefetch_tmap(&maps.boxA); prefetch_tmap(&maps.boxB); prefetch_tmap(&maps.boxC);
             prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
-            uint32_t hxz = 0, hyz = 0;
-            const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
-            const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
-            uint32_t fl_next = __ldg(flags + m_begin);
+            uint32_t hist = 0, hist_pf = 0;       // flag words of the last planes, 4 bits each (newest in the low nibble)
+            // prefetch stream: runs sp.pf planes ahead of the load stream
+            int mp = m_begin;
+            if (sp.pf > 0) {
+                for (; mp < min(m_end, m_begin + sp.pf); ++mp) hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);   // loaded directly
+            }
             for (int m = m_begin; m < m_end; ++m) {
-                const uint32_t fl = fl_next;
-                fl_next = __ldg(flags + min(m + 1, p.nz + 1));
-                const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
-                const bool xy = (fl & TF_XY) != 0, xz = (fl & TF_XZ) != 0, yz = (fl & TF_YZ) != 0;
-                hxz = ((hxz << 1) | (xz ? 1u : 0u)) & 15u;
-                hyz = ((hyz << 1) | (yz ? 1u : 0u)) & 15u;
-                const bool wxz = hxz != 0, wyz = hyz != 0;
-                const bool zs1 = in1 && z_in_slab(p, m - 1), zs2 = in2 && z_in_slab(p, m - 2);
+                if (sp.pf > 0 && mp < m_end) {
+                    hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
+                    Tma<true> t{nullptr, nullptr, 0};
+                    iss.run(t, mp, hist_pf);
+                    ++mp;
+                }
+                hist = (hist << 4) | (__ldg(flags + m) & 15u);
                 StageHdr h;
-                h.ctrl = (in0 ? VC_IN0 : 0u) | (in1 ? VC_IN1 : 0u) | (in2 ? VC_IN2 : 0u) | (xy ? VC_XY : 0u) | (xz ? VC_XZ : 0u) |
-                         (yz ? VC_YZ : 0u) | (wxz ? VC_WXZ : 0u) | (wyz ? VC_WYZ : 0u) | (zs1 ? VC_ZS1 : 0u) | (zs2 ? VC_ZS2 : 0u);
+                h.ctrl = iss.ctrl(m, hist);
                 h.az1 = h.bz1 = h.az2 = h.bz2 = 0.0f;
-                if (zs1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
-                if (zs2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
+                if (h.ctrl & VC_ZS1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
+                if (h.ctrl & VC_ZS2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
                 mbar_wait(&empty[s], ph ^ 1);
                 unsigned char *st = stages + s * sp.bytes;
-                uint64_t *bar = &full[s];
                 StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
                 hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
-                uint32_t bytes = C::D_BYTES + C::MX * C::MY;                       // szz, mat
-                if (xz) bytes += C::A_BYTES;
-                if (yz) bytes += C::B_BYTES;
-                if (in0) {
-                    bytes += C::A_BYTES + C::B_BYTES + (xy ? C::C_BYTES : 0);
-                    bytes += nx_boxes * xbox * (1u + (xy ? 1u : 0u) + (xz ? 1u : 0u));
-                    if (tY) bytes += C::D_BYTES * (1u + (xy ? 1u : 0u) + (yz ? 1u : 0u));
-                }
-                if (in1) bytes += 2 * C::D_BYTES;
-                if (in2) bytes += C::D_BYTES;
-                if (zs1) bytes += C::D_BYTES * ((wxz ? 1u : 0u) + (wyz ? 1u : 0u));
-                if (zs2) bytes += C::D_BYTES;
-                mbar_expect_tx(bar, bytes);
-                const int z = m + 2;
-                tma_load_4d(st + VS::SZZ, &maps.boxD, bar, x0, y0, z, SZZ);
-                if (xz) tma_load_4d(st + VS::SXZ, &maps.boxA, bar, x0 - 4, y0, z, SXZ);
-                if (yz) tma_load_4d(st + VS::SYZ, &maps.boxB, bar, x0, y0 - 2, z, SYZ);
-                if (in0) {
-                    tma_load_4d(st + VS::SXX, &maps.boxA, bar, x0 - 4, y0, z, SXX);
-                    tma_load_4d(st + VS::SYY, &maps.boxB, bar, x0, y0 - 1, z, SYY);
-                    if (xy) tma_load_4d(st + VS::SXY, &maps.boxC, bar, x0 - 4, y0 - 2, z, SXY);
-                    // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
-                    const bool use[3] = {true, xy, xz};
-                    const bool usey[3] = {xy, true, yz};
-#pragma unroll
-                    for (int t = 0; t < 3; ++t) {
-                        if (use[t]) {
-                            unsigned char *d = st + sp.psx + t * sp.xt;
-                            if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, t);
-                            if (tX.hi) tma_load_4d(d + sp.xhi, &maps.psx, bar, tX.cx_hi, y0, m, t);
-                        }
-                        if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, t);
-                    }
-                }
-                if (in1) {
-                    tma_load_4d(st + VS::VXO, &maps.boxD, bar, x0, y0, z - 1, VX);
-                    tma_load_4d(st + VS::VYO, &maps.boxD, bar, x0, y0, z - 1, VY);
-                }
-                if (in2) tma_load_4d(st + VS::VZO, &maps.boxD, bar, x0, y0, z - 2, VZ);
-                if (zs1) {
-                    const int kc = z_compact(p, m - 1);
-                    if (wxz) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, kc, 0);
-                    if (wyz) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, kc, 1);
-                }
-                if (zs2) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 2);
-                tma_load_3d(st + VS::MAT, &maps.mat, bar, x0, y0, m - 1);
+                Tma<false> t{st, &full[s], 0};
+                iss.run(t, m, hist);
+                mbar_expect_tx(&full[s], t.bytes);   // the arrival that lets the phase complete comes after the loads
                 if (++s == sp.ns) { s = 0; ph ^= 1; }
             }
         }
@@ -623,6 +669,76 @@ __device__ __forceinline__ void shear_update(const ShearCoef &k, float g, float 
     rn = fmaf(A, r0, -(k.cR * g));
     sn = s0 + fmaf(k.cU, g, hdt * (rn + r0));
 }
+
+// The loads of one stress iteration m (flag words of planes m, m-1, m-2 in hist, 4 bits each,
+// newest lowest); issues the real loads or, a few planes ahead, their L2 prefetches.
+template <class C>
+struct StrIssue {
+    const TiledMaps *maps; const Params *p; const StagePlan *sp;
+    TileX tX; bool tY; int jy0, x0, y0, kz0, kz1;
+    uint32_t sens;
+    __device__ __forceinline__ uint32_t ctrl(int m, uint32_t hist) const {
+        const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
+        const uint32_t f0 = hist & 15u, f1 = (hist >> 4) & 15u, f2 = (hist >> 8) & 15u;
+        uint32_t c = sens;
+        if (in0) c |= SC_IN0 | ((f0 & TF_XY) ? SC_XY0 : 0u) | ((f0 & TF_XZ) ? SC_XZ0 : 0u) | ((f0 & TF_YZ) ? SC_YZ0 : 0u);
+        if (in1) c |= SC_IN1 | ((f1 & TF_RII) ? SC_RII1 : 0u) | (z_in_slab(*p, m - 1) ? SC_ZS1 : 0u);
+        if (in2) c |= SC_IN2 | ((f2 & TF_XZ) ? SC_XZ2 : 0u) | ((f2 & TF_YZ) ? SC_YZ2 : 0u) | (z_in_slab(*p, m - 2) ? SC_ZS2 : 0u);
+        return c;
+    }
+    // mat_off: offset of the material ring slot of plane m relative to the stage base (loads only)
+    template <bool PF>
+    __device__ __forceinline__ void run(Tma<PF> &t, int m, uint32_t hist, int mat_off) const {
+        using SS = SStage<C>;
+        const uint32_t c = ctrl(m, hist);
+        const uint32_t xbox = (uint32_t)sp->wxb * C::TY * 4;
+        const int z = m + 2;
+        t.box4(SS::VXB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VX);
+        t.box4(SS::VYB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VY);
+        t.box4(SS::VZB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VZ);
+        if (c & SC_IN0) {
+            // psi of the x-y derivatives of plane m: x terms 3 (D-x vx), 4 (D+x vy), 5 (D+x vz);
+            // y terms 3 (D+y vx), 4 (D-y vy), 5 (D+y vz)
+            const bool use[3] = {true, (c & SC_XY0) != 0, (c & SC_XZ0) != 0};
+            const bool usey[3] = {(c & SC_XY0) != 0, true, (c & SC_YZ0) != 0};
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                if (use[q]) {
+                    const int d = sp->psx + q * sp->xt;
+                    if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, 3 + q);
+                    if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, 3 + q);
+                }
+                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, 3 + q);
+            }
+        }
+        if (c & SC_XY0) {
+            t.box4(SS::SXY, C::D_BYTES, &maps->boxD, x0, y0, z, SXY);
+            t.box4(SS::RXY, C::D_BYTES, &maps->boxD, x0, y0, z, RXY);
+        }
+        if (c & SC_IN1) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) t.box4(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, SXX + q);
+            if (c & SC_RII1) {
+#pragma unroll
+                for (int q = 0; q < 3; ++q) t.box4(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
+            }
+            if (c & SC_PEAK) t.box4(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, F_PEAK);
+            if (c & SC_RMS) t.box4(SS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 1, F_SUMSQ);
+            if (c & SC_ZS1) t.box4(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 1), 5);
+        }
+        if (c & SC_XZ2) {
+            t.box4(SS::SXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SXZ);
+            t.box4(SS::RXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RXZ);
+            if (c & SC_ZS2) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 3);
+        }
+        if (c & SC_YZ2) {
+            t.box4(SS::SYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SYZ);
+            t.box4(SS::RYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RYZ);
+            if (c & SC_ZS2) t.box4(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 4);
+        }
+        t.box3(mat_off, C::MX * C::MY, &maps->mat, x0, y0, m);
+    }
+};
 
 template <class C, bool EDGE>
 __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan &sp, unsigned char *stages, unsigned char *mat_ring,
@@ -843,96 +959,43 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
     __syncthreads();
 
     if (tid >= C::NC) {
+        // ================= producer warp =================
         if (tid == C::NC) {
             const uint32_t *flags = p.flagsS + (size_t)(blockIdx.x + p.ntxS * blockIdx.y) * (p.nz + 4) + 2;
-            const bool do_peak = p.do_peak != 0, do_rms = p.do_rms != 0;
-            const TileX tX = make_tilex<C>(p, x0);
-            const bool tY = tile_in_y<C>(p, y0);
-            const int jy0 = tile_jy0<C>(p, y0);
+            StrIssue<C> iss;
+            iss.maps = &maps; iss.p = &p; iss.sp = &sp;
+            iss.tX = make_tilex<C>(p, x0); iss.tY = tile_in_y<C>(p, y0); iss.jy0 = tile_jy0<C>(p, y0);
+            iss.x0 = x0; iss.y0 = y0; iss.kz0 = kz0; iss.kz1 = kz1;
+            iss.sens = (p.do_peak ? SC_PEAK : 0u) | (p.do_rms ? SC_RMS : 0u);
             prefetch_tmap(&maps.boxC); prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
             int mr = ((m_begin % MR) + MR) % MR;
-            uint32_t f1 = 0, f2 = 0;
-            const uint32_t xbox = (uint32_t)sp.wxb * C::TY * 4;
-            const uint32_t nx_boxes = (tX.lo ? 1u : 0u) + (tX.hi ? 1u : 0u);
-            uint32_t fl_next = __ldg(flags + m_begin);
+            uint32_t hist = 0, hist_pf = 0;       // flag words of planes m, m-1, m-2 ..., 4 bits each
+            int mp = m_begin;
+            if (sp.pf > 0) {
+                for (; mp < min(m_end, m_begin + sp.pf); ++mp) hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
+            }
             for (int m = m_begin; m < m_end; ++m) {
-                const uint32_t f0 = fl_next;
-                fl_next = __ldg(flags + min(m + 1, p.nz + 1));
-                const bool in0 = m >= kz0 && m < kz1, in1 = m - 1 >= kz0 && m - 1 < kz1, in2 = m - 2 >= kz0 && m - 2 < kz1;
-                const bool xy0 = in0 && (f0 & TF_XY), xz0 = in0 && (f0 & TF_XZ), yz0 = in0 && (f0 & TF_YZ);
-                const bool rii1 = in1 && (f1 & TF_RII);
-                const bool xz2 = in2 && (f2 & TF_XZ), yz2 = in2 && (f2 & TF_YZ);
-                f2 = f1; f1 = f0;
-                const bool zs1 = in1 && z_in_slab(p, m - 1), zs2 = in2 && z_in_slab(p, m - 2);
+                if (sp.pf > 0 && mp < m_end) {
+                    hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
+                    Tma<true> t{nullptr, nullptr, 0};
+                    iss.run(t, mp, hist_pf, 0);
+                    ++mp;
+                }
+                hist = (hist << 4) | (__ldg(flags + m) & 15u);
                 StageHdr h;
-                h.ctrl = (in0 ? SC_IN0 : 0u) | (in1 ? SC_IN1 : 0u) | (in2 ? SC_IN2 : 0u) | (xy0 ? SC_XY0 : 0u) | (xz0 ? SC_XZ0 : 0u) |
-                         (yz0 ? SC_YZ0 : 0u) | (rii1 ? SC_RII1 : 0u) | (xz2 ? SC_XZ2 : 0u) | (yz2 ? SC_YZ2 : 0u) | (zs1 ? SC_ZS1 : 0u) |
-                         (zs2 ? SC_ZS2 : 0u) | (do_peak ? SC_PEAK : 0u) | (do_rms ? SC_RMS : 0u);
+                h.ctrl = iss.ctrl(m, hist);
                 h.az1 = h.bz1 = h.az2 = h.bz2 = 0.0f;
-                if (zs1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
-                if (zs2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
+                if (h.ctrl & SC_ZS1) { h.az1 = __ldg(p.prof[2][0] + m - 1); h.bz1 = __ldg(p.prof[2][1] + m - 1); }
+                if (h.ctrl & SC_ZS2) { h.az2 = __ldg(p.prof[2][2] + m - 2); h.bz2 = __ldg(p.prof[2][3] + m - 2); }
                 mbar_wait(&empty[s], ph ^ 1);
                 unsigned char *st = stages + s * sp.bytes;
-                uint64_t *bar = &full[s];
                 StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
                 hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
-                uint32_t bytes = 3 * C::C_BYTES + C::MX * C::MY;
-                if (in0) {
-                    bytes += nx_boxes * xbox * (1u + (xy0 ? 1u : 0u) + (xz0 ? 1u : 0u));
-                    if (tY) bytes += C::D_BYTES * (1u + (xy0 ? 1u : 0u) + (yz0 ? 1u : 0u));
-                }
-                if (xy0) bytes += 2 * C::D_BYTES;
-                if (in1) bytes += C::D_BYTES * (3u + (rii1 ? 3u : 0u) + (do_peak ? 1u : 0u) + (do_rms ? 1u : 0u) + (zs1 ? 1u : 0u));
-                if (xz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
-                if (yz2) bytes += C::D_BYTES * (2u + (zs2 ? 1u : 0u));
-                mbar_expect_tx(bar, bytes);
-                const int z = m + 2;
-                tma_load_4d(st + SS::VXB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VX);
-                tma_load_4d(st + SS::VYB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VY);
-                tma_load_4d(st + SS::VZB, &maps.boxC, bar, x0 - 4, y0 - 2, z, VZ);
-                if (in0) {
-                    // psi of the x-y derivatives of plane m: x terms 3 (D-x vx), 4 (D+x vy), 5 (D+x vz);
-                    // y terms 3 (D+y vx), 4 (D-y vy), 5 (D+y vz)
-                    const bool use[3] = {true, xy0, xz0};
-                    const bool usey[3] = {xy0, true, yz0};
-#pragma unroll
-                    for (int t = 0; t < 3; ++t) {
-                        if (use[t]) {
-                            unsigned char *d = st + sp.psx + t * sp.xt;
-                            if (tX.lo) tma_load_4d(d, &maps.psx, bar, tX.cx_lo, y0, m, 3 + t);
-                            if (tX.hi) tma_load_4d(d + sp.xhi, &maps.psx, bar, tX.cx_hi, y0, m, 3 + t);
-                        }
-                        if (tY && usey[t]) tma_load_4d(st + sp.psy + t * C::D_BYTES, &maps.psy, bar, x0, jy0, m, 3 + t);
-                    }
-                }
-                if (xy0) {
-                    tma_load_4d(st + SS::SXY, &maps.boxD, bar, x0, y0, z, SXY);
-                    tma_load_4d(st + SS::RXY, &maps.boxD, bar, x0, y0, z, RXY);
-                }
-                if (in1) {
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::SII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, SXX + q);
-                    if (rii1) {
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) tma_load_4d(st + SS::RII + q * C::D_BYTES, &maps.boxD, bar, x0, y0, z - 1, RXX + q);
-                    }
-                    if (do_peak) tma_load_4d(st + SS::PEAK, &maps.boxD, bar, x0, y0, z - 1, F_PEAK);
-                    if (do_rms) tma_load_4d(st + SS::SUMSQ, &maps.boxD, bar, x0, y0, z - 1, F_SUMSQ);
-                    if (zs1) tma_load_4d(st + sp.psz + 2 * C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 1), 5);
-                }
-                if (xz2) {
-                    tma_load_4d(st + SS::SXZ, &maps.boxD, bar, x0, y0, z - 2, SXZ);
-                    tma_load_4d(st + SS::RXZ, &maps.boxD, bar, x0, y0, z - 2, RXZ);
-                    if (zs2) tma_load_4d(st + sp.psz, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 3);
-                }
-                if (yz2) {
-                    tma_load_4d(st + SS::SYZ, &maps.boxD, bar, x0, y0, z - 2, SYZ);
-                    tma_load_4d(st + SS::RYZ, &maps.boxD, bar, x0, y0, z - 2, RYZ);
-                    if (zs2) tma_load_4d(st + sp.psz + C::D_BYTES, &maps.psz, bar, x0, y0, z_compact(p, m - 2), 4);
-                }
-                tma_load_3d(mat_ring + mr * C::M_BYTES, &maps.mat, bar, x0, y0, m);
+                Tma<false> t{st, &full[s], 0};
+                iss.run(t, m, hist, (int)(mat_ring + mr * C::M_BYTES - st));
+                mbar_expect_tx(&full[s], t.bytes);   // the arrival that lets the phase complete comes after the loads
                 if (++mr == MR) mr = 0;
                 if (++s == sp.ns) { s = 0; ph ^= 1; }
             }
@@ -1090,6 +1153,8 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
     s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
     s.ns = ns;
+    s.pf = 0;   // off: on B200 the TMA L2 prefetch slowed both passes (profiles/r1c notes)
+    if (const char *c = std::getenv("BVFDTD_PF")) s.pf = std::max(0, std::min(8, std::atoi(c)));
     s.smem = ns * s.bytes + extra;
     return s;
 }
