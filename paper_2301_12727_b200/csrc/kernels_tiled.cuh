@@ -1138,13 +1138,14 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
 }
 
 template <class C>
-inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb) {
+inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb, int hdr_at = -1) {
     StagePlan s;
     s.wxb = wxb;
     s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
     s.yb = C::D_BYTES;
-    s.hdr = fixed;
-    s.psx = s.hdr + 128;
+    // header: its own 128 bytes, or (hdr_at >= 0) the unused tail of an existing slot
+    s.hdr = hdr_at >= 0 ? hdr_at : fixed;
+    s.psx = hdr_at >= 0 ? fixed : fixed + 128;
     // a tile touches both x slabs only on grids narrower than a tile + the slabs
     const bool both = L.P > 0 && (C::TX > L.xhb || L.P > C::TX);
     s.xhi = both ? s.xb : 0;
@@ -1187,8 +1188,14 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     int ns_v = env_v ? std::atoi(env_v) : 3, ns_s = env_s ? std::atoi(env_s) : 0;
     ns_v = std::max(2, std::min(MAX_STAGES, ns_v));
     const int v_extra = 256 * 4 + 4 * CfgV::TX * 4 + bar_bytes;
-    plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, ns_v, v_extra, wxb);
-    while (plan.sv.smem > smem_max && plan.sv.ns > 2) plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb);
+    // the velocity stage header lives in the slack of the material slot (720 of 768 bytes used)
+    static_assert(CfgV::M_BYTES - CfgV::MX * CfgV::MY >= (int)sizeof(StageHdr), "no room for the header behind the material box");
+    const int v_hdr = VStage<CfgV>::MAT + CfgV::M_BYTES - (int)sizeof(StageHdr);
+    plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, ns_v, v_extra, wxb, v_hdr);
+    // two resident CTAs per SM matter more than a third stage
+    const int smem_sm = 228 * 1024;
+    while (plan.sv.ns > 2 && (plan.sv.smem > smem_max || 2 * (plan.sv.smem + 1024) > smem_sm))
+        plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb, v_hdr);
     // stress pass: 64 x 16 tiles with 2 stages when they fit, else 64 x 8 tiles with up to 3 stages
     auto s_extra16 = [&](int ns) { return (ns + 3) * CfgS::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS::TX * 4 + bar_bytes; };
     auto s_extra8 = [&](int ns) { return (ns + 3) * CfgS8::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS8::TX * 4 + bar_bytes; };

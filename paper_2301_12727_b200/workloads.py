@@ -410,15 +410,20 @@ def blocky_domain(nx, ny, nz, pml, seed, steps=20, waveform=1, f0=500e3, dx=1e-3
                     n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
 
 
-def random_state(w: Workload, seed: int, scale_v: float = 1e-6) -> dict:
+def random_state(w: Workload, seed: int, scale_v: float = 1e-6, fields=None) -> dict:
     """Seeded random state for single-pass parity tests: 3 v, 6 sigma, 6 r as float32 arrays
-    shaped (nz, ny, nx) (values exactly representable in fp32 so both sides start equal)."""
+    shaped (nz, ny, nx) (values exactly representable in fp32 so both sides start equal).
+    ``fields``: draw only these (the others are left out of the result)."""
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + 2000 + seed))
     out = {}
-    for name in ("vx", "vy", "vz"):
-        out[name] = (scale_v * rng.standard_normal((w.nz, w.ny, w.nx))).astype(np.float32)
-    for name in ("sxx", "syy", "szz", "sxy", "sxz", "syz"):
-        out[name] = rng.standard_normal((w.nz, w.ny, w.nx)).astype(np.float32)
-    for name in ("rxx", "ryy", "rzz", "rxy", "rxz", "ryz"):
-        out[name] = (1e5 * rng.standard_normal((w.nz, w.ny, w.nx))).astype(np.float32)
+    shape = (w.nz, w.ny, w.nx)
+    for names, scale in ((("vx", "vy", "vz"), scale_v), (("sxx", "syy", "szz", "sxy", "sxz", "syz"), 1.0),
+                         (("rxx", "ryy", "rzz", "rxy", "rxz", "ryz"), 1e5)):
+        for name in names:
+            if fields is not None and name not in fields:
+                continue
+            a = rng.standard_normal(shape, dtype=np.float32)
+            if scale != 1.0:
+                a *= np.float32(scale)
+            out[name] = a
     return out

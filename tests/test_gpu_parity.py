@@ -265,6 +265,25 @@ def test_config2_full_size_short_run(bv):
     o.close()
 
 
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_config34_full_size_short_run(bv, cfg):
+    """Configs 3 (504x504x672, P 20, 255 materials) and 4 (480x480x600, P 24, array source) at their
+    full sizes in the default launch configuration (tile-class skipping on): 6 steps from a seeded
+    random velocity / normal-stress state (every cell carries data; shear stresses and memory
+    variables start at zero as in a real run), element by element against the fp64 oracle."""
+    w = wl.make(cfg, steps=6)
+    w.rms_begin = 3
+    st = wl.random_state(w, 7 + cfg, fields=("vx", "vy", "vz", "sxx", "syy", "szz"))
+    sim, o = run_both(bv, w, state=st)
+    del st
+    compare_state(sim, o, rel=1e-5)
+    peak, rms = sim.read_peak_pressure()
+    compare_map(peak, o.get("peak"), rel=1e-4)
+    compare_map(rms, o.get("rms_amp"), rel=1e-4)
+    sim.close()
+    o.close()
+
+
 def test_config2_tiled_vs_percell_kernels_long(bv):
     """Property at full size over a longer run: the tiled kernels and the one-thread-per-cell
     kernels implement the same arithmetic, so after 400 steps of config 2 their fields agree to

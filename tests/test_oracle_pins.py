@@ -139,6 +139,46 @@ def test_T2b_worked_numbers():
     assert Q < Q_lit and abs(Q / Q_lit - 1) < 0.05
 
 
+def _table1(f_hz):
+    """tests/golden/table1_materials.csv evaluated at frequency f."""
+    import os
+    rows = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "table1_materials.csv")):
+        if line.startswith("#") or not line.strip():
+            continue
+        n, rho, cl0, cls, cs0, css, al, as_ = line.strip().split(",")
+        f = float(f_hz)
+        rows[n] = (float(rho), float(cl0) + float(cls) * f, float(cs0) + float(css) * f,
+                   float(al) * f / 1e6, float(as_) * f / 1e6)
+    return rows
+
+
+@pytest.mark.parametrize("f_hz", [250e3, 500e3, 700e3, 1e6])
+def test_paper_table1_materials_are_representable(f_hz):
+    """Every row of the paper's Table 1, at the frequencies the paper uses (200 kHz - 1 MHz, L35),
+    is accepted by S0, and the one-mechanism SLS built from it reproduces the printed speed and
+    attenuation at f (Eq. 3): Q = w/(2 c alpha) within its low-loss approximation."""
+    w0 = 2 * math.pi * f_hz
+    rows = _table1(f_hz)
+    assert abs(rows["cortical"][1] - (2415 + 1.2e-4 * f_hz)) < 1e-9
+    der = fo.derive_materials(list(rows.values()), f_hz)
+    for (name, (rho, cL, cS, aL, aS)), d in zip(rows.items(), der):
+        dd = dict(zip(fo.DERIVED, d))
+        for c, a, MR, tau in ((cL, aL, dd["pi_R"], dd["tau_p"]), (cS, aS, dd["mu_R"], dd["tau_s"])):
+            if c == 0.0 or a == 0.0:
+                continue
+            M = MR * (1.0 + tau * 1j / (1.0 + 1j))
+            k = w0 * cmath.sqrt(rho / M)
+            assert abs(w0 / k.real - c) <= 1e-11 * c, name
+            assert abs(-k.imag - a) <= 1e-9 * a, name
+            Q_eq3 = w0 / (2.0 * c * a)                           # Eq. 3 of the paper
+            Q = M.real / M.imag
+            assert abs(Q / Q_eq3 - 1.0) < 0.75 / Q_eq3 ** 2 + 1e-12, (name, Q, Q_eq3)   # low-loss limit
+    # cortical bone at 500 kHz: Q_L = 7.787 by Eq. 3 (c_L 2475 m/s, alpha_L 81.5 Np/m)
+    if f_hz == 500e3:
+        assert abs(w0 / (2 * rows["cortical"][1] * rows["cortical"][3]) - 7.787) < 5e-3
+
+
 def test_invalid_rows_rejected():
     for row in [(0.0, 1500, 0, 0, 0), (1000, 0.0, 0, 0, 0), (1000, 1500, -1, 0, 0),
                 (1000, 1500, 1400, 0, 0),                        # cS >= sqrt(3)/2 cL
