@@ -90,11 +90,21 @@ struct StagePlan {
     int smem;              // dynamic shared memory of the launch
 };
 
+// z chunks of a launch: chunk c covers planes [b[c], b[c+1]).  Blocks are dispatched in blockIdx.z
+// order, so the long chunks come first and a few short ones last: they fill the gaps the last wave
+// would otherwise leave (the passes run at the memory system's ceiling while all SMs are busy; the
+// idle tail was 7-12 % of the kernel time with equal chunks).
+constexpr int MAX_CHUNKS = 48;
+struct ZChunks {
+    int n;
+    int b[MAX_CHUNKS + 1];
+};
+
 struct TiledPlan {
     TiledMaps mv, ms;      // velocity / stress pass (their tiles differ)
     StagePlan sv, ss;
     bool s16 = true;       // stress pass runs 64 x 16 tiles (else 64 x 8)
-    int chunks_v = 1, nzc_v = 0, chunks_s = 1, nzc_s = 0;
+    ZChunks zv, zs;        // z chunks of the velocity / stress launch
     bool ready = false;
 };
 
@@ -560,7 +570,7 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
 
 template <class C>
 __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
-                                                             const int nzc, const StagePlan sp) {
+                                                             const ZChunks zc, const StagePlan sp) {
     using VS = VStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
@@ -571,7 +581,7 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
 
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
+    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
     const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
 
     for (int q = tid; q < 256; q += C::NT) rho_tab[q] = p.rows[q].rho;
@@ -928,7 +938,7 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
 
 template <class C>
 __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
-                                                           const int nzc, const StagePlan sp) {
+                                                           const ZChunks zc, const StagePlan sp) {
     using SS = SStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
@@ -942,7 +952,7 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
 
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int kz0 = blockIdx.z * nzc, kz1 = min(p.nz, kz0 + nzc);
+    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
     const int m_begin = kz0 - 2, m_end = kz1 + 2;
 
     for (int q = tid; q < 256; q += C::NT) {
@@ -1064,21 +1074,37 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
 
 inline int round128(int v) { return (v + 127) / 128 * 128; }
 
-// z chunks: whole waves of resident CTAs cost (planes + 4 priming planes) each; half a wave is added
-// for the imbalance between all-fluid and partly solid tiles (measured on config 2: 14 chunks of 33
-// planes beat 3 chunks of 150 by 8 % in spite of the extra priming planes)
-inline void plan_chunks(int nz, long long tiles, long long slots, int &chunks, int &nzc) {
-    int best = 1;
-    double best_cost = 1e300;
-    for (int ch = 1; ch <= (nz + 7) / 8; ++ch) {
-        const int n = (nz + ch - 1) / ch;
-        const long long blocks = tiles * ((nz + n - 1) / n);
-        const double waves = (double)((blocks + slots - 1) / slots);
-        const double cost = (waves + 0.5) * (n + 4);
-        if (cost < best_cost - 1e-9) { best_cost = cost; best = ch; }
+// z chunks: a few long equal chunks (about 2.6 waves of resident CTAs; every chunk costs 4 priming
+// planes) followed by a tail of chunks of halving length, not below 8 planes.  Measured on config 2:
+// 90 90 90 90 45 25 12 8 planes -> 39.0 Gcell/s, nine equal chunks of 50 -> 36.6, three of 150 -> 33.6.
+inline ZChunks plan_chunks(int nz, long long tiles, long long slots, double waves) {
+    ZChunks z;
+    int big = (int)std::floor(waves * (double)slots / (double)tiles + 0.5);
+    big = std::max(1, std::min(big, std::min(nz / 16, MAX_CHUNKS - 8)));
+    const int len = std::max(8, (nz + big) / (big + 1));
+    int pos = 0, n = 0;
+    z.b[0] = 0;
+    while (n < big && nz - pos >= len + 8) { pos += len; z.b[++n] = pos; }
+    while (nz - pos >= 16 && n < MAX_CHUNKS - 1) { pos += (nz - pos + 1) / 2; z.b[++n] = pos; }
+    if (pos < nz) z.b[++n] = nz;
+    z.n = n;
+    return z;
+}
+inline bool parse_chunks(const char *env, int nz, ZChunks &z) {   // "56,56,...": explicit lengths (experiments)
+    if (!env) return false;
+    int pos = 0, n = 0;
+    z.b[0] = 0;
+    const char *c = env;
+    while (*c && n < MAX_CHUNKS && pos < nz) {
+        const int len = std::atoi(c);
+        if (len <= 0) break;
+        pos = std::min(nz, pos + len); z.b[++n] = pos;
+        while (*c && *c != ',') ++c;
+        if (*c == ',') ++c;
     }
-    nzc = (nz + best - 1) / best;
-    chunks = (nz + nzc - 1) / nzc;
+    if (pos < nz && n < MAX_CHUNKS) z.b[++n] = nz;
+    z.n = n;
+    return n > 0 && z.b[n] == nz;
 }
 
 template <class C>
@@ -1236,14 +1262,20 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
         (void)cudaGetLastError();
         return BVFDTD_ECUDA;
     }
-    plan_chunks(L.nz, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, plan.chunks_v, plan.nzc_v);
-    plan_chunks(L.nz, (long long)L.ntxS * L.ntyS, (long long)std::max(1, occ_s) * sms, plan.chunks_s, plan.nzc_s);
-    if (const char *c = std::getenv("BVFDTD_CHUNKS_V")) { plan.chunks_v = std::max(1, std::atoi(c)); plan.nzc_v = (L.nz + plan.chunks_v - 1) / plan.chunks_v; plan.chunks_v = (L.nz + plan.nzc_v - 1) / plan.nzc_v; }
-    if (const char *c = std::getenv("BVFDTD_CHUNKS_S")) { plan.chunks_s = std::max(1, std::atoi(c)); plan.nzc_s = (L.nz + plan.chunks_s - 1) / plan.chunks_s; plan.chunks_s = (L.nz + plan.nzc_s - 1) / plan.nzc_s; }
-    if (std::getenv("BVFDTD_VERBOSE"))
-        std::fprintf(stderr, "[bvfdtd] velocity: ns %d stage %d smem %d occ %d chunks %d x %d planes; stress: ns %d stage %d smem %d occ %d chunks %d x %d planes\n",
-                     plan.sv.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.chunks_v, plan.nzc_v, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s,
-                     plan.chunks_s, plan.nzc_s);
+    const char *env_w = std::getenv("BVFDTD_WAVES");
+    const double waves = env_w ? std::atof(env_w) : 2.6;
+    plan.zv = plan_chunks(L.nz, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, waves);
+    plan.zs = plan_chunks(L.nz, (long long)L.ntxS * L.ntyS, (long long)std::max(1, occ_s) * sms, waves);
+    parse_chunks(std::getenv("BVFDTD_ZB_V"), L.nz, plan.zv);
+    parse_chunks(std::getenv("BVFDTD_ZB_S"), L.nz, plan.zs);
+    if (std::getenv("BVFDTD_VERBOSE")) {
+        std::fprintf(stderr, "[bvfdtd] velocity: ns %d stage %d smem %d occ %d; stress: tile 64x%d ns %d stage %d smem %d occ %d\n[bvfdtd] z chunks velocity:",
+                     plan.sv.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.s16 ? 16 : 8, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s);
+        for (int c = 0; c < plan.zv.n; ++c) std::fprintf(stderr, " %d", plan.zv.b[c + 1] - plan.zv.b[c]);
+        std::fprintf(stderr, "; stress:");
+        for (int c = 0; c < plan.zs.n; ++c) std::fprintf(stderr, " %d", plan.zs.b[c + 1] - plan.zs.b[c]);
+        std::fprintf(stderr, "\n");
+    }
     plan.ready = true;
     return 0;
 }
@@ -1256,12 +1288,12 @@ inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV
     else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_velocity_tiled<CfgV><<<dim3(p.ntxV, p.ntyV, plan.chunks_v), CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.nzc_v, plan.sv);
+    k_velocity_tiled<CfgV><<<dim3(p.ntxV, p.ntyV, plan.zv.n), CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv);
     return 0;
 }
 inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    if (plan.s16) k_stress_tiled<CfgS><<<dim3(p.ntxS, p.ntyS, plan.chunks_s), CfgS::NT, plan.ss.smem, st>>>(plan.ms, p, plan.nzc_s, plan.ss);
-    else k_stress_tiled<CfgS8><<<dim3(p.ntxS, p.ntyS, plan.chunks_s), CfgS8::NT, plan.ss.smem, st>>>(plan.ms, p, plan.nzc_s, plan.ss);
+    if (plan.s16) k_stress_tiled<CfgS><<<dim3(p.ntxS, p.ntyS, plan.zs.n), CfgS::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss);
+    else k_stress_tiled<CfgS8><<<dim3(p.ntxS, p.ntyS, plan.zs.n), CfgS8::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss);
     return 0;
 }
 
