@@ -1080,7 +1080,7 @@ inline int round128(int v) { return (v + 127) / 128 * 128; }
 inline ZChunks plan_chunks(int nz, long long tiles, long long slots, double waves) {
     ZChunks z;
     int big = (int)std::floor(waves * (double)slots / (double)tiles + 0.5);
-    big = std::max(1, std::min(big, std::min(nz / 16, MAX_CHUNKS - 8)));
+    big = std::max(1, std::min(big, std::min(nz / 8, MAX_CHUNKS - 8)));
     const int len = std::max(8, (nz + big) / (big + 1));
     int pos = 0, n = 0;
     z.b[0] = 0;
