@@ -214,6 +214,44 @@ int bvfdtd_pml_mask(const bvfdtd_grid *grid, uint8_t *mask);
 double bvfdtd_max_courant(const bvfdtd_material *table, int32_t n_materials, double f0, double dt,
                           double dx);
 
+/*
+ * NEXT-2 of SURVEY.md 8(f): the reduction that turns the pressure maps of a tissue run and of the
+ * water-only run on the same grid into the paper's energy-loss factor.
+ *
+ * bvfdtd_plane_intensity: pulse-average intensity I_PA = rms_amp^2 / (2 rho cL) = sumsq / (count rho cL)
+ * of every cell (rho, cL = the table row of the cell's own material; rms_amp of reading P8) reduced
+ * over the cells OUTSIDE the PML mask of every z plane, on the device (fp32 per cell, fp64 sums in a
+ * fixed order).  plane_sum, plane_max: HOST arrays of nz doubles (W/m^2); planes inside the z slabs
+ * give 0.  BVFDTD_ESTATE when no step has been sampled into the rms window yet.  Synchronises the
+ * context's stream.
+ *
+ * bvfdtd_energy_loss (host only): z_m = the interior plane on which max_water is largest (first on
+ * ties), E_L = sum_tissue[z_m] / sum_water[z_m] (Eq. 2), T_S = sqrt(E_L)
+ * (PAPER.md:L164).  BVFDTD_ESTATE when the water plane carries no intensity.
+ */
+int bvfdtd_plane_intensity(bvfdtd_ctx *ctx, double *plane_sum, double *plane_max);
+int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const double *max_water,
+                       int32_t nz, int32_t pml, int32_t *z_m, double *E_L, double *T_S);
+
+/*
+ * NEXT-1 of SURVEY.md 8(f): Rayleigh-Sommerfeld field of a surface-decomposed transducer over a set of
+ * receiver points (the incident interface of the simulation domain), coupling medium water
+ * (PAPER.md:L95).  First Rayleigh integral of a baffled source, e^{+j w t} convention:
+ *     P(r) = (j rho0 c0 k / 2 pi) sum_s W_s exp(-j k |r - r_s|) / |r - r_s|,  k = 2 pi f / c0,
+ * W_s = u_s A_s the complex normal velocity times the element area (m^3/s).
+ *   src_xyz     DEVICE, n_src x 3 fp32 (m);   src_weight  DEVICE, n_src x 2 fp32 (Re, Im of W_s)
+ *   rcv_xyz     DEVICE, n_rcv x 3 fp32 (m); no receiver may coincide with a source element
+ *   p_re, p_im  DEVICE, n_rcv fp32 each (Pa)
+ *   amp, delay_s  DEVICE, n_rcv fp32 each, or both NULL: the same field as the (amplitude, delay)
+ *               pair bvfdtd_set_source takes for a CW source, p(t) = amp sin(2 pi f (t - delay)),
+ *               delay in [0, 1/f)
+ *   cuda_stream the launch is asynchronous on this stream
+ * fp32 arithmetic, one thread per receiver; no context is needed.
+ */
+int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv,
+                    const float *rcv_xyz, double f, double c0, double rho0, float *p_re, float *p_im,
+                    float *amp, float *delay_s, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -33,6 +33,7 @@ SYMBOLS = (
     "bvfdtd_read_peak_pressure", "bvfdtd_destroy", "bvfdtd_strerror", "bvfdtd_last_cuda_error",
     "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
     "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
+    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh",
 )
 
 
@@ -93,6 +94,9 @@ def lib():
         L.bvfdtd_pml_profiles.argtypes = [i32, i32, dbl, dbl, dbl, dbl, dbl, fp, fp, fp, fp]
         L.bvfdtd_pml_mask.argtypes = [C.POINTER(Grid), vp]
         L.bvfdtd_max_courant.argtypes = [C.POINTER(Material), i32, dbl, dbl, dbl]
+        L.bvfdtd_plane_intensity.argtypes = [vp, vp, vp]
+        L.bvfdtd_rayleigh.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
+        L.bvfdtd_energy_loss.argtypes = [vp, vp, vp, i32, i32, C.POINTER(i32), C.POINTER(dbl), C.POINTER(dbl)]
         L.bvfdtd_max_courant.restype = dbl
         _lib = L
     return _lib
@@ -153,6 +157,39 @@ def max_courant(table, f0, dt, dx):
 
 
 # ---- the simulation -----------------------------------------------------------------------
+
+def energy_loss(sum_tissue, sum_water, max_water, pml):
+    """(z_m, E_L, T_S) of PAPER.md Eq. 2 / L164 from the plane reductions of the two runs."""
+    a = np.ascontiguousarray(sum_tissue, dtype=np.float64)
+    b = np.ascontiguousarray(sum_water, dtype=np.float64)
+    c = np.ascontiguousarray(max_water, dtype=np.float64)
+    zm, el, ts = C.c_int32(0), C.c_double(0.0), C.c_double(0.0)
+    _check(lib().bvfdtd_energy_loss(a.ctypes.data, b.ctypes.data, c.ctypes.data, a.size, int(pml),
+                                    C.byref(zm), C.byref(el), C.byref(ts)), "bvfdtd_energy_loss")
+    return zm.value, el.value, ts.value
+
+
+def rayleigh(src_xyz, src_weight, rcv_xyz, f, c0=1500.0, rho0=1000.0, device="cuda:0", want_source=True):
+    """Rayleigh-Sommerfeld field (NEXT-1): complex64 pressure at the receivers and, if asked, the
+    (amp, delay) arrays for ``Simulation.set_source``.  Inputs are numpy arrays (n,3), (n,) complex."""
+    import torch
+    dev = torch.device(device)
+    s = torch.from_numpy(np.ascontiguousarray(src_xyz, dtype=np.float32)).to(dev)
+    wc = np.ascontiguousarray(src_weight, dtype=np.complex64)
+    w = torch.from_numpy(wc.view(np.float32).reshape(-1, 2).copy()).to(dev)
+    r = torch.from_numpy(np.ascontiguousarray(rcv_xyz, dtype=np.float32)).to(dev)
+    n_s, n_r = s.shape[0], r.shape[0]
+    out = torch.empty((4, n_r), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    _check(lib().bvfdtd_rayleigh(n_s, s.data_ptr(), w.data_ptr(), n_r, r.data_ptr(), float(f), float(c0), float(rho0),
+                                 out[0].data_ptr(), out[1].data_ptr(),
+                                 out[2].data_ptr() if want_source else None, out[3].data_ptr() if want_source else None,
+                                 stream), "bvfdtd_rayleigh")
+    torch.cuda.synchronize(dev)
+    o = out.cpu().numpy()
+    p = o[0].astype(np.complex64) + 1j * o[1].astype(np.complex64)
+    return (p, o[2], o[3]) if want_source else p
+
 
 class Simulation:
     """``bvfdtd_create`` .. ``bvfdtd_destroy`` around a torch-owned device workspace."""
@@ -281,6 +318,14 @@ class Simulation:
         _check(lib().bvfdtd_read_peak_pressure(self._h, p.data_ptr(), r.data_ptr(), 1),
                "bvfdtd_read_peak_pressure")
         return p, r
+
+    # -- NEXT-2: plane reductions of the pulse-average intensity ---------------------------
+    def plane_intensity(self):
+        """(plane_sum, plane_max) of I_PA over the interior cells of every z plane (float64, nz)."""
+        s = np.zeros(self.nz, dtype=np.float64)
+        m = np.zeros(self.nz, dtype=np.float64)
+        _check(lib().bvfdtd_plane_intensity(self._h, s.ctypes.data, m.ctypes.data), "bvfdtd_plane_intensity")
+        return s, m
 
     # -- device-time accounting (bench) ---------------------------------------------------
     def enable_kernel_timing(self, on=True):

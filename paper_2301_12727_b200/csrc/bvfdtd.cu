@@ -15,6 +15,8 @@
 #include "device_params.hpp"
 #include "kernels_ref.cuh"
 #include "kernels_tiled.cuh"
+#include "kernels_post.cuh"
+#include "kernels_rs.cuh"
 
 using namespace bvfdtd;
 
@@ -72,7 +74,7 @@ Layout make_layout(const bvfdtd_grid &g) {
 
 // Offsets (bytes) of every region of the caller's workspace.
 struct WsMap {
-    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, flagsV, flagsS, total;
+    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, flagsV, flagsS, invz, total;
 };
 
 WsMap make_wsmap(const Layout &L) {
@@ -90,6 +92,7 @@ WsMap make_wsmap(const Layout &L) {
     w.prof = take((size_t)4 * (L.nx + L.ny + L.nz) * 4);
     w.flagsV = take((size_t)L.flag_wordsV * 4);
     w.flagsS = take((size_t)L.flag_wordsS * 4);
+    w.invz = take(256 * 4);
     w.total = off;
     return w;
 }
@@ -333,6 +336,9 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     CU(cudaMemcpyAsync(c->ws + c->W.mat, mat.data(), mat.size(), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMemcpyAsync(c->ws + c->W.rows, rows.data(), 256 * sizeof(KRow), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMemcpyAsync(c->ws + c->W.prof, prof.data(), prof.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    float invz[256];
+    for (int m = 0; m < 256; ++m) invz[m] = m < n_materials ? (float)(1.0 / (table[m].rho * table[m].cL)) : 0.0f;
+    CU(cudaMemcpyAsync(c->ws + c->W.invz, invz, sizeof(invz), cudaMemcpyHostToDevice, c->stream));
     CU(cudaStreamSynchronize(c->stream));  // host staging buffers die at return
 
     Params &p = c->prm;
@@ -542,6 +548,53 @@ int bvfdtd_read_peak_pressure(bvfdtd_ctx *c, float *peak, float *rms_amp, int32_
         const int rc = deliver(c, rms_amp, target, bytes, dst_is_device);
         if (rc) return rc;
     }
+    return BVFDTD_OK;
+}
+
+int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) {
+    if (!c || !plane_sum || !plane_max) return BVFDTD_EINVAL;
+    if (c->rms_count <= 0) return BVFDTD_ESTATE;
+    const Layout &L = c->L;
+    double *d_out = (double *)(c->ws + c->W.scratch);          // 2 nz doubles of the dense scratch plane
+    k_plane_intensity<<<L.nz, 256, 0, c->stream>>>(c->prm, (const float *)(c->ws + c->W.invz), (float)(1.0 / (double)c->rms_count), d_out);
+    CU(cudaGetLastError());
+    std::vector<double> h(2 * (size_t)L.nz);
+    CU(cudaMemcpyAsync(h.data(), d_out, h.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    std::memcpy(plane_sum, h.data(), (size_t)L.nz * 8);
+    std::memcpy(plane_max, h.data() + L.nz, (size_t)L.nz * 8);
+    return BVFDTD_OK;
+}
+
+int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const double *max_water, int32_t nz, int32_t pml,
+                       int32_t *z_m, double *E_L, double *T_S) {
+    if (!sum_tissue || !sum_water || !max_water || !z_m || !E_L || !T_S || pml < 0 || nz <= 2 * pml) return BVFDTD_EINVAL;
+    int k = pml;
+    for (int q = pml; q < nz - pml; ++q)
+        if (max_water[q] > max_water[k]) k = q;
+    if (!(sum_water[k] > 0.0)) return BVFDTD_ESTATE;
+    *z_m = k;
+    *E_L = sum_tissue[k] / sum_water[k];
+    *T_S = std::sqrt(*E_L);
+    return BVFDTD_OK;
+}
+
+int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv, const float *rcv_xyz,
+                    double f, double c0, double rho0, float *p_re, float *p_im, float *amp, float *delay_s, void *cuda_stream) {
+    if (n_src <= 0 || n_rcv <= 0 || n_src > (1 << 30) || n_rcv > (1 << 30) || !src_xyz || !src_weight || !rcv_xyz || !p_re || !p_im)
+        return BVFDTD_EINVAL;
+    if (!(f > 0.0) || !(c0 > 0.0) || !(rho0 > 0.0) || (amp == nullptr) != (delay_s == nullptr)) return BVFDTD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const double w = 2.0 * 3.14159265358979323846 * f, k = w / c0;
+    // pack the sources as float4 (x, y, z, 0) on the device
+    float4 *d_src = nullptr;
+    CU(cudaMallocAsync(&d_src, (size_t)n_src * sizeof(float4), st));
+    CU(cudaMemsetAsync(d_src, 0, (size_t)n_src * sizeof(float4), st));
+    CU(cudaMemcpy2DAsync(d_src, sizeof(float4), src_xyz, 3 * sizeof(float), 3 * sizeof(float), (size_t)n_src, cudaMemcpyDeviceToDevice, st));
+    k_rayleigh<<<(unsigned)((n_rcv + 255) / 256), 256, 0, st>>>((int)n_src, d_src, (const float2 *)src_weight, (int)n_rcv, rcv_xyz, (float)k,
+                                                              (float)(rho0 * c0 * k / (2.0 * 3.14159265358979323846)), (float)w, p_re, p_im, amp, delay_s);
+    CU(cudaGetLastError());
+    CU(cudaFreeAsync(d_src, st));
     return BVFDTD_OK;
 }
 

@@ -410,6 +410,44 @@ def blocky_domain(nx, ny, nz, pml, seed, steps=20, waveform=1, f0=500e3, dx=1e-3
                     n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
 
 
+# ----------------------------------------------------------------------------------------
+# transducer surface decompositions (inputs of the Rayleigh-Sommerfeld step)
+# ----------------------------------------------------------------------------------------
+def disc_elements(radius: float, h: float, z: float = 0.0):
+    """A flat circular piston of the given radius in the plane z, cut into polar-ring elements of
+    side ~h (the paper uses areas of lambda^2/16, i.e. h = lambda/4): positions (n,3) and areas (n,).
+    The areas add up to pi radius^2 exactly."""
+    n_r = max(1, int(round(radius / h)))
+    dr = radius / n_r
+    pos, area = [], []
+    for i in range(n_r):
+        r = (i + 0.5) * dr
+        n_t = max(1, int(round(2.0 * math.pi * r / dr)))
+        t = (np.arange(n_t) + 0.5) * (2.0 * math.pi / n_t)
+        pos.append(np.stack([r * np.cos(t), r * np.sin(t), np.full(n_t, z)], axis=1))
+        area.append(np.full(n_t, math.pi * ((r + 0.5 * dr) ** 2 - (r - 0.5 * dr) ** 2) / n_t))
+    return np.concatenate(pos), np.concatenate(area)
+
+
+def bowl_elements(aperture: float, focal: float, h: float):
+    """A spherical-cap (focused bowl) radiator with its apex at the origin, axis +z and centre of
+    curvature at (0, 0, focal), cut into rings of elements of side ~h: positions and areas (the
+    areas add up to the cap area 2 pi focal^2 (1 - cos theta_max))."""
+    th_max = math.asin(0.5 * aperture / focal)
+    n_r = max(1, int(round(focal * th_max / h)))
+    dth = th_max / n_r
+    pos, area = [], []
+    for i in range(n_r):
+        th = (i + 0.5) * dth
+        ring_r = focal * math.sin(th)
+        n_t = max(1, int(round(2.0 * math.pi * ring_r / (focal * dth))))
+        t = (np.arange(n_t) + 0.5) * (2.0 * math.pi / n_t)
+        pos.append(np.stack([ring_r * np.cos(t), ring_r * np.sin(t), np.full(n_t, focal * (1.0 - math.cos(th)))], axis=1))
+        a_ring = 2.0 * math.pi * focal ** 2 * (math.cos(th - 0.5 * dth) - math.cos(th + 0.5 * dth))
+        area.append(np.full(n_t, a_ring / n_t))
+    return np.concatenate(pos), np.concatenate(area)
+
+
 def random_state(w: Workload, seed: int, scale_v: float = 1e-6, fields=None) -> dict:
     """Seeded random state for single-pass parity tests: 3 v, 6 sigma, 6 r as float32 arrays
     shaped (nz, ny, nx) (values exactly representable in fp32 so both sides start equal).

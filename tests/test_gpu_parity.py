@@ -310,6 +310,45 @@ def test_config2_tiled_vs_percell_kernels_long(bv):
 
 
 # ---------------------------------------------------------------------------------------------
+# NEXT-2: water-only companion run and the energy-loss reduction (Eq. 2)
+# ---------------------------------------------------------------------------------------------
+def test_energy_loss_reduction(bv):
+    """A bone plate in water and the water-only run on the same grid (cfg-0-like, smaller): the
+    device reduction of I_PA per plane and E_L / T_S / z_m against the oracle's definition."""
+    from oracle import post_oracle as po
+    w = wl.config0()
+    w.steps = 280
+    w.waveform = 1                      # CW so that the rms window sees the steady state
+    w.rms_begin = w.steps - 2 * w.spp
+    water = wl.config0()
+    water.steps, water.waveform, water.rms_begin = w.steps, 1, w.rms_begin
+    water.index_map = np.zeros_like(w.index_map)
+    red, ored = [], []
+    for ww in (w, water):
+        sim, o = run_both(bv, ww)
+        s, m = sim.plane_intensity()
+        os_, om = po.plane_reductions(o.get("sumsq"), o.rms_count, ww.table, ww.index_map, ww.pml)
+        inner = slice(ww.pml, ww.nz - ww.pml)
+        assert np.all(s[:ww.pml] == 0) and np.all(s[ww.nz - ww.pml:] == 0)
+        assert np.abs(s[inner] / os_[inner] - 1).max() < 2e-4
+        big = om > 0.05 * om.max()
+        assert np.abs(m[big] / om[big] - 1).max() < 1e-3
+        red.append((s, m)); ored.append((os_, om))
+        sim.close(); o.close()
+    zm, EL, TS = bv.energy_loss(red[0][0], red[1][0], red[1][1], w.pml)
+    ozm, oEL, oTS = po.energy_loss(ored[0][0], ored[1][0], ored[1][1], w.pml)
+    assert zm == ozm
+    assert abs(EL / oEL - 1) < 5e-4 and abs(TS / oTS - 1) < 5e-4
+    assert 0 < TS < 1.5
+    # no rms sample yet -> ESTATE
+    sim = bv.Simulation.from_workload(wl.random_domain(32, 32, 32, 4, seed=3))
+    with pytest.raises(bv.BvfdtdError) as e:
+        sim.plane_intensity()
+    assert e.value.code == bv.ESTATE
+    sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
 # error behaviour of the boundary
 # ---------------------------------------------------------------------------------------------
 def test_create_and_source_validation(bv):

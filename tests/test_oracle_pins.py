@@ -377,6 +377,63 @@ def test_T3_plate_transmission(alpha):
     assert abs(T_num / T_ref - 1) < 0.02
 
 
+def test_energy_loss_of_a_plate_is_its_transmission_squared():
+    """NEXT-2 oracle pin (Eq. 2, T_S = sqrt(E_L) L164): for a plane wave through an
+    absorbing plate with water on both sides, every plane behind the plate carries |T|^2 of the
+    water-only intensity, so T_S must equal the three-layer transmission coefficient (closed
+    form of T3) and z_m must lie in the water run's interior."""
+    from oracle import post_oracle as po
+    spp = 56
+    dt = 1.0 / (F0 * spp)
+    nz, P = 140, 16
+    alpha = 200.0
+    table = [WATER, (1900.0, 2800.0, 1500.0, alpha, alpha)]
+    red = []
+    for with_plate in (True, False):
+        idx = np.zeros((nz, 4, 4), np.uint8)
+        if with_plate:
+            idx[60:66] = 1
+        steps = 40 * spp
+        o, _ = homogeneous((4, 4, nz), None, (1, 1, 0), pml=P, dt=dt, table=table, idx=idx,
+                           rms_begin=steps - 3 * spp)
+        ks = P + 4
+        cells = (np.arange(4)[None, :] + 4 * (np.arange(4)[:, None] + 4 * ks)).ravel()
+        o.set_source(cells, np.ones(16), np.zeros(16), 1, F0, 3)
+        o.step(steps)
+        I = po.intensity_map(o.get("sumsq"), o.rms_count, table, idx)
+        # laterally periodic quasi-1-D run: no lateral PML, reduce over the full 4 x 4 cross-section
+        s = np.array([I[k].sum() if P <= k < nz - P else 0.0 for k in range(nz)])
+        m = np.array([I[k].max() if P <= k < nz - P else 0.0 for k in range(nz)])
+        red.append((s, m, I))
+        o.close()
+    (s_t, _, I_t), (s_w, m_w, I_w) = red
+    # closed form of a lossless plane wave: I = p_amp^2 / (2 rho c) is the same on every water plane
+    mid = I_w[70:120, 1, 1]
+    assert mid.std() / mid.mean() < 2e-2
+    # behind the plate (k >= 70) restrict z_m to the planes the wave has crossed the plate for
+    s_t2, s_w2, m_w2 = s_t.copy(), s_w.copy(), m_w.copy()
+    s_t2[:70] = s_w2[:70] = m_w2[:70] = 0.0
+    k, EL, TS = po.energy_loss(s_t2, s_w2, m_w2, P)
+    assert 70 <= k < nz - P
+    T_ref = _plate_T(1900.0, 2800.0, alpha, 6 * DX)
+    assert abs(TS / T_ref - 1) < 0.02
+    assert abs(EL - TS * TS) < 1e-12
+    # plane_reductions on a grid with lateral PML: brute force against the definition
+    rng = np.random.Generator(np.random.PCG64(5))
+    ss = rng.random((12, 11, 10))
+    im = rng.integers(0, 2, size=(12, 11, 10)).astype(np.uint8)
+    ps, pm = po.plane_reductions(ss, 7, table, im, 2)
+    for kk in range(12):
+        acc, mx = 0.0, 0.0
+        if 2 <= kk < 10:
+            for j in range(2, 9):
+                for i in range(2, 8):
+                    v = ss[kk, j, i] / (7 * table[im[kk, j, i]][0] * table[im[kk, j, i]][1])
+                    acc += v
+                    mx = max(mx, v)
+        assert abs(ps[kk] - acc) <= 1e-12 * max(acc, 1e-300) and pm[kk] == mx
+
+
 # --------------------------------------------------------------------------------------
 # T4  discrete energy in a rigid box (P = 0): constant when lossless, decaying when lossy
 # --------------------------------------------------------------------------------------
