@@ -43,7 +43,7 @@ bool grid_ok(const bvfdtd_grid *g) {
     if (g->nx < lim || g->ny < lim || g->nz < lim) return false;
     // the kernels address a field with 32-bit float offsets: keep a padded field under 2^31 floats
     if ((long long)(g->nx + 34) * (g->ny + 2) * (g->nz + 6) >= (1LL << 31)) return false;
-    return g->nx <= 65535 * 16 && g->ny <= 65535 && g->nz <= 65535;
+    return g->nx <= 65535 * 16 && g->ny <= 65533 && g->nz <= 65534;
 }
 
 Layout make_layout(const bvfdtd_grid &g) {
@@ -156,6 +156,21 @@ __global__ void k_rms_amp(float *__restrict__ dst, Params p, float two_over_coun
     if (i >= p.nx) return;
     const long long c = p.org + i + (long long)p.px * j + p.sz * k;
     dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = sqrtf(p.sumsq[c] * two_over_count);
+}
+// dense (nx, ny, nz) index map -> private layout (pitch px, py rows, nz + 1 planes) with the edges
+// replicated by one cell in +x, +y, +z (reading P2); max_index receives the largest index seen
+__global__ void k_pad_index_map(uint8_t *__restrict__ dst, const uint8_t *__restrict__ src, int nx, int ny, int nz, int px, int py,
+                                long long sz, int *max_index) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    int v = 0;
+    if (i < px) {
+        const int is = min(i, nx - 1), js = min(j, ny - 1), ks = min(k, nz - 1);
+        v = src[is + (long long)nx * (js + (long long)ny * ks)];
+        dst[i + (long long)px * j + sz * k] = (uint8_t)v;
+    }
+    v = __reduce_max_sync(0xffffffffu, v);
+    if ((threadIdx.x & 31) == 0 && v > 0) atomicMax(max_index, v);
 }
 __global__ void k_unpack_u8(uint8_t *__restrict__ dst, const uint8_t *__restrict__ src, Params p) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -294,8 +309,6 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     if (rc) return rc;
     if (max_courant(c->derived, dt, dx) > 0.494) return BVFDTD_ESTABILITY;
     const size_t cells = (size_t)grid->nx * grid->ny * grid->nz;
-    for (size_t q = 0; q < cells; ++q)
-        if (index_map[q] >= n_materials) return BVFDTD_EINVAL;
 
     c->L = make_layout(*grid);
     c->W = make_wsmap(c->L);
@@ -318,22 +331,22 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
         for (const std::vector<float> *v : {&c->pml[a].a_int, &c->pml[a].b_int, &c->pml[a].a_half, &c->pml[a].b_half})
             prof.insert(prof.end(), v->begin(), v->end());
     }
-    // index map in the private layout, edges replicated (reading P2)
-    std::vector<uint8_t> mat((size_t)L.mat_bytes);
-    for (int k = 0; k <= L.nz; ++k) {
-        const int ks = std::min(k, L.nz - 1);
-        for (int j = 0; j < L.py; ++j) {
-            const int js = std::min(j, L.ny - 1);
-            const uint8_t *src = index_map + (size_t)L.nx * (js + (size_t)L.ny * ks);
-            uint8_t *dst = mat.data() + (size_t)L.px * j + (size_t)L.sz * k;
-            std::memcpy(dst, src, L.nx);
-            std::memset(dst + L.nx, src[L.nx - 1], L.px - L.nx);
-        }
-    }
-
     // zero the whole workspace (state, sensors, psi; reading P9), then upload
     CU(cudaMemsetAsync(c->ws, 0, c->W.total, c->stream));
-    CU(cudaMemcpyAsync(c->ws + c->W.mat, mat.data(), mat.size(), cudaMemcpyHostToDevice, c->stream));
+    // index map: dense upload into the scratch plane, then validated and padded into the private
+    // layout on the device (edges replicated, reading P2)
+    CU(cudaMemcpyAsync(c->ws + c->W.scratch, index_map, cells, cudaMemcpyHostToDevice, c->stream));
+    {
+        int *d_max = (int *)(c->ws + c->W.invz);      // zeroed by the memset above; the table is uploaded after the check
+        const dim3 b(128), g((L.px + 127) / 128, L.py, L.nz + 1);
+        k_pad_index_map<<<g, b, 0, c->stream>>>((uint8_t *)(c->ws + c->W.mat), (const uint8_t *)(c->ws + c->W.scratch), L.nx, L.ny, L.nz, L.px, L.py, L.sz, d_max);
+        CU(cudaGetLastError());
+        int h_max = 0;
+        CU(cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        if (h_max >= n_materials) return BVFDTD_EINVAL;
+        CU(cudaMemsetAsync(c->ws + c->W.scratch, 0, cells, c->stream));
+    }
     CU(cudaMemcpyAsync(c->ws + c->W.rows, rows.data(), 256 * sizeof(KRow), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMemcpyAsync(c->ws + c->W.prof, prof.data(), prof.size() * 4, cudaMemcpyHostToDevice, c->stream));
     float invz[256];
