@@ -86,7 +86,6 @@ struct StagePlan {
     int wxb;               // x-psi box width in floats
     int bytes;             // stage size (multiple of 128)
     int ns;                // pipeline stages
-    int pf;                // L2 prefetch distance in planes (0 = off)
     int smem;              // dynamic shared memory of the launch
 };
 
@@ -144,30 +143,16 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
         ::"r"(smem_u32(dst)), "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int x, int y, int z, int f) {
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
-                 ::"l"(map), "r"(x), "r"(y), "r"(z), "r"(f) : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *map, int x, int y, int z) {
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
-                 ::"l"(map), "r"(x), "r"(y), "r"(z) : "memory");
-}
-// One box: either a load into the stage (counting its bytes for the barrier) or, PF = true, an L2
-// prefetch of the same box for an iteration a few planes ahead.  The prefetch moves the DRAM latency
-// out of the shared-memory pipeline: L2 (126 MB) holds the bytes in flight, the stages only have to
-// cover the L2 -> SM hop.
-template <bool PF>
+// One box load into the stage, counting its bytes for the stage barrier.
 struct Tma {
     unsigned char *st;
     uint64_t *bar;
     uint32_t bytes;
     __device__ __forceinline__ void box4(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z, int f) {
-        if (PF) tma_prefetch_4d(map, x, y, z, f);
-        else { tma_load_4d(st + off, map, bar, x, y, z, f); bytes += nbytes; }
+        tma_load_4d(st + off, map, bar, x, y, z, f); bytes += nbytes;
     }
     __device__ __forceinline__ void box3(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z) {
-        if (PF) tma_prefetch_3d(map, x, y, z);
-        else { tma_load_3d(st + off, map, bar, x, y, z); bytes += nbytes; }
+        tma_load_3d(st + off, map, bar, x, y, z); bytes += nbytes;
     }
 };
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap *m) {
@@ -366,8 +351,7 @@ enum : uint32_t {
 };
 
 // The loads of one velocity iteration m, derived from the chunk range and the flag words of planes
-// m-3..m (hist, 4 bits per plane, newest lowest).  The same routine issues the real loads and, a few
-// planes ahead, their L2 prefetches.
+// m-3..m (hist, 4 bits per plane, newest lowest).
 template <class C>
 struct VelIssue {
     const TiledMaps *maps; const Params *p; const StagePlan *sp;
@@ -385,8 +369,7 @@ struct VelIssue {
         if (in2 && z_in_slab(*p, m - 2)) c |= VC_ZS2;
         return c;
     }
-    template <bool PF>
-    __device__ __forceinline__ void run(Tma<PF> &t, int m, uint32_t hist) const {
+    __device__ __forceinline__ void run(Tma &t, int m, uint32_t hist) const {
         using VS = VStage<C>;
         const uint32_t c = ctrl(m, hist);
         const bool xy = c & VC_XY, xz = c & VC_XZ, yz = c & VC_YZ;
@@ -605,19 +588,8 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
             prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
-            uint32_t hist = 0, hist_pf = 0;       // flag words of the last planes, 4 bits each (newest in the low nibble)
-            // prefetch stream: runs sp.pf planes ahead of the load stream
-            int mp = m_begin;
-            if (sp.pf > 0) {
-                for (; mp < min(m_end, m_begin + sp.pf); ++mp) hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);   // loaded directly
-            }
+            uint32_t hist = 0;       // flag words of the last planes, 4 bits each (newest in the low nibble)
             for (int m = m_begin; m < m_end; ++m) {
-                if (sp.pf > 0 && mp < m_end) {
-                    hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
-                    Tma<true> t{nullptr, nullptr, 0};
-                    iss.run(t, mp, hist_pf);
-                    ++mp;
-                }
                 hist = (hist << 4) | (__ldg(flags + m) & 15u);
                 StageHdr h;
                 h.ctrl = iss.ctrl(m, hist);
@@ -628,7 +600,7 @@ __global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_consta
                 unsigned char *st = stages + s * sp.bytes;
                 StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
                 hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
-                Tma<false> t{st, &full[s], 0};
+                Tma t{st, &full[s], 0};
                 iss.run(t, m, hist);
                 mbar_expect_tx(&full[s], t.bytes);   // the arrival that lets the phase complete comes after the loads
                 if (++s == sp.ns) { s = 0; ph ^= 1; }
@@ -681,7 +653,7 @@ __device__ __forceinline__ void shear_update(const ShearCoef &k, float g, float 
 }
 
 // The loads of one stress iteration m (flag words of planes m, m-1, m-2 in hist, 4 bits each,
-// newest lowest); issues the real loads or, a few planes ahead, their L2 prefetches.
+// newest lowest).
 template <class C>
 struct StrIssue {
     const TiledMaps *maps; const Params *p; const StagePlan *sp;
@@ -697,8 +669,7 @@ struct StrIssue {
         return c;
     }
     // mat_off: offset of the material ring slot of plane m relative to the stage base (loads only)
-    template <bool PF>
-    __device__ __forceinline__ void run(Tma<PF> &t, int m, uint32_t hist, int mat_off) const {
+    __device__ __forceinline__ void run(Tma &t, int m, uint32_t hist, int mat_off) const {
         using SS = SStage<C>;
         const uint32_t c = ctrl(m, hist);
         const uint32_t xbox = (uint32_t)sp->wxb * C::TY * 4;
@@ -981,18 +952,8 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
             int mr = ((m_begin % MR) + MR) % MR;
-            uint32_t hist = 0, hist_pf = 0;       // flag words of planes m, m-1, m-2 ..., 4 bits each
-            int mp = m_begin;
-            if (sp.pf > 0) {
-                for (; mp < min(m_end, m_begin + sp.pf); ++mp) hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
-            }
+            uint32_t hist = 0;       // flag words of planes m, m-1, m-2 ..., 4 bits each
             for (int m = m_begin; m < m_end; ++m) {
-                if (sp.pf > 0 && mp < m_end) {
-                    hist_pf = (hist_pf << 4) | (__ldg(flags + mp) & 15u);
-                    Tma<true> t{nullptr, nullptr, 0};
-                    iss.run(t, mp, hist_pf, 0);
-                    ++mp;
-                }
                 hist = (hist << 4) | (__ldg(flags + m) & 15u);
                 StageHdr h;
                 h.ctrl = iss.ctrl(m, hist);
@@ -1003,7 +964,7 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
                 unsigned char *st = stages + s * sp.bytes;
                 StageHdr *hd = reinterpret_cast<StageHdr *>(st + sp.hdr);
                 hd->ctrl = h.ctrl; hd->az1 = h.az1; hd->bz1 = h.bz1; hd->az2 = h.az2; hd->bz2 = h.bz2;
-                Tma<false> t{st, &full[s], 0};
+                Tma t{st, &full[s], 0};
                 iss.run(t, m, hist, (int)(mat_ring + mr * C::M_BYTES - st));
                 mbar_expect_tx(&full[s], t.bytes);   // the arrival that lets the phase complete comes after the loads
                 if (++mr == MR) mr = 0;
@@ -1180,8 +1141,6 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
     s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
     s.ns = ns;
-    s.pf = 0;   // off: on B200 the TMA L2 prefetch slowed both passes (profiles/r1c notes)
-    if (const char *c = std::getenv("BVFDTD_PF")) s.pf = std::max(0, std::min(8, std::atoi(c)));
     s.smem = ns * s.bytes + extra;
     return s;
 }

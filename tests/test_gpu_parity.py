@@ -208,6 +208,17 @@ def test_tile_class_skipping(bv, dims, P, seed):
     dense.close()
 
 
+def test_full_material_table(bv):
+    """256 materials (the uint8 limit): every table row is used by some voxel, ids up to 255."""
+    w = wl.random_domain(52, 36, 40, 5, seed=61, n_mat=256, steps=40, waveform=1)
+    assert w.table.shape[0] == 256 and w.index_map.max() == 255
+    sim, o = run_both(bv, w)
+    compare_state(sim, o)
+    peak, rms = sim.read_peak_pressure()
+    compare_map(peak, o.get("peak"))
+    sim.close()
+
+
 def test_sensor_windows(bv):
     """peak window [5, 25), rms window [10, 25): nothing sampled outside them."""
     w = wl.random_domain(32, 32, 32, 4, seed=40, steps=40)
