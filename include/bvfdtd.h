@@ -71,12 +71,16 @@ enum { /* bvfdtd_opts.flags */
     BVFDTD_FLAG_REFERENCE_KERNELS = 1, /* debug: run the one-thread-per-cell kernels instead of
                                           the tiled TMA kernels (same arithmetic, same results up
                                           to fp32 rounding order) */
-    BVFDTD_FLAG_DENSE = 2              /* sweep every array everywhere: do not skip the shear
+    BVFDTD_FLAG_DENSE = 2,             /* sweep every array everywhere: do not skip the shear
                                           stresses / memory variables of tile-planes in which they
                                           are identically zero (all-fluid or lossless regions,
                                           DESIGN.md section 6).  Results are the same either way;
                                           bvfdtd_write_fields of a shear stress or a memory variable
                                           selects this mode by itself. */
+    BVFDTD_FLAG_PHASOR = 4             /* NEXT-3 of SURVEY.md 8(f): over the window [rms_begin, sensor_end) the
+                                          stress pass accumulates the single-frequency phasor of the
+                                          pressure at f0 (in-kernel DFT) INSTEAD of the running peak and the
+                                          sum of squares; read it with bvfdtd_read_phasor */
 };
 
 typedef struct {
@@ -213,6 +217,17 @@ int bvfdtd_pml_mask(const bvfdtd_grid *grid, uint8_t *mask);
 /* Largest unrelaxed Courant number c_U*dt/dx of the table (reading P6), or a negative status. */
 double bvfdtd_max_courant(const bvfdtd_material *table, int32_t n_materials, double f0, double dt,
                           double dx);
+
+/*
+ * NEXT-3 of SURVEY.md 8(f): complex pressure amplitude (for refocusing "a punctual source
+ * is placed at the intended target, back-propagated to the domain interface", which needs amplitude and
+ * phase there).  With BVFDTD_FLAG_PHASOR the sensor accumulates A = sum p cos(w t), B = sum p sin(w t),
+ * w = 2 pi f0, t = (n + 1) dt (the time level after S3 of step n), over rms_begin <= n < sensor_end.
+ * bvfdtd_read_phasor returns P = (2 / count)(A - j B), i.e. p(t) = Re{P e^{j w t}} in the steady state:
+ *   re, im   nx*ny*nz fp32 each, host or device (dst_is_device); host destinations synchronise the
+ *            stream.  BVFDTD_ESTATE without BVFDTD_FLAG_PHASOR.
+ */
+int bvfdtd_read_phasor(bvfdtd_ctx *ctx, float *re, float *im, int32_t dst_is_device);
 
 /*
  * NEXT-2 of SURVEY.md 8(f): the reduction that turns the pressure maps of a tissue run and of the

@@ -61,6 +61,8 @@ typedef struct orc {
     double *psi[18];               /* slab-compact C-PML memory, index axis*6 + term */
     double *prof[3][4];            /* per axis: a_int, b_int, a_half, b_half */
     double *peak, *sumsq;          /* dense nx*ny*nz */
+    double *phre, *phim;           /* phasor accumulators sum p cos(w t), sum p sin(w t) (NEXT-3), or NULL */
+    int phasor;                    /* 1: the rms window accumulates the phasor instead of peak / sumsq */
     int64_t peak_begin, rms_begin, sensor_end, count;
     int64_t step;
     int64_t nsrc;
@@ -198,7 +200,7 @@ void orc_free(orc *o)
     for (int q = 0; q < NFIELD; ++q) free(o->f[q]);
     for (int q = 0; q < 18; ++q) free(o->psi[q]);
     for (int a = 0; a < 3; ++a) for (int q = 0; q < 4; ++q) free(o->prof[a][q]);
-    free(o->peak); free(o->sumsq); free(o->scell); free(o->samp); free(o->sdelay);
+    free(o->peak); free(o->sumsq); free(o->phre); free(o->phim); free(o->scell); free(o->samp); free(o->sdelay);
     free(o);
 }
 
@@ -505,6 +507,26 @@ void orc_sensor(orc *o)
     int in_end = (o->sensor_end < 0) || (n < o->sensor_end);
     int do_peak = in_end && n >= o->peak_begin;
     int do_rms = in_end && n >= o->rms_begin;
+    if (o->phasor) {
+        /* NEXT-3 (refocusing needs amplitude AND phase on the domain interface): single-
+         * frequency DFT of p over the window [rms_begin, sensor_end) at f0; the state after S3 of step
+         * n is time level (n + 1) dt.  A += p cos(w t), B += p sin(w t); P = (2 / count) (A - j B), so
+         * that p(t) = Re{P e^{j w t}} in the steady state. */
+        if (!do_rms) return;
+        const double wt = 2.0 * 3.14159265358979323846 * o->f0 * (double)(n + 1) * o->dt;
+        const double cs = cos(wt), sn = sin(wt);
+#pragma omp parallel for collapse(2) schedule(static) if ((size_t)nx * ny * nz > 32768)
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t c = AT(o, i, j, k), q = DENSE(o, i, j, k);
+                    double p = -(o->f[SXX][c] + o->f[SYY][c] + o->f[SZZ][c]) / 3.0;
+                    o->phre[q] += p * cs;
+                    o->phim[q] += p * sn;
+                }
+        o->count++;
+        return;
+    }
     if (!do_peak && !do_rms) return;
 #pragma omp parallel for collapse(2) schedule(static) if ((size_t)nx * ny * nz > 32768)
     for (int k = 0; k < nz; ++k)
@@ -533,15 +555,29 @@ void orc_step(orc *o, int64_t nsteps)
 int64_t orc_step_index(const orc *o) { return o->step; }
 void orc_set_step_index(orc *o, int64_t n) { o->step = n; }
 int64_t orc_rms_count(const orc *o) { return o->count; }
+/* switch the sensor to phasor mode (before stepping); returns 0 or -1 (out of memory) */
+int orc_set_phasor(orc *o, int on)
+{
+    const size_t nc = (size_t)o->n[0] * o->n[1] * o->n[2];
+    o->phasor = on != 0;
+    if (o->phasor && !o->phre) {
+        o->phre = (double *)calloc(nc, sizeof(double));
+        o->phim = (double *)calloc(nc, sizeof(double));
+        if (!o->phre || !o->phim) return -1;
+    }
+    return 0;
+}
 
 /* ------------------------------------------------------------------------------------ */
 /* field access: dense x-fastest nx*ny*nz doubles.  field 0..14 state, 15 p = -tr/3,      */
-/* 16 peak, 17 rms_amp = sqrt(2 sumsq / count) (0 if count = 0), 18 sumsq                 */
+/* 16 peak, 17 rms_amp = sqrt(2 sumsq / count) (0 if count = 0), 18 sumsq,                */
+/* 19, 20 Re P, Im P of the phasor P = (2 / count)(A - j B) (phasor mode only)            */
 /* ------------------------------------------------------------------------------------ */
 int orc_get_field(const orc *o, int field, double *out)
 {
     const int nx = o->n[0], ny = o->n[1], nz = o->n[2];
-    if (field < 0 || field > 18) return -1;
+    if (field < 0 || field > 20) return -1;
+    if (field >= 19 && !o->phre) return -1;
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
@@ -550,7 +586,9 @@ int orc_get_field(const orc *o, int field, double *out)
                 else if (field == 15) out[q] = -(o->f[SXX][c] + o->f[SYY][c] + o->f[SZZ][c]) / 3.0;
                 else if (field == 16) out[q] = o->peak[q];
                 else if (field == 17) out[q] = o->count ? sqrt(2.0 * o->sumsq[q] / (double)o->count) : 0.0;
-                else out[q] = o->sumsq[q];
+                else if (field == 18) out[q] = o->sumsq[q];
+                else if (field == 19) out[q] = o->count ? 2.0 * o->phre[q] / (double)o->count : 0.0;
+                else out[q] = o->count ? -2.0 * o->phim[q] / (double)o->count : 0.0;
             }
     return 0;
 }

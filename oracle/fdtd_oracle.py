@@ -23,7 +23,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 FIELDS = ("vx", "vy", "vz", "sxx", "syy", "szz", "sxy", "sxz", "syz",
           "rxx", "ryy", "rzz", "rxy", "rxz", "ryz")
 FIELD_ID = {n: i for i, n in enumerate(FIELDS)}
-FIELD_ID.update(p=15, peak=16, rms_amp=17, sumsq=18)
+FIELD_ID.update(p=15, peak=16, rms_amp=17, sumsq=18, phasor_re=19, phasor_im=20)
 DERIVED = ("rho", "pi_R", "mu_R", "tau_p", "tau_s", "pi_U", "mu_U", "c_U")
 
 
@@ -57,6 +57,7 @@ def lib():
         L.orc_step_index.restype = C.c_int64
         L.orc_step_index.argtypes = [C.c_void_p]
         L.orc_set_step_index.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_set_phasor.argtypes = [C.c_void_p, C.c_int]
         L.orc_rms_count.restype = C.c_int64
         L.orc_rms_count.argtypes = [C.c_void_p]
         L.orc_get_field.argtypes = [C.c_void_p, C.c_int, dp]
@@ -173,6 +174,11 @@ class Oracle:
     @property
     def rms_count(self):
         return lib().orc_rms_count(self._h)
+
+    def set_phasor(self, on=True):
+        """NEXT-3: the rms window accumulates the single-frequency phasor at f0 instead of peak / rms."""
+        if lib().orc_set_phasor(self._h, 1 if on else 0):
+            raise MemoryError("phasor accumulators")
 
     def get(self, name):
         out = np.zeros(self.shape)

@@ -23,6 +23,7 @@ FIELD_ID = {n: i for i, n in enumerate(FIELDS)}
 FIELD_ID.update(p=15, material=16, pml_mask=17, derived=18, pml_profiles=19, sumsq=20)
 FLAG_REFERENCE_KERNELS = 1
 FLAG_DENSE = 2
+FLAG_PHASOR = 4
 
 OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 
@@ -33,7 +34,7 @@ SYMBOLS = (
     "bvfdtd_read_peak_pressure", "bvfdtd_destroy", "bvfdtd_strerror", "bvfdtd_last_cuda_error",
     "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
     "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
-    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh",
+    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_read_phasor",
 )
 
 
@@ -95,6 +96,7 @@ def lib():
         L.bvfdtd_pml_mask.argtypes = [C.POINTER(Grid), vp]
         L.bvfdtd_max_courant.argtypes = [C.POINTER(Material), i32, dbl, dbl, dbl]
         L.bvfdtd_plane_intensity.argtypes = [vp, vp, vp]
+        L.bvfdtd_read_phasor.argtypes = [vp, vp, vp, i32]
         L.bvfdtd_rayleigh.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
         L.bvfdtd_energy_loss.argtypes = [vp, vp, vp, i32, i32, C.POINTER(i32), C.POINTER(dbl), C.POINTER(dbl)]
         L.bvfdtd_max_courant.restype = dbl
@@ -318,6 +320,14 @@ class Simulation:
         _check(lib().bvfdtd_read_peak_pressure(self._h, p.data_ptr(), r.data_ptr(), 1),
                "bvfdtd_read_peak_pressure")
         return p, r
+
+    # -- NEXT-3: complex pressure amplitude -------------------------------------------------
+    def read_phasor(self):
+        """complex64 (nz, ny, nx): P with p(t) = Re{P exp(j 2 pi f0 t)} (needs FLAG_PHASOR)."""
+        re = np.empty(self.shape, dtype=np.float32)
+        im = np.empty(self.shape, dtype=np.float32)
+        _check(lib().bvfdtd_read_phasor(self._h, re.ctypes.data, im.ctypes.data, 0), "bvfdtd_read_phasor")
+        return re + 1j * im
 
     # -- NEXT-2: plane reductions of the pulse-average intensity ---------------------------
     def plane_intensity(self):

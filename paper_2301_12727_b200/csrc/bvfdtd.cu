@@ -74,7 +74,7 @@ Layout make_layout(const bvfdtd_grid &g) {
 
 // Offsets (bytes) of every region of the caller's workspace.
 struct WsMap {
-    size_t field[NSTATE], peak, sumsq, scratch, mat, psi[18], rows, prof, flagsV, flagsS, invz, total;
+    size_t field[NSTATE], peak, sumsq, phre, phim, scratch, mat, psi[18], rows, prof, flagsV, flagsS, invz, total;
 };
 
 WsMap make_wsmap(const Layout &L) {
@@ -84,6 +84,8 @@ WsMap make_wsmap(const Layout &L) {
     for (int q = 0; q < NSTATE; ++q) w.field[q] = take(L.field_floats * 4);
     w.peak = take(L.field_floats * 4);
     w.sumsq = take(L.field_floats * 4);
+    w.phre = take(L.field_floats * 4);
+    w.phim = take(L.field_floats * 4);
     w.scratch = take((size_t)L.nx * L.ny * L.nz * 4);
     w.mat = take(L.mat_bytes);
     for (int a = 0; a < 3; ++a)
@@ -134,6 +136,12 @@ __global__ void k_unpack(float *__restrict__ dst, const float *__restrict__ src,
     const int j = blockIdx.y, k = blockIdx.z;
     if (i >= p.nx) return;
     dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = src[p.org + i + (long long)p.px * j + p.sz * k];
+}
+__global__ void k_unpack_scaled(float *__restrict__ dst, const float *__restrict__ src, Params p, float scale) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = scale * src[p.org + i + (long long)p.px * j + p.sz * k];
 }
 __global__ void k_pack(float *__restrict__ dst, const float *__restrict__ src, Params p, int hold_axis) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -364,6 +372,8 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     for (int q = 0; q < NSTATE; ++q) p.f[q] = (float *)(c->ws + c->W.field[q]);
     p.peak = (float *)(c->ws + c->W.peak);
     p.sumsq = (float *)(c->ws + c->W.sumsq);
+    p.phre = (float *)(c->ws + c->W.phre);
+    p.phim = (float *)(c->ws + c->W.phim);
     p.mat = (const uint8_t *)(c->ws + c->W.mat);
     for (int q = 0; q < 18; ++q) p.psi[q] = (float *)(c->ws + c->W.psi[q]);
     p.rows = (const KRow *)(c->ws + c->W.rows);
@@ -446,6 +456,16 @@ int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
         Params p = c->prm;
         p.do_peak = in_end && step >= c->opts.peak_begin;
         p.do_rms = in_end && step >= c->opts.rms_begin;
+        p.do_phasor = 0; p.ph_cos = p.ph_sin = 0.0f;
+        if (c->opts.flags & BVFDTD_FLAG_PHASOR) {
+            // NEXT-3: the window [rms_begin, sensor_end) accumulates the phasor at f0; no peak / rms
+            p.do_phasor = p.do_rms;
+            p.do_peak = p.do_rms = 0;
+            if (p.do_phasor) {
+                const double wt = 2.0 * 3.14159265358979323846 * c->opts.f0 * (double)(step + 1) * c->dt;
+                p.ph_cos = (float)std::cos(wt); p.ph_sin = (float)std::sin(wt);
+            }
+        }
         const bool timed = c->timing && c->timed_steps < BVFDTD_MAX_TIMED_STEPS;
         cudaEvent_t *ev = nullptr;
         if (timed) {
@@ -475,7 +495,7 @@ int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
             if (rc) return cuda_fail(cudaGetLastError(), "tiled_stress");
         }
         if (timed) { CU(cudaEventRecord(ev[3], c->stream)); c->timed_steps++; }
-        if (p.do_rms) c->rms_count++;
+        if (p.do_rms || p.do_phasor) c->rms_count++;
         c->step++;
     }
     CU(cudaGetLastError());
@@ -564,9 +584,27 @@ int bvfdtd_read_peak_pressure(bvfdtd_ctx *c, float *peak, float *rms_amp, int32_
     return BVFDTD_OK;
 }
 
+int bvfdtd_read_phasor(bvfdtd_ctx *c, float *re, float *im, int32_t dst_is_device) {
+    if (!c || !re || !im) return BVFDTD_EINVAL;
+    if (!(c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
+    const Layout &L = c->L;
+    const size_t bytes = (size_t)L.nx * L.ny * L.nz * 4;
+    float *scratch = (float *)(c->ws + c->W.scratch);
+    const float sc = c->rms_count > 0 ? (float)(2.0 / (double)c->rms_count) : 0.0f;
+    for (int part = 0; part < 2; ++part) {
+        float *dst = part ? im : re;
+        float *target = dst_is_device ? dst : scratch;
+        k_unpack_scaled<<<grid3(L), 128, 0, c->stream>>>(target, part ? c->prm.phim : c->prm.phre, c->prm, part ? -sc : sc);
+        CU(cudaGetLastError());
+        const int rc = deliver(c, dst, target, bytes, dst_is_device);
+        if (rc) return rc;
+    }
+    return BVFDTD_OK;
+}
+
 int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) {
     if (!c || !plane_sum || !plane_max) return BVFDTD_EINVAL;
-    if (c->rms_count <= 0) return BVFDTD_ESTATE;
+    if (c->rms_count <= 0 || (c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
     const Layout &L = c->L;
     double *d_out = (double *)(c->ws + c->W.scratch);          // 2 nz doubles of the dense scratch plane
     k_plane_intensity<<<L.nz, 256, 0, c->stream>>>(c->prm, (const float *)(c->ws + c->W.invz), (float)(1.0 / (double)c->rms_count), d_out);

@@ -39,12 +39,15 @@ struct Params {
     long long sz, org;
     float *f[NSTATE];
     float *peak, *sumsq;
+    float *phre, *phim;    // phasor accumulators sum p cos(w t), sum p sin(w t) (NEXT-3)
     const uint8_t *mat;
     float *psi[18];        // axis*6 + term; terms 0-2 velocity pass, 3-5 stress pass
     const KRow *rows;      // 256 rows
     const float *prof[3][4];  // per axis: a_int, b_int, a_half, b_half
     float inv_dx, dt, half_dt, A, B;
     int do_peak, do_rms;
+    int do_phasor;         // this step accumulates the phasor (then do_peak = do_rms = 0)
+    float ph_cos, ph_sin;  // cos / sin of w0 (n + 1) dt for this step
     // tile-class flags: one word per (tile, plane + 2), planes -2..nz+1
     const uint32_t *flagsV, *flagsS;
 };

@@ -173,7 +173,11 @@ __global__ void __launch_bounds__(256) k_stress_ref(const Params p) {
     g = pml_term(p, s, 2, 4, 1, dplus(vy, c, sz, idx)) + pml_term(p, s, 1, 5, 1, dplus(vz, c, px, idx));
     sls(p, p.f[SYZ], p.f[RYZ], c, p.dt * (mu_h * (1.0f + ts_h)) * g, p.B * (mu_h * ts_h) * g);
 
-    if (p.do_peak | p.do_rms) {
+    if (p.do_phasor) {
+        const float pr = (p.f[SXX][c] + p.f[SYY][c] + p.f[SZZ][c]) * (-1.0f / 3.0f);
+        p.phre[c] = fmaf(p.ph_cos, pr, p.phre[c]);
+        p.phim[c] = fmaf(p.ph_sin, pr, p.phim[c]);
+    } else if (p.do_peak | p.do_rms) {
         const float pr = (p.f[SXX][c] + p.f[SYY][c] + p.f[SZZ][c]) * (-1.0f / 3.0f);
         if (p.do_peak) p.peak[c] = fmaxf(p.peak[c], fabsf(pr));
         if (p.do_rms) p.sumsq[c] = fmaf(pr, pr, p.sumsq[c]);

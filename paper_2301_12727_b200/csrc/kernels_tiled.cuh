@@ -107,7 +107,7 @@ struct TiledPlan {
     bool ready = false;
 };
 
-enum { F_PEAK = NSTATE, F_SUMSQ = NSTATE + 1 };
+enum { F_PEAK = NSTATE, F_SUMSQ = NSTATE + 1, F_PHRE = NSTATE + 2, F_PHIM = NSTATE + 3, NGRID = NSTATE + 4 };
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers: mbarrier + TMA
@@ -703,8 +703,9 @@ struct StrIssue {
 #pragma unroll
                 for (int q = 0; q < 3; ++q) t.box4(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
             }
-            if (c & SC_PEAK) t.box4(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, F_PEAK);
-            if (c & SC_RMS) t.box4(SS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 1, F_SUMSQ);
+            // phasor mode (NEXT-3) keeps its two accumulators in the peak / sumsq slots
+            if (c & SC_PEAK) t.box4(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHRE : F_PEAK);
+            if (c & SC_RMS) t.box4(SS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHIM : F_SUMSQ);
             if (c & SC_ZS1) t.box4(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 1), 5);
         }
         if (c & SC_XZ2) {
@@ -811,12 +812,16 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
                 }
                 if (ctrl & (SC_PEAK | SC_RMS)) {
                     const Q4 pr = q_muls(tr, -1.0f / 3.0f);
-                    if (ctrl & SC_PEAK) {
+                    if (p.do_phasor) {
+                        // single-frequency DFT of p: A += p cos(w t), B += p sin(w t)
+                        q_store<EDGE>(p.phre + gq, q_fmas(p.ph_cos, pr, q_ld(dbase + SS::PEAK / 4)), g.nv);
+                        q_store<EDGE>(p.phim + gq, q_fmas(p.ph_sin, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
+                    } else if (ctrl & SC_PEAK) {
                         const Q4 pk = q_ld(dbase + SS::PEAK / 4);
                         q_store<EDGE>(p.peak + gq, q_make(fmaxf(pk.a.x, fabsf(pr.a.x)), fmaxf(pk.a.y, fabsf(pr.a.y)),
                                                           fmaxf(pk.b.x, fabsf(pr.b.x)), fmaxf(pk.b.y, fabsf(pr.b.y))), g.nv);
                     }
-                    if (ctrl & SC_RMS) q_store<EDGE>(p.sumsq + gq, q_fma(pr, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
+                    if (!p.do_phasor && (ctrl & SC_RMS)) q_store<EDGE>(p.sumsq + gq, q_fma(pr, pr, q_ld(dbase + SS::SUMSQ / 4)), g.nv);
                 }
             }
             if (ctrl & (SC_XZ2 | SC_YZ2)) {
@@ -947,7 +952,7 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
             iss.maps = &maps; iss.p = &p; iss.sp = &sp;
             iss.tX = make_tilex<C>(p, x0); iss.tY = tile_in_y<C>(p, y0); iss.jy0 = tile_jy0<C>(p, y0);
             iss.x0 = x0; iss.y0 = y0; iss.kz0 = kz0; iss.kz1 = kz1;
-            iss.sens = (p.do_peak ? SC_PEAK : 0u) | (p.do_rms ? SC_RMS : 0u);
+            iss.sens = p.do_phasor ? (SC_PEAK | SC_RMS) : ((p.do_peak ? SC_PEAK : 0u) | (p.do_rms ? SC_RMS : 0u));
             prefetch_tmap(&maps.boxC); prefetch_tmap(&maps.boxD); prefetch_tmap(&maps.mat);
             if (p.P > 0) { prefetch_tmap(&maps.psx); prefetch_tmap(&maps.psy); prefetch_tmap(&maps.psz); }
             int s = 0; uint32_t ph = 0;
@@ -1085,7 +1090,7 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
     const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
     {
         void *base = (void *)(p.f[0] + (L.org - 2 * L.sz));      // cell (0,0,-2)
-        const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), 17};
+        const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), (cuuint64_t)NGRID};
         const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
         struct { CUtensorMap *m; cuuint32_t bx, by; } boxes[4] = {
             {&maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
@@ -1155,12 +1160,14 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
         return BVFDTD_ECUDA;
     }
     PFN_encodeTiled enc = (PFN_encodeTiled)fn;
-    // the 17 grid arrays (15 state + peak + sumsq) are laid out back to back at a constant stride
+    // the grid arrays (15 state, peak, sumsq, the two phasor accumulators) are laid out back to back at a constant stride
     const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
     for (int q = 0; q < NSTATE; ++q)
         if ((const char *)p.f[q] - (const char *)p.f[0] != fstride * q) return BVFDTD_EINVAL;
     if ((const char *)p.peak - (const char *)p.f[0] != fstride * F_PEAK) return BVFDTD_EINVAL;
     if ((const char *)p.sumsq - (const char *)p.f[0] != fstride * F_SUMSQ) return BVFDTD_EINVAL;
+    if ((const char *)p.phre - (const char *)p.f[0] != fstride * F_PHRE) return BVFDTD_EINVAL;
+    if ((const char *)p.phim - (const char *)p.f[0] != fstride * F_PHIM) return BVFDTD_EINVAL;
     const int wxb = L.P > 0 ? std::min(L.xph, CfgV::TX) : 4;
     if (int rc = encode_maps<CfgV>(enc, plan.mv, L, p, psi_base, psi_stride, wxb)) return rc;
 

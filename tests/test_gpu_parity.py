@@ -321,6 +321,38 @@ def test_config2_tiled_vs_percell_kernels_long(bv):
 
 
 # ---------------------------------------------------------------------------------------------
+# NEXT-3: in-kernel phasor sensor (complex pressure amplitude at f0)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("flags", [0, 1])
+def test_phasor_sensor(bv, flags):
+    """BVFDTD_FLAG_PHASOR: the stress pass accumulates the single-frequency DFT of p over the rms
+    window; compared with the oracle's phasor (pinned on CPU against the DFT of stored traces)."""
+    w = wl.blocky_domain(70, 45, 52, 6, seed=5, steps=5 * 62, waveform=1)
+    w.rms_begin = w.steps - 2 * w.spp
+    sim = bv.Simulation.from_workload(w, flags=flags | bv.FLAG_PHASOR)
+    o = orc.Oracle.from_workload(w)
+    o.set_phasor(True)
+    sim.step(w.steps)
+    o.step(w.steps)
+    P = sim.read_phasor().astype(np.complex128)
+    ref = o.get("phasor_re") + 1j * o.get("phasor_im")
+    assert np.linalg.norm(P - ref) <= 1e-4 * np.linalg.norm(ref)
+    big = np.abs(ref) > 0.1 * np.abs(ref).max()
+    assert np.abs(P[big] / ref[big] - 1).max() < 1e-3
+    compare_state(sim, o)
+    peak, rms = sim.read_peak_pressure()
+    assert not peak.any() and not rms.any()          # phasor mode replaces peak / rms
+    with pytest.raises(bv.BvfdtdError):
+        sim.plane_intensity()
+    sim.close()
+    plain = bv.Simulation.from_workload(w)
+    with pytest.raises(bv.BvfdtdError) as e:
+        plain.read_phasor()
+    assert e.value.code == bv.ESTATE
+    plain.close()
+
+
+# ---------------------------------------------------------------------------------------------
 # NEXT-2: water-only companion run and the energy-loss reduction (PAPER.md Eq. 2, L107-L110, L164)
 # ---------------------------------------------------------------------------------------------
 def test_energy_loss_reduction(bv):

@@ -377,6 +377,48 @@ def test_T3_plate_transmission(alpha):
     assert abs(T_num / T_ref - 1) < 0.02
 
 
+def test_phasor_sensor_is_the_dft_of_the_stored_trace():
+    """NEXT-3 oracle pin: the in-sweep phasor accumulators equal the single-frequency DFT of the
+    pressure traces stored step by step (numpy, outside the oracle), and in a CW steady state the
+    phasor magnitude equals the rms amplitude of a twin run."""
+    spp = 56
+    dt = 1.0 / (F0 * spp)
+    n, P = 28, 6
+    rng = np.random.Generator(np.random.PCG64(11))
+    idx = np.zeros((n, n, n), np.uint8)
+    idx[12:17, 9:20, 8:21] = 1
+    table = [WATER, BONE]
+    steps, win = 14 * spp, 3 * spp
+    src = np.array([n // 2 + n * (n // 2 + n * (P + 2))])
+    probes = np.array([14 + n * (14 + n * 20), 10 + n * (12 + n * 14), 20 + n * (8 + n * 22)])
+    runs = {}
+    for mode in ("phasor", "rms"):
+        o, _ = homogeneous((n, n, n), None, (0, 0, 0), pml=P, dt=dt, table=table, idx=idx, rms_begin=steps - win)
+        o.set_source(src, np.ones(1), np.zeros(1), 1, F0, 3)
+        if mode == "phasor":
+            o.set_phasor(True)
+        trace = np.zeros((steps, probes.size))
+        for s in range(steps):
+            o.step(1)
+            trace[s] = o.probe("p", probes)
+        runs[mode] = (o, trace)
+    o, trace = runs["phasor"]
+    assert o.rms_count == win
+    tn = (np.arange(steps - win, steps) + 1) * dt                       # time level after S3 of step n
+    dft = 2.0 / win * (trace[steps - win:] * np.exp(-2j * math.pi * F0 * tn)[:, None]).sum(axis=0)
+    re, im = o.get("phasor_re").ravel()[probes], o.get("phasor_im").ravel()[probes]
+    assert np.abs(re + 1j * im - dft).max() <= 1e-12 * np.abs(dft).max()
+    # phasor mode leaves peak and sumsq untouched
+    assert not o.get("peak").any() and not o.get("sumsq").any()
+    # steady state: p(t) = Re{P e^{jwt}} reproduces the trace, and |P| = rms amplitude
+    rec = np.real(dft[None, :] * np.exp(2j * math.pi * F0 * tn)[:, None])
+    assert np.abs(rec - trace[steps - win:]).max() < 2e-2 * np.abs(trace[steps - win:]).max()
+    o2, _ = runs["rms"]
+    amp = o2.get("rms_amp").ravel()[probes]
+    assert np.abs(np.abs(dft) / amp - 1).max() < 2e-3
+    o.close(); o2.close()
+
+
 def test_energy_loss_of_a_plate_is_its_transmission_squared():
     """NEXT-2 oracle pin (Eq. 2, T_S = sqrt(E_L) L164): for a plane wave through an
     absorbing plate with water on both sides, every plane behind the plate carries |T|^2 of the
