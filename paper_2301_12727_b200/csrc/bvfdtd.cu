@@ -642,7 +642,7 @@ int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight
     CU(cudaMallocAsync(&d_src, (size_t)n_src * sizeof(float4), st));
     CU(cudaMemsetAsync(d_src, 0, (size_t)n_src * sizeof(float4), st));
     CU(cudaMemcpy2DAsync(d_src, sizeof(float4), src_xyz, 3 * sizeof(float), 3 * sizeof(float), (size_t)n_src, cudaMemcpyDeviceToDevice, st));
-    k_rayleigh<<<(unsigned)((n_rcv + 255) / 256), 256, 0, st>>>((int)n_src, d_src, (const float2 *)src_weight, (int)n_rcv, rcv_xyz, (float)k,
+    k_rayleigh<<<(unsigned)((n_rcv + 127) / 128), 128, 0, st>>>((int)n_src, d_src, (const float2 *)src_weight, (int)n_rcv, rcv_xyz, (float)k,
                                                               (float)(rho0 * c0 * k / (2.0 * 3.14159265358979323846)), (float)w, p_re, p_im, amp, delay_s);
     CU(cudaGetLastError());
     CU(cudaFreeAsync(d_src, st));

@@ -7,8 +7,11 @@
 // Reading (the paper gives no formula): first Rayleigh integral of a baffled
 // source with normal surface velocity u_s on elements of area A_s, e^{+j w t} convention,
 //     P(r) = (j rho c k / 2 pi) sum_s u_s A_s exp(-j k R_s) / R_s,   R_s = |r - r_s|.
-// One thread per receiver; the sources stream through shared memory in tiles.  ALU/SFU bound
-// (one rsqrt and one sincos per pair), fp32; the sum is accumulated per receiver in a fixed order.
+// One thread per receiver; the sources stream through shared memory in tiles.  SFU bound: per
+// (source, receiver) pair one MUFU.RSQ and, after an explicit reduction of the phase to one turn
+// (k R / 2 pi = R / lambda, minus its nearest integer: no slow path for large arguments), one
+// MUFU.SIN and one MUFU.COS, plus ~20 FMA-class instructions; fp32; the sum is accumulated per
+// receiver in a fixed order.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -16,8 +19,12 @@ namespace bvfdtd {
 
 constexpr int RS_TILE = 1024;
 
+__device__ __forceinline__ float rs_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rs_sin(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rs_cos(float x) { float r; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 // src: n_src x (x, y, z, 0) and weight: n_src x (Re, Im) of u_s A_s;  rcv: n_rcv x (x, y, z)
-__global__ void __launch_bounds__(256) k_rayleigh(const int n_src, const float4 *__restrict__ src, const float2 *__restrict__ wgt,
+__global__ void __launch_bounds__(128) k_rayleigh(const int n_src, const float4 *__restrict__ src, const float2 *__restrict__ wgt,
                                                   const int n_rcv, const float *__restrict__ rcv, const float k, const float pref,
                                                   const float omega, float *__restrict__ p_re, float *__restrict__ p_im,
                                                   float *__restrict__ amp, float *__restrict__ delay) {
@@ -28,6 +35,7 @@ __global__ void __launch_bounds__(256) k_rayleigh(const int n_src, const float4 
     float x = 0.0f, y = 0.0f, z = 0.0f;
     if (live) { x = rcv[3 * r]; y = rcv[3 * r + 1]; z = rcv[3 * r + 2]; }
     float ar = 0.0f, ai = 0.0f;
+    const float inv_lambda = k * 0.15915494309189535f;
     for (int s0 = 0; s0 < n_src; s0 += RS_TILE) {
         const int n = min(RS_TILE, n_src - s0);
         __syncthreads();
@@ -39,9 +47,10 @@ __global__ void __launch_bounds__(256) k_rayleigh(const int n_src, const float4 
                 const float4 s = spos[q];
                 const float dx = x - s.x, dy = y - s.y, dz = z - s.z;
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                const float ir = rsqrtf(r2);
-                float sn, cs;
-                sincosf(-k * (r2 * ir), &sn, &cs);
+                const float ir = rs_rsqrt(r2);
+                const float turns = (r2 * ir) * inv_lambda;                 // k R / 2 pi
+                const float ph = -6.283185307179586f * (turns - rintf(turns));   // -k R reduced to [-pi, pi]
+                const float sn = rs_sin(ph), cs = rs_cos(ph);
                 const float2 w = sw[q];
                 ar = fmaf(fmaf(w.x, cs, -w.y * sn), ir, ar);
                 ai = fmaf(fmaf(w.x, sn, w.y * cs), ir, ai);
