@@ -364,6 +364,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
 
     Params &p = c->prm;
     p.nx = L.nx; p.ny = L.ny; p.nz = L.nz; p.P = L.P;
+    p.n_mat = n_materials;
     p.px = L.px; p.py = L.py; p.wx = L.wx; p.sz = L.sz; p.org = L.org;
     p.xp4 = L.xp4; p.xhb = L.xhb; p.xph = L.xph;
     p.ntxV = L.ntxV; p.ntyV = L.ntyV; p.ntxS = L.ntxS; p.ntyS = L.ntyS;
@@ -397,7 +398,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
             psi_base[a] = c->ws + c->W.psi[a * 6];
             psi_stride[a] = (long long)(c->W.psi[a * 6 + 1] - c->W.psi[a * 6]);
         }
-        rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride);
+        rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride, (opts->flags & BVFDTD_FLAG_DENSE) != 0);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
         c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;
         tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);

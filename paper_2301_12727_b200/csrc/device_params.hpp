@@ -33,6 +33,7 @@ struct Layout {
 
 struct Params {
     int nx, ny, nz, P;
+    int n_mat;             // rows of the material table in use
     int px, py, wx;
     int xp4, xhb, xph;     // x-slab compact index: i < P ? i : xp4 + (i - xhb)
     int ntxV, ntyV, ntxS, ntyS;

@@ -913,16 +913,17 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
 }
 
 template <class C>
-__global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
+__global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
                                                            const ZChunks zc, const StagePlan sp) {
     using SS = SStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
-    const int MR = sp.ns + 3;                                   // material ring planes
+    const int MR = sp.ns + 2;                                   // material ring: planes m-2..m in use, ns-1 in flight
+    const int NM = (p.n_mat + 31) & ~31;                        // table rows kept in shared memory
     unsigned char *mat_ring = smem + sp.ns * sp.bytes;
     float4 *tabN = reinterpret_cast<float4 *>(mat_ring + MR * C::M_BYTES);   // eP, eS, bP, bS
-    float2 *tabS = reinterpret_cast<float2 *>(tabN + 256);                   // 1/mu_R (inf = fluid), tau_s
-    float *sprof = reinterpret_cast<float *>(tabS + 256);
+    float2 *tabS = reinterpret_cast<float2 *>(tabN + NM);                   // 1/mu_R (inf = fluid), tau_s
+    float *sprof = reinterpret_cast<float *>(tabS + NM);
     uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * C::TX);
     uint64_t *empty = full + MAX_STAGES;
 
@@ -931,7 +932,7 @@ __global__ void __launch_bounds__(C::NT, 1) k_stress_tiled(const __grid_constant
     const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
     const int m_begin = kz0 - 2, m_end = kz1 + 2;
 
-    for (int q = tid; q < 256; q += C::NT) {
+    for (int q = tid; q < NM; q += C::NT) {
         const KRow r = p.rows[q];
         tabN[q] = make_float4(r.eP, r.eS, r.bP, r.bS);
         tabS[q] = make_float2(r.solid == 0.0f ? __int_as_float(0x7f800000) : r.invMu, r.tauS);
@@ -1150,7 +1151,7 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     return s;
 }
 
-inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const psi_base[3], const long long psi_stride[3]) {
+inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const psi_base[3], const long long psi_stride[3], bool dense) {
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -1188,18 +1189,29 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     const int smem_sm = 228 * 1024;
     while (plan.sv.ns > 2 && (plan.sv.smem > smem_max || 2 * (plan.sv.smem + 1024) > smem_sm))
         plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb, v_hdr);
-    // stress pass: 64 x 16 tiles with 2 stages when they fit, else 64 x 8 tiles with up to 3 stages
-    auto s_extra16 = [&](int ns) { return (ns + 3) * CfgS::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS::TX * 4 + bar_bytes; };
-    auto s_extra8 = [&](int ns) { return (ns + 3) * CfgS8::M_BYTES + 256 * 16 + 256 * 8 + 4 * CfgS8::TX * 4 + bar_bytes; };
-    plan.s16 = !(env_ty && std::atoi(env_ty) == 8);
-    if (plan.s16) {
+    // stress pass, in order of preference (measured on config 2: 0.647 / 0.673 / 0.775 ms):
+    //   64 x 8 tiles, 2 stages, TWO resident CTAs per SM (fits up to PML 16 with <= 128 materials);
+    //   64 x 16 tiles, 2 stages, one CTA with 8 consumer warps;
+    //   64 x 8 tiles, up to 3 stages, one CTA (very thick PML on a narrow grid).
+    const int nm = (p.n_mat + 31) & ~31;
+    auto s_extra16 = [&](int ns) { return (ns + 2) * CfgS::M_BYTES + nm * 24 + 4 * CfgS::TX * 4 + bar_bytes; };
+    auto s_extra8 = [&](int ns) { return (ns + 2) * CfgS8::M_BYTES + nm * 24 + 4 * CfgS8::TX * 4 + bar_bytes; };
+    const int ty_req = env_ty ? std::atoi(env_ty) : 0;
+    bool chosen = false;
+    // (the dense sweep, whose every iteration fills the whole stage, measured better on the 64 x 16 tile)
+    if (ty_req != 16 && (!ns_s || ns_s == 2) && !(dense && ty_req != 8)) {
+        plan.ss = make_stage<CfgS8>(L, SStage<CfgS8>::FIXED, 2, s_extra8(2), wxb);
+        if (2 * (plan.ss.smem + 1024) <= smem_sm) { plan.s16 = false; chosen = true; }
+    }
+    if (!chosen && ty_req != 8) {
         const int ns = ns_s ? std::max(2, std::min(MAX_STAGES, ns_s)) : 2;
         plan.ss = make_stage<CfgS>(L, SStage<CfgS>::FIXED, ns, s_extra16(ns), wxb);
         while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage<CfgS>(L, SStage<CfgS>::FIXED, plan.ss.ns - 1, s_extra16(plan.ss.ns - 1), wxb);
-        if (plan.ss.smem > smem_max) plan.s16 = false;
+        if (plan.ss.smem <= smem_max) { plan.s16 = true; chosen = true; }
     }
-    if (!plan.s16) {
+    if (!chosen) {
         const int ns = ns_s ? std::max(2, std::min(MAX_STAGES, ns_s)) : 3;
+        plan.s16 = false;
         plan.ss = make_stage<CfgS8>(L, SStage<CfgS8>::FIXED, ns, s_extra8(ns), wxb);
         while (plan.ss.smem > smem_max && plan.ss.ns > 2) plan.ss = make_stage<CfgS8>(L, SStage<CfgS8>::FIXED, plan.ss.ns - 1, s_extra8(plan.ss.ns - 1), wxb);
     }
