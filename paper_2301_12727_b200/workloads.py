@@ -465,3 +465,80 @@ def random_state(w: Workload, seed: int, scale_v: float = 1e-6, fields=None) -> 
                 a *= np.float32(scale)
             out[name] = a
     return out
+
+
+# ----------------------------------------------------------------------------------------
+# thermal step: inputs only
+# ----------------------------------------------------------------------------------------
+# PAPER.md lists no thermal tissue constants ("must be supplied by the
+# user"); these are typical literature values (chosen): k W/m/K, specific heat J/kg/K, perfusion
+# coefficient w_b rho_b C_b W/m^3/K.
+THERMAL_WATER = (0.60, 4180.0, 0.0)
+THERMAL_SOFT = (0.51, 3630.0, 4.0e4)
+THERMAL_BONE = (0.32, 1313.0, 7.0e2)
+BONE_ABSORBED_FRACTION = 0.16
+
+
+def thermal_table_for(table) -> np.ndarray:
+    """(k, rho C, w) rows for an acoustic table: solids are bone, lossy fluids soft tissue, the rest water."""
+    rows = []
+    for rho, cL, cS, aL, aS in np.asarray(table, dtype=np.float64):
+        k, c, w = THERMAL_BONE if cS > 0 else (THERMAL_SOFT if aL > 0 else THERMAL_WATER)
+        rows.append((k, rho * c, w))
+    return np.array(rows, dtype=np.float64)
+
+
+def absorbed_fraction_for(table) -> np.ndarray:
+    """Fraction of the attenuation turned into heat: 0.16 in bone, 1 elsewhere."""
+    t = np.asarray(table, dtype=np.float64)
+    return np.where(t[:, 2] > 0, BONE_ABSORBED_FRACTION, 1.0)
+
+
+def thermal_dt(table_thermal, dx: float, fraction: float = 0.4) -> float:
+    """A time step (an input): `fraction` of dx^2 min(rho C) / (6 max k), two significant digits."""
+    t = np.asarray(table_thermal, dtype=np.float64)
+    dt = fraction * dx * dx * t[:, 1].min() / (6.0 * t[:, 0].max())
+    e = 10.0 ** (math.floor(math.log10(dt)) - 1)
+    return math.floor(dt / e) * e
+
+
+def focal_heat(nx, ny, nz, dx, centre_mm, fwhm_mm=(3.0, 3.0, 12.0), q_max=2.0e6) -> np.ndarray:
+    """A Gaussian focal spot of heat deposition (W/m^3), float32 (nz, ny, nx): the shape of the
+    pressure-squared focus of an F# ~ 1 transducer at 500 kHz (about 3 x 3 x 12 mm)."""
+    ax = [np.arange(n, dtype=np.float64) * dx * 1e3 for n in (nx, ny, nz)]
+    g = [np.exp(-4.0 * math.log(2.0) * ((a - c) / f) ** 2) for a, c, f in zip(ax, centre_mm, fwhm_mm)]
+    return (q_max * g[2][:, None, None] * g[1][None, :, None] * g[0][None, None, :]).astype(np.float32)
+
+
+def thermal_domain(nx, ny, nz, seed, n_mat=5, dx=1e-3 / 3.0, T_b=37.0) -> dict:
+    """A small heterogeneous block map with random thermal rows and a focal heat source plus
+    scattered hot cells, for kernel-level parity tests of the thermal step."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 3000 + seed))
+    rows = [(THERMAL_WATER[0], 1000.0 * THERMAL_WATER[1], 0.0)]
+    for m in range(1, n_mat):
+        rows.append((0.2 + rng.random(), 2.0e6 + 2.2e6 * rng.random(), 5.0e4 * rng.random() * (m % 2)))
+    table = np.array(rows, dtype=np.float64)
+    bz, by, bx = (nz + 2) // 3, (ny + 2) // 3, (nx + 2) // 3
+    blocks = rng.integers(0, n_mat, size=(bz, by, bx), dtype=np.int64)
+    idx = np.repeat(np.repeat(np.repeat(blocks, 3, 0), 3, 1), 3, 2)[:nz, :ny, :nx]
+    idx = np.ascontiguousarray(idx).astype(np.uint8)
+    dt = thermal_dt(table, dx)
+    c_mm = [0.5 * n * dx * 1e3 for n in (nx, ny, nz)]
+    # strong enough to heat by a few kelvin within ~50 steps of this small dt
+    Q = focal_heat(nx, ny, nz, dx, c_mm, fwhm_mm=(2.0, 1.5, 3.0), q_max=0.2 * 3.0e6 / dt)
+    Q = Q + (rng.random((nz, ny, nx)) < 0.02).astype(np.float32) * np.float32(0.05 * 3.0e6 / dt)
+    return dict(nx=nx, ny=ny, nz=nz, dx=dx, dt=dt, T_b=T_b, table=table, index_map=idx, Q=Q)
+
+
+def thermal_config2() -> dict:
+    """Thermal run on config 2's domain (300 x 300 x 450, 128 materials): tissue rows by
+    `thermal_table_for`, a focal spot 60 mm beyond the source plane (the bowl's focus), 40 s on at
+    30 % duty + 20 s off in steps of dt."""
+    w = config2(steps=1)
+    table = thermal_table_for(w.table)
+    dt = thermal_dt(table, w.dx)
+    k_s = w.pml + 4
+    c_mm = [(w.nx - 1) / 2 * w.dx * 1e3, (w.ny - 1) / 2 * w.dx * 1e3, k_s * w.dx * 1e3 + 60.0]
+    Q = focal_heat(w.nx, w.ny, w.nz, w.dx, c_mm, q_max=2.0e6)
+    return dict(nx=w.nx, ny=w.ny, nz=w.nz, dx=w.dx, dt=dt, T_b=37.0, table=table, index_map=w.index_map, Q=Q,
+                duty=0.3, steps_on=int(round(40.0 / dt)), steps_off=int(round(20.0 / dt)))
