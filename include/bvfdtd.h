@@ -267,6 +267,72 @@ int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight
                     const float *rcv_xyz, double f, double c0, double rho0, float *p_re, float *p_im,
                     float *amp, float *delay_s, void *cuda_stream);
 
+/*
+ * NEXT-4 of SURVEY.md 8(f): thermal step ("solves the Bio Heat Transfer Equation (BHTE)
+ * with a finite-difference time-difference solver in Cartesian coordinates [46].  Boundary conditions
+ * are assumed conservatively with a temperature of 37 C at the domain's borders ... duration of
+ * ultrasound, time off after ultrasound, and duty cycle ... fraction of attenuation in skull bone
+ * transformed into heat was set to 0.16 ... maximal temperature, and thermal dose [48]").
+ *
+ * Readings (the paper prints neither the equation nor its discretisation):
+ *   rho C dT/dt = div(k grad T) - w (T - T_b) + s Q     (Pennes; w = w_b rho_b C_b, arterial T = T_b)
+ * forward Euler, conservative 7-point stencil on the cell grid of the acoustic run, face conductivity
+ * = series mean 2 ka kb / (ka + kb), the cells on the six borders of the box held at T_b, s = the
+ * `heat_scale` of the step (duty cycle while the ultrasound is on, 0 while it is off), and with the
+ * temperature reached at the end of each step: CEM43 += (dt/60) R^(43 - T), R = 0.5 for T >= 43 else
+ * 0.25, and the running maximum.  fp32 arithmetic; the state is kept as the rise T - T_b.
+ */
+typedef struct bvfdtd_bhte bvfdtd_bhte; /* opaque */
+
+typedef struct {
+    double k;     /* thermal conductivity, W/m/K, > 0 */
+    double rho_c; /* density x specific heat, J/m^3/K, > 0 */
+    double perf;  /* perfusion coefficient w_b rho_b C_b, W/m^3/K, >= 0 */
+} bvfdtd_thermal;
+
+enum { BVFDTD_BHTE_TRACK_MAX = 1u }; /* keep the running maximum temperature (8 more bytes per cell-step) */
+enum { BVFDTD_BHTE_T = 0, BVFDTD_BHTE_DOSE = 1, BVFDTD_BHTE_TMAX = 2, BVFDTD_BHTE_RISE = 3 };
+
+/* Bytes of device workspace a thermal context of this grid needs. */
+int bvfdtd_bhte_workspace_bytes(int32_t nx, int32_t ny, int32_t nz, uint32_t flags, size_t *out_bytes);
+/*
+ * table        HOST, n_materials rows (1..256); index_map HOST, nx*ny*nz uint8, x fastest (same map
+ *              as the acoustic run); copied during the call.
+ * T_b          border = arterial = initial temperature (deg C; 37 in the paper)
+ * d_workspace  DEVICE, caller-owned, >= bvfdtd_bhte_workspace_bytes, 256-byte aligned, must outlive
+ *              the context; cuda_stream: every launch of the context goes to this stream.
+ * Errors: EINVAL (dims < 3, a non-positive k or rho_c, negative perf, an index >= n_materials,
+ * misaligned workspace), ENOMEM (workspace too small), ESTABILITY (dt (6 k_max/dx^2 + w) / (rho C) > 1
+ * for some material: forward Euler would oscillate), ECUDA.  A failed create leaves *out = NULL.
+ */
+int bvfdtd_bhte_create(bvfdtd_bhte **out, int32_t nx, int32_t ny, int32_t nz, double dx, double dt,
+                       const bvfdtd_thermal *table, int32_t n_materials, const uint8_t *index_map,
+                       double T_b, uint32_t flags, void *d_workspace, size_t workspace_bytes,
+                       void *cuda_stream);
+/* Heat deposition Q (W/m^3), nx*ny*nz fp32 dense x-fastest, host or device; copied. */
+int bvfdtd_bhte_set_heat(bvfdtd_bhte *ctx, const float *Q, int32_t src_is_device);
+/* Initial temperature (deg C), same layout; border cells are set to T_b whatever is passed; the
+ * running maximum takes it into account. */
+int bvfdtd_bhte_set_temperature(bvfdtd_bhte *ctx, const float *T, int32_t src_is_device);
+/* Enqueue n steps with the source scaled by heat_scale (>= 0); asynchronous. */
+int bvfdtd_bhte_step(bvfdtd_bhte *ctx, int64_t n, double heat_scale);
+/* what: BVFDTD_BHTE_T temperature, _DOSE CEM43 in minutes, _TMAX running maximum (ESTATE without
+ * BVFDTD_BHTE_TRACK_MAX), _RISE T - T_b at full fp32 precision.  dst: nx*ny*nz fp32; a host
+ * destination synchronises the stream. */
+int bvfdtd_bhte_read(bvfdtd_bhte *ctx, uint32_t what, float *dst, size_t dst_bytes, int32_t dst_is_device);
+int bvfdtd_bhte_destroy(bvfdtd_bhte *ctx);
+
+/*
+ * Heat deposition from the acoustic run: with the pressure amplitude of the rms window
+ * (reading P8), I = p_amp^2 / (2 rho cL) and Q = scale * a_m * 2 alphaL_m * I per cell, a_m = the
+ * fraction of the attenuation of material m turned into heat (0.16 in bone, 1 in soft tissue), scale =
+ * the caller's intensity calibration factor.
+ *   absorbed_fraction  HOST, one double per material of the context;  Q  DEVICE, nx*ny*nz fp32 dense.
+ * BVFDTD_ESTATE when no step has been sampled into the rms window (or with BVFDTD_FLAG_PHASOR).
+ * Asynchronous on the context's stream.
+ */
+int bvfdtd_heat_source(bvfdtd_ctx *ctx, const double *absorbed_fraction, double scale, float *Q);
+
 #ifdef __cplusplus
 }
 #endif

@@ -35,7 +35,12 @@ SYMBOLS = (
     "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
     "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
     "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_read_phasor",
+    "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
+    "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
+    "bvfdtd_heat_source",
 )
+BHTE_TRACK_MAX = 1
+BHTE_WHAT = {"T": 0, "dose": 1, "tmax": 2, "rise": 3}
 
 
 class Grid(C.Structure):
@@ -45,6 +50,10 @@ class Grid(C.Structure):
 class Material(C.Structure):
     _fields_ = [("rho", C.c_double), ("cL", C.c_double), ("cS", C.c_double),
                 ("alphaL", C.c_double), ("alphaS", C.c_double)]
+
+
+class Thermal(C.Structure):
+    _fields_ = [("k", C.c_double), ("rho_c", C.c_double), ("perf", C.c_double)]
 
 
 class Opts(C.Structure):
@@ -100,6 +109,15 @@ def lib():
         L.bvfdtd_rayleigh.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
         L.bvfdtd_energy_loss.argtypes = [vp, vp, vp, i32, i32, C.POINTER(i32), C.POINTER(dbl), C.POINTER(dbl)]
         L.bvfdtd_max_courant.restype = dbl
+        L.bvfdtd_bhte_workspace_bytes.argtypes = [i32, i32, i32, u32, C.POINTER(C.c_size_t)]
+        L.bvfdtd_bhte_create.argtypes = [C.POINTER(vp), i32, i32, i32, dbl, dbl, C.POINTER(Thermal), i32, vp, dbl, u32,
+                                         vp, C.c_size_t, vp]
+        L.bvfdtd_bhte_set_heat.argtypes = [vp, vp, i32]
+        L.bvfdtd_bhte_set_temperature.argtypes = [vp, vp, i32]
+        L.bvfdtd_bhte_step.argtypes = [vp, i64, dbl]
+        L.bvfdtd_bhte_read.argtypes = [vp, u32, vp, C.c_size_t, i32]
+        L.bvfdtd_bhte_destroy.argtypes = [vp]
+        L.bvfdtd_heat_source.argtypes = [vp, vp, dbl, vp]
         _lib = L
     return _lib
 
@@ -337,6 +355,17 @@ class Simulation:
         _check(lib().bvfdtd_plane_intensity(self._h, s.ctypes.data, m.ctypes.data), "bvfdtd_plane_intensity")
         return s, m
 
+    # -- NEXT-4: heat deposition of the harmonic field ---------------------------------------
+    def heat_source(self, absorbed_fraction, scale=1.0):
+        """Q (W/m^3) as a dense float32 torch tensor (nz, ny, nx) on the device."""
+        torch = self._torch
+        a = np.ascontiguousarray(absorbed_fraction, dtype=np.float64)
+        if a.size != self.n_materials:
+            raise ValueError("one absorbed fraction per material")
+        q = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        _check(lib().bvfdtd_heat_source(self._h, a.ctypes.data, float(scale), q.data_ptr()), "bvfdtd_heat_source")
+        return q
+
     # -- device-time accounting (bench) ---------------------------------------------------
     def enable_kernel_timing(self, on=True):
         _check(lib().bvfdtd_enable_kernel_timing(self._h, 1 if on else 0),
@@ -348,3 +377,89 @@ class Simulation:
         _check(lib().bvfdtd_kernel_times(self._h, ms, n), "bvfdtd_kernel_times")
         names = ("inject", "velocity", "stress_sensor")
         return {k: {"ms": ms[i], "launches": n[i]} for i, k in enumerate(names)}
+
+
+class Bhte:
+    """``bvfdtd_bhte_create`` .. ``bvfdtd_bhte_destroy`` (NEXT-4, thermal step) around a torch-owned
+    device workspace.  ``table`` rows are (k, rho C, perfusion coefficient)."""
+
+    def __init__(self, nx, ny, nz, dx, dt, table, index_map, T_b=37.0, track_max=True, device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("bvfdtd needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.cells = self.nx * self.ny * self.nz
+        self.device = torch.device(device)
+        self.T_b = float(T_b)
+        idx = np.ascontiguousarray(index_map, dtype=np.uint8)
+        if idx.size != self.cells:
+            raise ValueError("index_map size does not match the grid")
+        t = np.ascontiguousarray(table, dtype=np.float64).reshape(-1, 3)
+        arr = (Thermal * t.shape[0])()
+        C.memmove(arr, t.ctypes.data, t.nbytes)
+        flags = BHTE_TRACK_MAX if track_max else 0
+        nbytes = C.c_size_t(0)
+        _check(lib().bvfdtd_bhte_workspace_bytes(self.nx, self.ny, self.nz, flags, C.byref(nbytes)),
+               "bvfdtd_bhte_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p(None)
+            rc = lib().bvfdtd_bhte_create(C.byref(h), self.nx, self.ny, self.nz, float(dx), float(dt), arr, t.shape[0],
+                                          idx.ctypes.data, self.T_b, flags, self.workspace.data_ptr(), nbytes.value,
+                                          self._stream.cuda_stream)
+        _check(rc, "bvfdtd_bhte_create")
+        self._h = h
+
+    def close(self):
+        h = getattr(self, "_h", None)
+        if h:
+            lib().bvfdtd_bhte_destroy(h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _src(self, a):
+        """(pointer, is_device, keep-alive) of a dense float32 field given as numpy or a torch device tensor."""
+        torch = self._torch
+        if isinstance(a, torch.Tensor):
+            t = a.to(device=self.device, dtype=torch.float32).contiguous()
+            if t.numel() != self.cells:
+                raise ValueError("field size does not match the grid")
+            return t.data_ptr(), 1, t
+        n = np.ascontiguousarray(a, dtype=np.float32)
+        if n.size != self.cells:
+            raise ValueError("field size does not match the grid")
+        return n.ctypes.data, 0, n
+
+    def set_heat(self, Q):
+        p, dev, keep = self._src(Q)
+        _check(lib().bvfdtd_bhte_set_heat(self._h, p, dev), "bvfdtd_bhte_set_heat")
+        if dev:
+            self._stream.synchronize()      # `keep` may be a temporary
+
+    def set_temperature(self, T):
+        p, dev, keep = self._src(T)
+        _check(lib().bvfdtd_bhte_set_temperature(self._h, p, dev), "bvfdtd_bhte_set_temperature")
+        if dev:
+            self._stream.synchronize()
+
+    def step(self, n, heat_scale):
+        _check(lib().bvfdtd_bhte_step(self._h, int(n), float(heat_scale)), "bvfdtd_bhte_step")
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    def read(self, what, out=None):
+        """Host float32 (nz, ny, nx): "T", "dose" (CEM43 minutes), "tmax", "rise" (T - T_b)."""
+        a = np.empty(self.shape, dtype=np.float32) if out is None else out
+        _check(lib().bvfdtd_bhte_read(self._h, BHTE_WHAT[what], a.ctypes.data, a.nbytes, 0), "bvfdtd_bhte_read")
+        return a

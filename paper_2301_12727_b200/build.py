@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbvfdtd.so")
-SOURCES = [os.path.join(CSRC, "bvfdtd.cu"), os.path.join(CSRC, "host_tables.cpp")]
+SOURCES = [os.path.join(CSRC, "bvfdtd.cu"), os.path.join(CSRC, "bhte.cu"), os.path.join(CSRC, "host_tables.cpp")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",

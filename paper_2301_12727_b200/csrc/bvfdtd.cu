@@ -13,6 +13,7 @@
 
 #include "../../include/bvfdtd.h"
 #include "device_params.hpp"
+#include "host_common.hpp"
 #include "kernels_ref.cuh"
 #include "kernels_tiled.cuh"
 #include "kernels_post.cuh"
@@ -21,19 +22,16 @@
 using namespace bvfdtd;
 
 namespace {
-
 thread_local char g_cuda_err[256] = "";
+}
 
-int cuda_fail(cudaError_t e, const char *what) {
+int bvfdtd::cuda_fail(cudaError_t e, const char *what) {
     std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
     (void)cudaGetLastError();
     return BVFDTD_ECUDA;
 }
-#define CU(call)                                              \
-    do {                                                      \
-        cudaError_t e__ = (call);                             \
-        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
-    } while (0)
+
+namespace {
 
 long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
 
@@ -109,6 +107,7 @@ struct bvfdtd_ctx {
     double dx = 0, dt = 0;
     bvfdtd_opts opts{};
     int n_materials = 0;
+    std::vector<bvfdtd_material> table;   // the caller's rows (bvfdtd_heat_source needs alphaL)
     std::vector<Derived> derived;
     PmlAxis pml[3];
     Params prm{};
@@ -324,6 +323,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     c->ws = (char *)d_workspace;
     c->stream = (cudaStream_t)cuda_stream;
     c->dx = dx; c->dt = dt; c->opts = *opts; c->opts.pml_R = R; c->n_materials = n_materials;
+    c->table.assign(table, table + n_materials);
     const Layout &L = c->L;
 
     // S0 tables
@@ -615,6 +615,28 @@ int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) 
     CU(cudaStreamSynchronize(c->stream));
     std::memcpy(plane_sum, h.data(), (size_t)L.nz * 8);
     std::memcpy(plane_max, h.data() + L.nz, (size_t)L.nz * 8);
+    return BVFDTD_OK;
+}
+
+int bvfdtd_heat_source(bvfdtd_ctx *c, const double *absorbed_fraction, double scale, float *Q) {
+    if (!c || !absorbed_fraction || !Q || !(scale >= 0.0) || !std::isfinite(scale)) return BVFDTD_EINVAL;
+    if (c->rms_count <= 0 || (c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
+    // Q = scale a 2 alphaL I,  I = p_amp^2 / (2 rho cL) = sumsq / (count rho cL): one fp32 factor per material
+    float coef[256];
+    for (int m = 0; m < 256; ++m) {
+        coef[m] = 0.0f;
+        if (m >= c->n_materials) continue;
+        if (!(absorbed_fraction[m] >= 0.0) || !std::isfinite(absorbed_fraction[m])) return BVFDTD_EINVAL;
+        const bvfdtd_material &t = c->table[m];
+        coef[m] = (float)(scale * absorbed_fraction[m] * 2.0 * t.alphaL / ((double)c->rms_count * t.rho * t.cL));
+    }
+    const Layout &L = c->L;
+    float *d_coef = (float *)(c->ws + c->W.scratch);           // 1 KB of the dense scratch plane
+    CU(cudaMemcpyAsync(d_coef, coef, sizeof(coef), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));                       // coef lives on this stack frame
+    dim3 b(128), g((L.nx + 127) / 128, L.ny, L.nz);
+    k_heat_source<<<g, b, 0, c->stream>>>(c->prm, d_coef, Q);
+    CU(cudaGetLastError());
     return BVFDTD_OK;
 }
 

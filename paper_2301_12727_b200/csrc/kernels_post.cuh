@@ -39,4 +39,13 @@ __global__ void __launch_bounds__(256) k_plane_intensity(const Params p, const f
     if (threadIdx.x == 0) { out[k] = ssum[0]; out[p.nz + k] = smax[0]; }
 }
 
+// NEXT-4: heat deposition of the harmonic field, Q = coef[material] * sumsq with
+// coef = scale a 2 alphaL / (count rho cL) folded on the host; dense x-fastest output.
+__global__ void __launch_bounds__(128) k_heat_source(const Params p, const float *__restrict__ coef, float *__restrict__ Q) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    const long long cm = i + (long long)p.px * j + p.sz * k;
+    Q[i + (long long)p.nx * (j + (long long)p.ny * k)] = __ldg(coef + p.mat[cm]) * p.sumsq[p.org + cm];
+}
+
 }  // namespace bvfdtd

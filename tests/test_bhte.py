@@ -197,10 +197,14 @@ def _run_pair(w, schedule, track_max=True, T0=None):
 
 
 def _check(sim, o, w, track_max=True):
-    T = sim.read("T").astype(np.float64)
-    rise, ref = T - w["T_b"], o.T - w["T_b"]
+    """Tolerances: the rise T - T_b is the fp32 state: relative L2 1e-5, max
+    error 2e-5 of the largest rise; the temperature itself adds half an ulp of fp32 at 37-64 C (4e-6)."""
+    ref = o.T - w["T_b"]
+    rise = sim.read("rise").astype(np.float64)
     assert np.linalg.norm(rise - ref) <= 1e-5 * np.linalg.norm(ref), np.linalg.norm(rise - ref) / np.linalg.norm(ref)
-    assert np.abs(rise - ref).max() <= 2e-5 * np.abs(ref).max() + 4e-6      # + half an ulp of fp32 at 37-60 C
+    assert np.abs(rise - ref).max() <= 2e-5 * np.abs(ref).max()
+    T = sim.read("T").astype(np.float64)
+    assert np.abs(T - o.T).max() <= 2e-5 * np.abs(ref).max() + 4e-6
     dose = sim.read("dose").astype(np.float64)
     np.testing.assert_allclose(dose, o.dose, rtol=2e-4)
     if track_max:
@@ -265,7 +269,7 @@ def test_gpu_heat_source_from_acoustic_run():
     o.step(w.steps)
     frac = np.where(w.table[:, 2] > 0, 0.16, 1.0)
     Qd = sim.heat_source(frac, scale=2.5)                      # device tensor, dense nx*ny*nz
-    Qref = bo.heat_source(o.rms_amp(), w.table, frac, w.index_map, scale=2.5)
+    Qref = bo.heat_source(o.get("rms_amp"), w.table, frac, w.index_map, scale=2.5)
     Q = Qd.cpu().numpy().reshape(Qref.shape).astype(np.float64)
     m = Qref > 0.01 * Qref.max()
     assert m.any()
