@@ -7,6 +7,9 @@ NEXT-1 Rayleigh-Sommerfeld: config 2's focused bowl (aperture 64 mm, F# 1) decom
 SFU-bound: 3 MUFU operations (rsqrt, sin, cos) per (source, receiver) pair; peak = SMs x 16 MUFU
 lanes per SM x SM clock / 3 (16 lanes per SM = 4 per scheduler is the figure assumed for sm_100).
 NEXT-2 plane intensity: one read of the sum-of-squares map and the index map of config 2 (HBM-bound).
+NEXT-4 thermal step on config 2's grid: HBM-bound, algorithmic bytes per cell-step = rise read + write,
+Q read, dose read + write, material byte (21 B) + running maximum read + write (29 B); peak = the
+measured copy bandwidth of MEASURED_PEAKS.json.
 """
 from __future__ import annotations
 
@@ -76,6 +79,35 @@ def main():
     print(json.dumps({"kernel": "k_plane_intensity", "workload": wk.name, "ms": dt * 1e3,
                       "value": bytes_ / dt / 1e9, "unit": "GB/s (sumsq + index map, wall clock incl. the 7 KB read-back)"}))
     sim.close()
+    del sim
+    torch.cuda.empty_cache()
+
+    import os
+    peaks = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+    hbm = json.load(open(peaks))["hbm_gbs"] if os.path.exists(peaks) else 6400.0
+    tw = wl.thermal_config2()
+    for track_max in (False, True):
+        th = bv.Bhte(tw["nx"], tw["ny"], tw["nz"], tw["dx"], tw["dt"], tw["table"], tw["index_map"], track_max=track_max, device=dev)
+        th.set_heat(tw["Q"])
+        th.step(5, tw["duty"])
+        torch.cuda.synchronize()
+        reps = 50
+        e0.record()
+        th.step(reps, tw["duty"])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        cells = tw["nx"] * tw["ny"] * tw["nz"]
+        b = 29.0 if track_max else 21.0
+        gbs = cells * b / (ms * 1e-3) / 1e9
+        print(json.dumps({"kernel": "k_bhte<%s>" % ("true" if track_max else "false"),
+                          "workload": "thermal step on config 2's grid (300x300x450, 128 materials), %d launches" % reps,
+                          "ms": ms, "value": cells / (ms * 1e-3) / 1e9, "unit": "Gcell-updates/s",
+                          "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+                                       "bytes_per_cell_step": b}}))
+        th.close()
+        del th
+        torch.cuda.empty_cache()
 
 
 if __name__ == "__main__":

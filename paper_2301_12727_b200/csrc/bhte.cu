@@ -6,6 +6,8 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -100,15 +102,34 @@ int bvfdtd_bhte_create(bvfdtd_bhte **out, int32_t nx, int32_t ny, int32_t nz, do
     c->flags = flags; c->dx = dx; c->dt = dt; c->T_b = T_b;
     c->ws = (char *)d_workspace; c->W = W; c->stream = (cudaStream_t)cuda_stream; c->n_mat = n_materials;
 
-    // z chunks: enough CTAs for two full waves of 3 resident CTAs per SM, chunks of at least 8 planes
-    int dev = 0, sms = 148;
+    // z chunks: the grid is (tiles) x (chunks); pick the chunk count (chunks of >= 8 planes, 3 to 8
+    // waves of the resident slots: short chunks balance better than one long wave, measured) whose
+    // CTA count fills whole waves best (a 2.1-wave grid idles a third of the kernel), fewer on ties
+    int dev = 0, sms = 148, occ = 3;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (flags & BVFDTD_BHTE_TRACK_MAX) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bhte<true>, 256, 0));
+    else CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bhte<false>, 256, 0));
+    const int slots = sms * std::max(occ, 1);
     const int tiles = ((nx + 63) / 64) * ((ny + 15) / 16);
-    int nchunk = std::max(1, (sms * 3 * 2 + tiles - 1) / tiles);
-    nchunk = std::min(nchunk, std::max(1, nz / 8));
-    c->zlen = (nz + nchunk - 1) / nchunk;
+    const int max_chunks = std::max(1, nz / 8);
+    int best = max_chunks;                                     // small grids: as many chunks as allowed
+    double best_eff = 0.0;
+    for (int n = 1; n <= max_chunks; ++n) {
+        const int zl = (nz + n - 1) / n;
+        if ((nz + zl - 1) / zl != n) continue;                 // this count is not reachable with equal chunks
+        const long long ctas = (long long)tiles * n;
+        const long long waves = (ctas + slots - 1) / slots;
+        if (waves < 3) continue;
+        if (waves > 8) break;
+        const double eff = (double)ctas / (double)(waves * slots);
+        if (eff > best_eff + 0.02) { best_eff = eff; best = n; }
+    }
+    if (const char *e = std::getenv("BVFDTD_BHTE_CHUNKS"); e && *e) best = std::max(1, std::min(max_chunks, std::atoi(e)));
+    c->zlen = (nz + best - 1) / best;
     c->nchunk = (nz + c->zlen - 1) / c->zlen;
+    if (std::getenv("BVFDTD_VERBOSE"))
+        std::fprintf(stderr, "[bvfdtd] bhte: tiles %d chunks %d (zlen %d) occ %d slots %d\n", tiles, c->nchunk, c->zlen, occ, slots);
 
     const size_t cells = (size_t)nx * ny * nz;
     CU(cudaMemsetAsync(c->ws, 0, W.total, c->stream));

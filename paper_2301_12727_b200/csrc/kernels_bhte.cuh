@@ -11,7 +11,9 @@
 // read + write) = 21 (29) B.  One CTA = a 64 x 16 column of cells marched along a z chunk: a thread
 // owns 4 consecutive x cells (float4), keeps its own column's planes k-1, k, k+1 in registers, takes
 // the x neighbours by shuffles inside its 16-lane row (edge lanes load one scalar) and the y
-// neighbours as float4 loads that hit L1/L2 (the rows belong to the warps next door).
+// neighbours as float4 loads that hit L1/L2 (the rows belong to the warps next door).  Where the
+// whole neighbourhood of a warp's cells is one material (water, brain: most of a head) every face
+// mean is k itself and the warp takes a path with no table look-ups or reciprocals per face.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -41,6 +43,7 @@ constexpr int TX = 64, TY = 16, NT = 256;
 __device__ __forceinline__ float4 ld4(const float *base, int idx) { return __ldg(reinterpret_cast<const float4 *>(base + idx)); }
 __device__ __forceinline__ uint32_t ldm(const uint8_t *base, int idx) { return __ldg(reinterpret_cast<const uint32_t *>(base + idx)); }
 __device__ __forceinline__ float rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 // series mean of two conductivities given their inverses: 2 / (1/ka + 1/kb)
 __device__ __forceinline__ float kface(float ia, float ib) { return 2.0f * rcp(ia + ib); }
 __device__ __forceinline__ float4 inv_k(const float4 *tab, uint32_t m4) {
@@ -49,7 +52,7 @@ __device__ __forceinline__ float4 inv_k(const float4 *tab, uint32_t m4) {
 }  // namespace bhte_detail
 
 template <bool TMAX>
-__global__ void __launch_bounds__(bhte_detail::NT, 3) k_bhte(const BhteParams p) {
+__global__ void __launch_bounds__(bhte_detail::NT, 4) k_bhte(const BhteParams p) {
     using namespace bhte_detail;
     __shared__ float4 tab[256];
     const int tid = threadIdx.x;
@@ -67,23 +70,16 @@ __global__ void __launch_bounds__(bhte_detail::NT, 3) k_bhte(const BhteParams p)
     // neighbours outside the box are only ever used by border cells, whose result is discarded: clamp
     const int oc = i0 + p.px * j, oym = i0 + p.px * max(j - 1, 0), oyp = i0 + p.px * min(j + 1, p.ny - 1);
     const int oxl = max(i0 - 1, 0) + p.px * j, oxr = min(i0 + 4, p.nx - 1) + p.px * j;
-    bool xin[4];
+    // bit c set: cell c of the quad is NOT held (strictly inside the box in x and y)
+    uint32_t free_xy = 0;
 #pragma unroll
-    for (int c = 0; c < 4; ++c) xin[c] = (i0 + c > 0) && (i0 + c < p.nx - 1);
+    for (int c = 0; c < 4; ++c) free_xy |= ((i0 + c > 0) && (i0 + c < p.nx - 1) && !yborder) ? (1u << c) : 0u;
 
     const int km = max(k0 - 1, 0);
     float4 th_m = ld4(p.th_in, oc + p.sz * km);
     float4 th_c = ld4(p.th_in, oc + p.sz * k0);
+    uint32_t mm = ldm(p.mat, oc + p.sz * km);
     uint32_t mc = ldm(p.mat, oc + p.sz * k0);
-    float4 ik_c = inv_k(tab, mc);
-    float gz[4];   // conductive flux (per dx) into the cell through its lower z face
-    {
-        const float4 ik_m = inv_k(tab, ldm(p.mat, oc + p.sz * km));
-        gz[0] = kface(ik_m.x, ik_c.x) * (th_m.x - th_c.x);
-        gz[1] = kface(ik_m.y, ik_c.y) * (th_m.y - th_c.y);
-        gz[2] = kface(ik_m.z, ik_c.z) * (th_m.z - th_c.z);
-        gz[3] = kface(ik_m.w, ik_c.w) * (th_m.w - th_c.w);
-    }
 
     for (int k = k0; k < k1; ++k) {
         const int kp = min(k + 1, p.nz - 1);
@@ -97,38 +93,60 @@ __global__ void __launch_bounds__(bhte_detail::NT, 3) k_bhte(const BhteParams p)
         const float4 d4 = ld4(p.dose, oc + zo);
         float4 x4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (TMAX) x4 = ld4(p.tmax, oc + zo);
-        float t_l = __shfl_up_sync(0xffffffffu, th_c.w, 1, 16), ik_l = __shfl_up_sync(0xffffffffu, ik_c.w, 1, 16);
-        float t_r = __shfl_down_sync(0xffffffffu, th_c.x, 1, 16), ik_r = __shfl_down_sync(0xffffffffu, ik_c.x, 1, 16);
-        if (l16 == 0) { t_l = __ldg(p.th_in + oxl + zo); ik_l = tab[__ldg(p.mat + oxl + zo)].x; }
-        if (l16 == 15) { t_r = __ldg(p.th_in + oxr + zo); ik_r = tab[__ldg(p.mat + oxr + zo)].x; }
-        const float4 ik_p = inv_k(tab, mp), ik_ym = inv_k(tab, m_ym), ik_yp = inv_k(tab, m_yp);
+        float t_l = __shfl_up_sync(0xffffffffu, th_c.w, 1, 16);
+        float t_r = __shfl_down_sync(0xffffffffu, th_c.x, 1, 16);
+        uint32_t m_l = __shfl_up_sync(0xffffffffu, mc, 1, 16) >> 24;
+        uint32_t m_r = __shfl_down_sync(0xffffffffu, mc, 1, 16) & 255u;
+        if (l16 == 0) { t_l = __ldg(p.th_in + oxl + zo); m_l = __ldg(p.mat + oxl + zo); }
+        if (l16 == 15) { t_r = __ldg(p.th_in + oxr + zo); m_r = __ldg(p.mat + oxr + zo); }
 
         const float T[6] = {t_l, th_c.x, th_c.y, th_c.z, th_c.w, t_r};
-        const float IK[6] = {ik_l, ik_c.x, ik_c.y, ik_c.z, ik_c.w, ik_r};
         const float Tym[4] = {t_ym.x, t_ym.y, t_ym.z, t_ym.w}, Typ[4] = {t_yp.x, t_yp.y, t_yp.z, t_yp.w};
-        const float Iym[4] = {ik_ym.x, ik_ym.y, ik_ym.z, ik_ym.w}, Iyp[4] = {ik_yp.x, ik_yp.y, ik_yp.z, ik_yp.w};
-        const float Tp[4] = {th_p.x, th_p.y, th_p.z, th_p.w}, Ip[4] = {ik_p.x, ik_p.y, ik_p.z, ik_p.w};
+        const float Tm[4] = {th_m.x, th_m.y, th_m.z, th_m.w}, Tp[4] = {th_p.x, th_p.y, th_p.z, th_p.w};
+        float s[4];    // sum over the six faces of k_f (T_neighbour - T)
+
+        // one material in the whole neighbourhood of the warp's cells: every face mean is k itself
+        const uint32_t m0 = mc & 255u, rep = m0 * 0x01010101u;
+        const bool same = (mc == rep) & (mm == rep) & (mp == rep) & (m_ym == rep) & (m_yp == rep) & (m_l == m0) & (m_r == m0);
+        if (__all_sync(0xffffffffu, same)) {
+            const float kc = rcp(tab[m0].x);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float th = T[c + 1];
+                s[c] = kc * (((T[c] - th) + (T[c + 2] - th)) + ((Tym[c] - th) + (Typ[c] - th)) + ((Tm[c] - th) + (Tp[c] - th)));
+            }
+        } else {
+            const float4 ik_c = inv_k(tab, mc), ik_m = inv_k(tab, mm), ik_p = inv_k(tab, mp);
+            const float4 ik_ym = inv_k(tab, m_ym), ik_yp = inv_k(tab, m_yp);
+            const float IK[6] = {tab[m_l].x, ik_c.x, ik_c.y, ik_c.z, ik_c.w, tab[m_r].x};
+            const float Iym[4] = {ik_ym.x, ik_ym.y, ik_ym.z, ik_ym.w}, Iyp[4] = {ik_yp.x, ik_yp.y, ik_yp.z, ik_yp.w};
+            const float Im[4] = {ik_m.x, ik_m.y, ik_m.z, ik_m.w}, Ip[4] = {ik_p.x, ik_p.y, ik_p.z, ik_p.w};
+            float gx[5];   // flux through the x faces of the quad: gx[c] = k_f (T[c] - T[c+1])
+#pragma unroll
+            for (int c = 0; c < 5; ++c) gx[c] = kface(IK[c], IK[c + 1]) * (T[c] - T[c + 1]);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float th = T[c + 1], ik = IK[c + 1];
+                float a = gx[c] - gx[c + 1];
+                a += kface(ik, Iym[c]) * (Tym[c] - th) + kface(ik, Iyp[c]) * (Typ[c] - th);
+                a += kface(ik, Im[c]) * (Tm[c] - th) + kface(ik, Ip[c]) * (Tp[c] - th);
+                s[c] = a;
+            }
+        }
+
         const float Qs[4] = {q4.x, q4.y, q4.z, q4.w};
         float dose[4] = {d4.x, d4.y, d4.z, d4.w}, tmx[4] = {x4.x, x4.y, x4.z, x4.w};
-        float gx[5];   // flux through the x faces: gx[c] = k_f (T[c] - T[c+1]) between cells c-1 and c of the quad
-#pragma unroll
-        for (int c = 0; c < 5; ++c) gx[c] = kface(IK[c], IK[c + 1]) * (T[c] - T[c + 1]);
-        const bool zborder = (k == 0) || (k == p.nz - 1);
+        const uint32_t free_c = ((k == 0) || (k == p.nz - 1)) ? 0u : free_xy;
         float out[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-            const float th = T[c + 1], ik = IK[c + 1];
-            const float gzh = kface(ik, Ip[c]) * (Tp[c] - th);            // through the upper z face
-            float s = gx[c] - gx[c + 1];
-            s += kface(ik, Iym[c]) * (Tym[c] - th) + kface(ik, Iyp[c]) * (Typ[c] - th);
-            s += gz[c] + gzh;
-            gz[c] = -gzh;
+            const float th = T[c + 1];
             const float4 row = tab[(mc >> (8 * c)) & 255u];
-            float tn = th + row.y * s - row.z * th + row.w * (p.hs * Qs[c]);
-            if (yborder || zborder || !xin[c]) tn = 0.0f;                 // Dirichlet border at T_b
+            float tn = th + row.y * s[c] - row.z * th + row.w * (p.hs * Qs[c]);
+            if (!((free_c >> c) & 1u)) tn = 0.0f;                         // Dirichlet border at T_b
             out[c] = tn;
             const float e = tn + p.d43;                                    // T - 43
-            dose[c] += p.dose_dt * exp2f(e >= 0.0f ? e : 2.0f * e);        // R^(43 - T), R = 0.5 / 0.25
+            dose[c] += p.dose_dt * ex2(e >= 0.0f ? e : 2.0f * e);          // R^(43 - T), R = 0.5 / 0.25
             if (TMAX) tmx[c] = fmaxf(tmx[c], tn);
         }
         if (store) {
@@ -136,7 +154,7 @@ __global__ void __launch_bounds__(bhte_detail::NT, 3) k_bhte(const BhteParams p)
             *reinterpret_cast<float4 *>(p.dose + oc + zo) = make_float4(dose[0], dose[1], dose[2], dose[3]);
             if (TMAX) *reinterpret_cast<float4 *>(p.tmax + oc + zo) = make_float4(tmx[0], tmx[1], tmx[2], tmx[3]);
         }
-        th_c = th_p; ik_c = ik_p; mc = mp;
+        th_m = th_c; th_c = th_p; mm = mc; mc = mp;
     }
 }
 

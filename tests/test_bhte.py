@@ -285,3 +285,58 @@ def test_gpu_heat_source_from_acoustic_run():
     rise = th.read("T").astype(np.float64) - 37.0
     assert np.linalg.norm(rise - (ob.T - 37.0)) <= 1e-5 * np.linalg.norm(ob.T - 37.0) + 1e-7 * rise.size ** 0.5
     th.close(); sim.close()
+
+
+@pytest.mark.gpu
+def test_gpu_bhte_full_size_config2_cropped_oracle():
+    """Config 2's grid (300 x 300 x 450, 128 materials) in the launch configuration the bench times.
+    The explicit stencil moves information one cell per step, so after n steps the cells of a
+    sub-box that lie at least n cells inside it depend on the sub-box only: the oracle runs on two
+    cropped sub-boxes (around the focus inside the skull cap, and across the skull) and is compared
+    there cell by cell; outside, properties that hold at any size (borders at T_b, no cooling below
+    T_b, untouched far field)."""
+    from paper_2301_12727_b200 import binding as bv
+    w = wl.thermal_config2()
+    n = 6
+    sim = bv.Bhte(w["nx"], w["ny"], w["nz"], w["dx"], w["dt"], w["table"], w["index_map"], T_b=w["T_b"], track_max=True)
+    sim.set_heat(w["Q"])
+    sim.step(n, 1.0)
+    rise = sim.read("rise").astype(np.float64)
+    dose = sim.read("dose").astype(np.float64)
+    nz, ny, nx = rise.shape
+    kf = int(np.unravel_index(np.argmax(w["Q"]), w["Q"].shape)[0])
+    for (z0, y0, x0) in ((kf - 24, ny // 2 - 24, nx // 2 - 24), (60, 100, 120), (nz - 48, ny - 48, nx - 48), (0, 0, 0)):
+        sl = (slice(z0, z0 + 48), slice(y0, y0 + 48), slice(x0, x0 + 48))
+        o = bo.BhteOracle(w["table"], w["index_map"][sl], w["dx"], w["dt"], T_b=w["T_b"])
+        o.set_heat(w["Q"][sl])
+        o.step(n, 1.0)
+        # the crop's own faces are held at T_b by the oracle: valid cells are n inside, except where
+        # a crop face is a face of the full box (there the border condition is the real one)
+        lo = [0 if a == 0 else n for a in (z0, y0, x0)]
+        hi = [48 if a + 48 == full else 48 - n for a, full in ((z0, nz), (y0, ny), (x0, nx))]
+        inner = tuple(slice(l, h) for l, h in zip(lo, hi))
+        ref = (o.T - w["T_b"])[inner]
+        got = rise[sl][inner]
+        assert np.abs(got - ref).max() <= 2e-5 * max(np.abs(ref).max(), 1e-30) + 1e-12
+        np.testing.assert_allclose(dose[sl][inner], o.dose[inner], rtol=2e-4)
+    assert rise.min() >= 0.0 and rise.max() > 0.0
+    for face in (rise[0], rise[-1], rise[:, 0], rise[:, -1], rise[:, :, 0], rise[:, :, -1]):
+        assert np.all(face == 0.0)
+    sim.close()
+
+
+@pytest.mark.gpu
+def test_gpu_bhte_uniform_regions_and_interfaces():
+    """Large single-material regions (the warp-uniform path of the kernel) separated by a slab and a
+    box of other materials (the general path), including interfaces that cut a warp's cells."""
+    w = _thermal_case(150, 40, 45, seed=8)
+    idx = np.ones((45, 40, 150), np.uint8)
+    idx[10:14] = 2
+    idx[20:30, 8:20, 30:71] = 3
+    idx[:, :, 129:] = 0
+    idx[31:, 33:, :] = 4
+    w["index_map"] = idx
+    sim, o = _run_pair(w, [(50, 0.5), (20, 0.0)])
+    _check(sim, o, w)
+    assert o.T.max() - w["T_b"] > 1.0
+    sim.close()
