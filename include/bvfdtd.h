@@ -77,10 +77,16 @@ enum { /* bvfdtd_opts.flags */
                                           DESIGN.md section 6).  Results are the same either way;
                                           bvfdtd_write_fields of a shear stress or a memory variable
                                           selects this mode by itself. */
-    BVFDTD_FLAG_PHASOR = 4             /* NEXT-3 of SURVEY.md 8(f): over the window [rms_begin, sensor_end) the
+    BVFDTD_FLAG_PHASOR = 4,            /* NEXT-3 of SURVEY.md 8(f): over the window [rms_begin, sensor_end) the
                                           stress pass accumulates the single-frequency phasor of the
                                           pressure at f0 (in-kernel DFT) INSTEAD of the running peak and the
                                           sum of squares; read it with bvfdtd_read_phasor */
+    BVFDTD_FLAG_ZLO_OPEN = 8,          /* NEXT-5 of SURVEY.md 8(f): the z = 0 face of this box is an interface
+                                          with the neighbouring z slab of a larger domain, not an outer
+                                          boundary: no absorber on that face (its C-PML profile is inert,
+                                          the mask bit is clear, sources are allowed there); the two
+                                          outermost planes are halo planes the caller refreshes */
+    BVFDTD_FLAG_ZHI_OPEN = 16          /* the same for the z = nz - 1 face */
 };
 
 typedef struct {
@@ -332,6 +338,30 @@ int bvfdtd_bhte_destroy(bvfdtd_bhte *ctx);
  * Asynchronous on the context's stream.
  */
 int bvfdtd_heat_source(bvfdtd_ctx *ctx, const double *absorbed_fraction, double scale, float *Q);
+
+/*
+ * NEXT-5 of SURVEY.md 8(e)/(f): z-slab decomposition over several GPUs (PAPER.md:L41 footnote: the
+ * large domains exceed one device).  A rank owns a contiguous range of z planes and holds them in a
+ * context whose box is that range plus two halo planes on every face that is an interface
+ * (BVFDTD_FLAG_ZLO_OPEN / _ZHI_OPEN; the 4th-order staggered differences reach two planes).  Per step:
+ *     bvfdtd_step_phase(ctx, 0)   inject (S1)
+ *     exchange the halo planes of the six stresses with the z neighbours
+ *     bvfdtd_step_phase(ctx, 1)   velocity pass (S2)
+ *     exchange the halo planes of the three velocities
+ *     bvfdtd_step_phase(ctx, 2)   stress + sensor pass (S3 + S4); the step counter advances
+ * Values the passes compute IN the halo planes are meaningless and are overwritten by the next
+ * exchange; the owned planes are bit-identical to those of the undivided run.  Phases must be called in
+ * order (BVFDTD_ESTATE otherwise; bvfdtd_step is refused in the middle of a step).
+ *
+ * bvfdtd_plane_span (host only, no context): byte offset inside the workspace, and byte count, of the
+ * contiguous block that holds planes k .. k + n_planes - 1 of state field `field_id` (0-14) in the
+ * private layout.  The block includes the layout's padding, which is identical on both sides of an
+ * interface because x and y extents are: a halo exchange is a plain copy of this block between the
+ * workspaces of two ranks (device-to-device, NCCL send/recv or a peer-to-peer put).
+ */
+int bvfdtd_step_phase(bvfdtd_ctx *ctx, int32_t phase);
+int bvfdtd_plane_span(const bvfdtd_grid *grid, uint32_t field_id, int32_t k, int32_t n_planes,
+                      size_t *offset_bytes, size_t *bytes);
 
 #ifdef __cplusplus
 }

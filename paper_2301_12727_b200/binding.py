@@ -24,6 +24,8 @@ FIELD_ID.update(p=15, material=16, pml_mask=17, derived=18, pml_profiles=19, sum
 FLAG_REFERENCE_KERNELS = 1
 FLAG_DENSE = 2
 FLAG_PHASOR = 4
+FLAG_ZLO_OPEN = 8
+FLAG_ZHI_OPEN = 16
 
 OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 
@@ -37,7 +39,7 @@ SYMBOLS = (
     "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_read_phasor",
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
-    "bvfdtd_heat_source",
+    "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
 )
 BHTE_TRACK_MAX = 1
 BHTE_WHAT = {"T": 0, "dose": 1, "tmax": 2, "rise": 3}
@@ -118,6 +120,8 @@ def lib():
         L.bvfdtd_bhte_read.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_bhte_destroy.argtypes = [vp]
         L.bvfdtd_heat_source.argtypes = [vp, vp, dbl, vp]
+        L.bvfdtd_step_phase.argtypes = [vp, i32]
+        L.bvfdtd_plane_span.argtypes = [C.POINTER(Grid), u32, i32, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         _lib = L
     return _lib
 
@@ -280,6 +284,10 @@ class Simulation:
 
     def step(self, n=1):
         _check(lib().bvfdtd_step(self._h, int(n)), "bvfdtd_step")
+
+    def step_phase(self, phase):
+        """NEXT-5: one pass of the current step (0 inject, 1 velocity, 2 stress + sensor), in order."""
+        _check(lib().bvfdtd_step_phase(self._h, int(phase)), "bvfdtd_step_phase")
 
     @property
     def step_index(self):

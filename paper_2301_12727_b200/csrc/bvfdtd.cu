@@ -112,6 +112,7 @@ struct bvfdtd_ctx {
     PmlAxis pml[3];
     Params prm{};
     int64_t step = 0;
+    int phase_done = 0;   // passes of the current step already run through bvfdtd_step_phase (bit 0 inject, 1 velocity)
     int64_t rms_count = 0;
     // source
     int64_t n_src = 0;
@@ -185,7 +186,7 @@ __global__ void k_unpack_u8(uint8_t *__restrict__ dst, const uint8_t *__restrict
     if (i >= p.nx) return;
     dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = src[i + (long long)p.px * j + p.sz * k];
 }
-__global__ void k_mask(uint8_t *__restrict__ dst, Params p) {
+__global__ void k_mask(uint8_t *__restrict__ dst, Params p, int open_lo, int open_hi) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y, k = blockIdx.z;
     if (i >= p.nx) return;
@@ -193,7 +194,7 @@ __global__ void k_mask(uint8_t *__restrict__ dst, Params p) {
     uint8_t m = 0;
     if (i < P || i >= p.nx - P) m |= 1;
     if (j < P || j >= p.ny - P) m |= 2;
-    if (k < P || k >= p.nz - P) m |= 4;
+    if ((k < P && !open_lo) || (k >= p.nz - P && !open_hi)) m |= 4;
     dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = m;
 }
 
@@ -335,7 +336,8 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     const int dims[3] = {L.nx, L.ny, L.nz};
     std::vector<float> prof;
     for (int a = 0; a < 3; ++a) {
-        pml_axis(dims[a], L.P, dx, dt, opts->f0, R, c_ref, c->pml[a]);
+        pml_axis(dims[a], L.P, dx, dt, opts->f0, R, c_ref, c->pml[a], a == 2 && (opts->flags & BVFDTD_FLAG_ZLO_OPEN),
+                 a == 2 && (opts->flags & BVFDTD_FLAG_ZHI_OPEN));
         for (const std::vector<float> *v : {&c->pml[a].a_int, &c->pml[a].b_int, &c->pml[a].a_half, &c->pml[a].b_half})
             prof.insert(prof.end(), v->begin(), v->end());
     }
@@ -426,7 +428,8 @@ int bvfdtd_set_source(bvfdtd_ctx *c, int64_t n_src, const int64_t *cell, const f
             if (s && sorted[s - 1] == q) return BVFDTD_EINVAL;
             const int i = (int)(q % L.nx), j = (int)((q / L.nx) % L.ny), k = (int)(q / ((int64_t)L.nx * L.ny));
             const int P = L.P;
-            if (i < P || i >= L.nx - P || j < P || j >= L.ny - P || k < P || k >= L.nz - P) return BVFDTD_EINVAL;
+            const bool zlo = !(c->opts.flags & BVFDTD_FLAG_ZLO_OPEN), zhi = !(c->opts.flags & BVFDTD_FLAG_ZHI_OPEN);
+            if (i < P || i >= L.nx - P || j < P || j >= L.ny - P || (zlo && k < P) || (zhi && k >= L.nz - P)) return BVFDTD_EINVAL;
             if (!std::isfinite(amp[s]) || !std::isfinite(delay_s[s])) return BVFDTD_EINVAL;
         }
     }
@@ -447,59 +450,98 @@ int bvfdtd_set_source(bvfdtd_ctx *c, int64_t n_src, const int64_t *cell, const f
     return BVFDTD_OK;
 }
 
-int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
-    if (!c || n < 0) return BVFDTD_EINVAL;
+namespace {
+
+enum { PH_INJECT = 1, PH_VELOCITY = 2, PH_STRESS = 4, PH_ALL = 7 };
+
+// The passes of step c->step selected by `phases`; the step counter advances with the stress pass.
+int run_phases(bvfdtd_ctx *c, int phases) {
     const Layout &L = c->L;
     const bool ref = (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) != 0;
-    for (int64_t s = 0; s < n; ++s) {
-        const int64_t step = c->step;
-        const bool in_end = c->opts.sensor_end < 0 || step < c->opts.sensor_end;
-        Params p = c->prm;
-        p.do_peak = in_end && step >= c->opts.peak_begin;
-        p.do_rms = in_end && step >= c->opts.rms_begin;
-        p.do_phasor = 0; p.ph_cos = p.ph_sin = 0.0f;
-        if (c->opts.flags & BVFDTD_FLAG_PHASOR) {
-            // NEXT-3: the window [rms_begin, sensor_end) accumulates the phasor at f0; no peak / rms
-            p.do_phasor = p.do_rms;
-            p.do_peak = p.do_rms = 0;
-            if (p.do_phasor) {
-                const double wt = 2.0 * 3.14159265358979323846 * c->opts.f0 * (double)(step + 1) * c->dt;
-                p.ph_cos = (float)std::cos(wt); p.ph_sin = (float)std::sin(wt);
-            }
+    const int64_t step = c->step;
+    const bool in_end = c->opts.sensor_end < 0 || step < c->opts.sensor_end;
+    Params p = c->prm;
+    p.do_peak = in_end && step >= c->opts.peak_begin;
+    p.do_rms = in_end && step >= c->opts.rms_begin;
+    p.do_phasor = 0; p.ph_cos = p.ph_sin = 0.0f;
+    if (c->opts.flags & BVFDTD_FLAG_PHASOR) {
+        // NEXT-3: the window [rms_begin, sensor_end) accumulates the phasor at f0; no peak / rms
+        p.do_phasor = p.do_rms;
+        p.do_peak = p.do_rms = 0;
+        if (p.do_phasor) {
+            const double wt = 2.0 * 3.14159265358979323846 * c->opts.f0 * (double)(step + 1) * c->dt;
+            p.ph_cos = (float)std::cos(wt); p.ph_sin = (float)std::sin(wt);
         }
-        const bool timed = c->timing && c->timed_steps < BVFDTD_MAX_TIMED_STEPS;
-        cudaEvent_t *ev = nullptr;
-        if (timed) {
-            if (c->ev.size() < (size_t)(c->timed_steps + 1) * 4) {
-                for (int q = 0; q < 4; ++q) { cudaEvent_t e; CU(cudaEventCreate(&e)); c->ev.push_back(e); }
-            }
-            ev = &c->ev[c->timed_steps * 4];
-            CU(cudaEventRecord(ev[0], c->stream));
+    }
+    const bool timed = phases == PH_ALL && c->timing && c->timed_steps < BVFDTD_MAX_TIMED_STEPS;
+    cudaEvent_t *ev = nullptr;
+    if (timed) {
+        if (c->ev.size() < (size_t)(c->timed_steps + 1) * 4) {
+            for (int q = 0; q < 4; ++q) { cudaEvent_t e; CU(cudaEventCreate(&e)); c->ev.push_back(e); }
         }
-        if (c->n_src > 0) {
-            const int tb = 128;
-            k_inject<<<(unsigned)((c->n_src + tb - 1) / tb), tb, 0, c->stream>>>(
-                p, c->n_src, c->d_cell, c->d_amp, c->d_delay, c->waveform, c->f_src, c->n_cycles,
-                (double)step * c->dt);
-        }
-        if (timed) CU(cudaEventRecord(ev[1], c->stream));
-        if (ref) {
-            const dim3 b(32, 4, 2), g((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
-            k_velocity_ref<<<g, b, 0, c->stream>>>(p);
-            if (timed) CU(cudaEventRecord(ev[2], c->stream));
-            k_stress_ref<<<g, b, 0, c->stream>>>(p);
-        } else {
-            int rc = tiled_velocity(c->plan, p, c->stream);
-            if (rc) return cuda_fail(cudaGetLastError(), "tiled_velocity");
-            if (timed) CU(cudaEventRecord(ev[2], c->stream));
-            rc = tiled_stress(c->plan, p, c->stream);
-            if (rc) return cuda_fail(cudaGetLastError(), "tiled_stress");
-        }
-        if (timed) { CU(cudaEventRecord(ev[3], c->stream)); c->timed_steps++; }
+        ev = &c->ev[c->timed_steps * 4];
+        CU(cudaEventRecord(ev[0], c->stream));
+    }
+    if ((phases & PH_INJECT) && c->n_src > 0) {
+        const int tb = 128;
+        k_inject<<<(unsigned)((c->n_src + tb - 1) / tb), tb, 0, c->stream>>>(
+            p, c->n_src, c->d_cell, c->d_amp, c->d_delay, c->waveform, c->f_src, c->n_cycles,
+            (double)step * c->dt);
+    }
+    if (timed) CU(cudaEventRecord(ev[1], c->stream));
+    const dim3 rb(32, 4, 2), rg((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
+    if (phases & PH_VELOCITY) {
+        if (ref) k_velocity_ref<<<rg, rb, 0, c->stream>>>(p);
+        else if (tiled_velocity(c->plan, p, c->stream)) return cuda_fail(cudaGetLastError(), "tiled_velocity");
+    }
+    if (timed) CU(cudaEventRecord(ev[2], c->stream));
+    if (phases & PH_STRESS) {
+        if (ref) k_stress_ref<<<rg, rb, 0, c->stream>>>(p);
+        else if (tiled_stress(c->plan, p, c->stream)) return cuda_fail(cudaGetLastError(), "tiled_stress");
+    }
+    if (timed) { CU(cudaEventRecord(ev[3], c->stream)); c->timed_steps++; }
+    if (phases & PH_STRESS) {
         if (p.do_rms || p.do_phasor) c->rms_count++;
         c->step++;
+        c->phase_done = 0;
+    } else {
+        c->phase_done |= phases;
+    }
+    return BVFDTD_OK;
+}
+
+}  // namespace
+
+int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
+    if (!c || n < 0) return BVFDTD_EINVAL;
+    if (c->phase_done != 0) return BVFDTD_ESTATE;   // a step begun with bvfdtd_step_phase must be finished first
+    for (int64_t s = 0; s < n; ++s) {
+        int rc = run_phases(c, PH_ALL);
+        if (rc) return rc;
     }
     CU(cudaGetLastError());
+    return BVFDTD_OK;
+}
+
+int bvfdtd_step_phase(bvfdtd_ctx *c, int32_t phase) {
+    if (!c || phase < 0 || phase > 2) return BVFDTD_EINVAL;
+    // the passes of one step run in order: inject (0), velocity (1), stress + sensor (2)
+    const int bit = 1 << phase;
+    const int before = bit - 1;                       // every earlier pass must have run, this one not
+    if ((c->phase_done & before) != before || (c->phase_done & bit)) return BVFDTD_ESTATE;
+    int rc = run_phases(c, bit);
+    if (rc) return rc;
+    CU(cudaGetLastError());
+    return BVFDTD_OK;
+}
+
+int bvfdtd_plane_span(const bvfdtd_grid *grid, uint32_t field_id, int32_t k, int32_t n_planes, size_t *offset_bytes, size_t *bytes) {
+    if (!grid_ok(grid) || field_id >= NSTATE || !offset_bytes || !bytes || k < 0 || n_planes < 1 || k + n_planes > grid->nz)
+        return BVFDTD_EINVAL;
+    const Layout L = make_layout(*grid);
+    const WsMap W = make_wsmap(L);
+    *offset_bytes = W.field[field_id] + (size_t)(L.org + L.sz * k) * 4;
+    *bytes = (size_t)L.sz * n_planes * 4;
     return BVFDTD_OK;
 }
 
@@ -535,7 +577,7 @@ int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, 
     else if (id == BVFDTD_F_SUMSQ) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.sumsq, c->prm);
     else if (id == BVFDTD_F_PRESSURE) k_pressure<<<g, b, 0, c->stream>>>((float *)target, c->prm);
     else if (id == BVFDTD_F_MATERIAL) k_unpack_u8<<<g, b, 0, c->stream>>>((uint8_t *)target, c->prm.mat, c->prm);
-    else k_mask<<<g, b, 0, c->stream>>>((uint8_t *)target, c->prm);
+    else k_mask<<<g, b, 0, c->stream>>>((uint8_t *)target, c->prm, (c->opts.flags & BVFDTD_FLAG_ZLO_OPEN) != 0, (c->opts.flags & BVFDTD_FLAG_ZHI_OPEN) != 0);
     CU(cudaGetLastError());
     return deliver(c, dst, target, need, dst_is_device);
 }

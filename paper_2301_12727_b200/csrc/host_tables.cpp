@@ -76,7 +76,7 @@ void kernel_rows(const std::vector<Derived> &d, double dt, double f0, std::vecto
 
 // C-PML, kappa = 1 (reading P5).  Node i sits at i dx (integer) or (i + 1/2) dx (half); the
 // layer/interior interfaces are at (P - 1/2) dx and (n - P - 1/2) dx; xi = depth into the layer.
-void pml_axis(int n, int pml, double dx, double dt, double f0, double R, double c_ref, PmlAxis &p) {
+void pml_axis(int n, int pml, double dx, double dt, double f0, double R, double c_ref, PmlAxis &p, bool open_lo, bool open_hi) {
     p.a_int.assign(n, 0.0f);
     p.b_int.assign(n, 1.0f);
     p.a_half.assign(n, 0.0f);
@@ -89,8 +89,8 @@ void pml_axis(int n, int pml, double dx, double dt, double f0, double R, double 
         for (int half = 0; half < 2; ++half) {
             const double x = (i + (half ? 0.5 : 0.0)) * dx;
             double xi = 0.0;
-            if (lo_face - x > xi) xi = lo_face - x;
-            if (x - hi_face > xi) xi = x - hi_face;
+            if (!open_lo && lo_face - x > xi) xi = lo_face - x;   // an open face is a slab interface (NEXT-5):
+            if (!open_hi && x - hi_face > xi) xi = x - hi_face;   // no absorber there, the profile stays inert
             const double s = xi / L;
             const double d = d0 * s * s;
             const double al = kPi * f0 * (1.0 - s);

@@ -35,7 +35,8 @@ struct PmlAxis {
 // returns BVFDTD_OK or BVFDTD_EINVAL
 int derive_materials(const bvfdtd_material *table, int n, double f0, std::vector<Derived> &out);
 void kernel_rows(const std::vector<Derived> &d, double dt, double f0, std::vector<KRow> &rows);
-void pml_axis(int n, int pml, double dx, double dt, double f0, double R, double c_ref, PmlAxis &p);
+void pml_axis(int n, int pml, double dx, double dt, double f0, double R, double c_ref, PmlAxis &p, bool open_lo = false,
+              bool open_hi = false);
 double max_courant(const std::vector<Derived> &d, double dt, double dx);
 
 }  // namespace bvfdtd
