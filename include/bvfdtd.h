@@ -363,6 +363,28 @@ int bvfdtd_step_phase(bvfdtd_ctx *ctx, int32_t phase);
 int bvfdtd_plane_span(const bvfdtd_grid *grid, uint32_t field_id, int32_t k, int32_t n_planes,
                       size_t *offset_bytes, size_t *bytes);
 
+/*
+ * NEXT-3, second half ("a punctual source is placed at the intended target,
+ * back-propagated to the domain interface, and then propagated back with Rayleigh-Sommerfeld to the
+ * transducer elements to calculate the corrected phase programming of the transducer elements").
+ * The chain is: a run with BVFDTD_FLAG_PHASOR from a one-cell source at the target; the phasors of the
+ * entry plane as the weights of bvfdtd_rayleigh towards the surface points of the array (the plane
+ * radiates back as a baffled source with weight proportional to P); then this call:
+ *   E_m = sum of the field over the surface points of element m,
+ *   time reversal: element m emits Re{conj(E_m)/|E_m| e^{j w t}} = cos(w (t - tau_m)), tau_m = arg(E_m)/w
+ *   taken in [0, 1/f); every surface point q of element m gets the weight u0 area_q conj(E_m)/|E_m|,
+ * which is the src_weight of the forward bvfdtd_rayleigh call.
+ *   p_re, p_im  DEVICE, n_pts fp32 each: the field at the surface points
+ *   element     DEVICE, n_pts int32 in [0, n_elem) (EINVAL otherwise); area  DEVICE, n_pts fp32 (m^2)
+ *   w_pts       DEVICE, n_pts x 2 fp32 (Re, Im);  delay_s  DEVICE, n_elem fp32
+ *   E           DEVICE, n_elem x 2 fp32, or NULL
+ * An element that received no field keeps weight u0 area and delay 0.  Synchronises the stream once
+ * (index validation).  fp64 sums in a fixed order.
+ */
+int bvfdtd_refocus_weights(int64_t n_pts, const float *p_re, const float *p_im, const int32_t *element,
+                           const float *area, int32_t n_elem, double f, double u0, float *w_pts,
+                           float *delay_s, float *E, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

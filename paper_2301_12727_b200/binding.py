@@ -40,6 +40,7 @@ SYMBOLS = (
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
+    "bvfdtd_refocus_weights",
 )
 BHTE_TRACK_MAX = 1
 BHTE_WHAT = {"T": 0, "dose": 1, "tmax": 2, "rise": 3}
@@ -121,6 +122,7 @@ def lib():
         L.bvfdtd_bhte_destroy.argtypes = [vp]
         L.bvfdtd_heat_source.argtypes = [vp, vp, dbl, vp]
         L.bvfdtd_step_phase.argtypes = [vp, i32]
+        L.bvfdtd_refocus_weights.argtypes = [i64, vp, vp, vp, vp, i32, dbl, dbl, vp, vp, vp, vp]
         L.bvfdtd_plane_span.argtypes = [C.POINTER(Grid), u32, i32, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         _lib = L
     return _lib
@@ -354,6 +356,14 @@ class Simulation:
         im = np.empty(self.shape, dtype=np.float32)
         _check(lib().bvfdtd_read_phasor(self._h, re.ctypes.data, im.ctypes.data, 0), "bvfdtd_read_phasor")
         return re + 1j * im
+
+    def read_phasor_device(self):
+        """(re, im) as dense float32 torch tensors on the device."""
+        torch = self._torch
+        re = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        im = torch.empty(self.shape, dtype=torch.float32, device=self.device)
+        _check(lib().bvfdtd_read_phasor(self._h, re.data_ptr(), im.data_ptr(), 1), "bvfdtd_read_phasor")
+        return re, im
 
     # -- NEXT-2: plane reductions of the pulse-average intensity ---------------------------
     def plane_intensity(self):

@@ -695,6 +695,39 @@ int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const 
     return BVFDTD_OK;
 }
 
+namespace {
+__global__ void k_check_elements(const int n_pts, const int *__restrict__ element, const int n_elem, int *__restrict__ bad) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n_pts && (element[q] < 0 || element[q] >= n_elem)) atomicExch(bad, 1);
+}
+}  // namespace
+
+int bvfdtd_refocus_weights(int64_t n_pts, const float *p_re, const float *p_im, const int32_t *element, const float *area,
+                           int32_t n_elem, double f, double u0, float *w_pts, float *delay_s, float *E, void *cuda_stream) {
+    if (n_pts <= 0 || n_pts > (1 << 30) || n_elem <= 0 || n_elem > 65535 || !p_re || !p_im || !element || !area || !w_pts || !delay_s)
+        return BVFDTD_EINVAL;
+    if (!(f > 0.0) || !std::isfinite(u0)) return BVFDTD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float2 *d_unit = nullptr;
+    int *d_bad = nullptr;
+    CU(cudaMallocAsync(&d_unit, (size_t)n_elem * sizeof(float2), st));
+    CU(cudaMallocAsync(&d_bad, sizeof(int), st));
+    CU(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
+    k_check_elements<<<(unsigned)((n_pts + 127) / 128), 128, 0, st>>>((int)n_pts, element, n_elem, d_bad);
+    int bad = 0;
+    CU(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (!bad) {
+        k_element_phase<<<n_elem, 128, 0, st>>>((int)n_pts, p_re, p_im, element, (float)(1.0 / (2.0 * 3.14159265358979323846 * f)), d_unit,
+                                               delay_s, (float2 *)E);
+        k_point_weights<<<(unsigned)((n_pts + 127) / 128), 128, 0, st>>>((int)n_pts, element, area, d_unit, (float)u0, (float2 *)w_pts);
+    }
+    CU(cudaGetLastError());
+    CU(cudaFreeAsync(d_unit, st));
+    CU(cudaFreeAsync(d_bad, st));
+    return bad ? BVFDTD_EINVAL : BVFDTD_OK;
+}
+
 int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv, const float *rcv_xyz,
                     double f, double c0, double rho0, float *p_re, float *p_im, float *amp, float *delay_s, void *cuda_stream) {
     if (n_src <= 0 || n_rcv <= 0 || n_src > (1 << 30) || n_rcv > (1 << 30) || !src_xyz || !src_weight || !rcv_xyz || !p_re || !p_im)
