@@ -102,6 +102,8 @@ struct ZChunks {
 struct TiledPlan {
     TiledMaps mv, ms;      // velocity / stress pass (their tiles differ)
     StagePlan sv, ss;
+    StagePlan svc{};       // compact velocity stage plan (ns = 0: unused), see k_velocity_tiled
+    int occ_v = 2;         // register budget of the velocity instantiation in use (2 or 3 resident CTAs)
     bool s16 = true;       // stress pass runs 64 x 16 tiles (else 64 x 8)
     ZChunks zv, zs;        // z chunks of the velocity / stress launch
     bool ready = false;
@@ -551,21 +553,27 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
     }
 }
 
-template <class C>
-__global__ void __launch_bounds__(C::NT, 2) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
-                                                             const ZChunks zc, const StagePlan sp) {
+// OCC = resident CTAs per SM the registers are budgeted for.  `spf` is the stage plan with every psi
+// slot; `spc` a compact one without the y- and z-psi slots (more stages in the same shared memory) that
+// a CTA uses when its tile lies outside the y slabs and its chunk outside the z slabs (spc.ns = 0:
+// every CTA uses spf).  The pass is bound by the latency of its consumer warps, not by issue slots or
+// DRAM: three resident CTAs (12 consumer warps per SM) measured 8 % faster than two.
+template <class C, int OCC>
+__global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
+                                                               const ZChunks zc, const StagePlan spf, const StagePlan spc) {
     using VS = VStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
+    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
+    const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
+    const bool compact = spc.ns > 0 && !tile_in_y<C>(p, y0) && !(p.P > 0 && (kz0 < p.P || kz1 > p.nz - p.P));
+    const StagePlan sp = compact ? spc : spf;
     unsigned char *stages = smem;
     float *rho_tab = reinterpret_cast<float *>(smem + sp.ns * sp.bytes);
     float *sprof = rho_tab + 256;
     uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * C::TX);
     uint64_t *empty = full + MAX_STAGES;
-
-    const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
-    const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
 
     for (int q = tid; q < 256; q += C::NT) rho_tab[q] = p.rows[q].rho;
     fill_xprof<C>(sprof, p, x0, tid);
@@ -1058,7 +1066,7 @@ inline ZChunks plan_chunks(int nz, long long tiles, long long slots, double wave
     return z;
 }
 inline bool parse_chunks(const char *env, int nz, ZChunks &z) {   // "56,56,...": explicit lengths (experiments)
-    if (!env) return false;
+    if (!env || !*env) return false;
     int pos = 0, n = 0;
     z.b[0] = 0;
     const char *c = env;
@@ -1131,7 +1139,7 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
 }
 
 template <class C>
-inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb, int hdr_at = -1) {
+inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb, int hdr_at = -1, bool yz_slots = true) {
     StagePlan s;
     s.wxb = wxb;
     s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
@@ -1144,8 +1152,8 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     s.xhi = both ? s.xb : 0;
     s.xt = both ? 2 * s.xb : s.xb;
     s.psy = s.psx + 3 * s.xt;
-    s.psz = s.psy + (L.P > 0 ? 3 * C::D_BYTES : 0);
-    s.bytes = s.psz + (L.P > 0 ? 3 * C::D_BYTES : 0);
+    s.psz = s.psy + (L.P > 0 && yz_slots ? 3 * C::D_BYTES : 0);
+    s.bytes = s.psz + (L.P > 0 && yz_slots ? 3 * C::D_BYTES : 0);
     s.ns = ns;
     s.smem = ns * s.bytes + extra;
     return s;
@@ -1184,11 +1192,34 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     // the velocity stage header lives in the slack of the material slot (720 of 768 bytes used)
     static_assert(CfgV::M_BYTES - CfgV::MX * CfgV::MY >= (int)sizeof(StageHdr), "no room for the header behind the material box");
     const int v_hdr = VStage<CfgV>::MAT + CfgV::M_BYTES - (int)sizeof(StageHdr);
-    plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, ns_v, v_extra, wxb, v_hdr);
-    // two resident CTAs per SM matter more than a third stage
     const int smem_sm = 228 * 1024;
-    while (plan.sv.ns > 2 && (plan.sv.smem > smem_max || 2 * (plan.sv.smem + 1024) > smem_sm))
-        plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb, v_hdr);
+    // velocity pass, in order of preference (measured on config 2, PML 16: 0.320 / 0.337 / 0.344 ms):
+    //   THREE resident CTAs per SM (124 registers): 3 stages where the CTA needs no y- / z-psi slots
+    //   (compact plan), 2 stages elsewhere;  needs 3 (smem + 1 KB) <= 228 KB;
+    //   two resident CTAs (141 registers), up to 3 stages (thick PMLs).
+    const char *env_occ = std::getenv("BVFDTD_OCC_V");
+    const int occ_req = env_occ ? std::atoi(env_occ) : 0;
+    plan.svc = StagePlan{};
+    plan.occ_v = 2;
+    // (the dense sweep fills every stage and is bandwidth-bound: it measured better with 2 x 3 stages; small
+    // grids are launch-latency bound and lose more to the extra chunks than they gain)
+    if (occ_req != 2 && !env_v && (occ_req == 3 || (!dense && L.nz - 2 * L.P >= 128))) {
+        const StagePlan full2 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, L.P > 0 ? 2 : 3, v_extra, wxb, v_hdr);
+        const StagePlan comp3 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, 3, v_extra, wxb, v_hdr, false);
+        const int need = std::max(full2.smem, L.P > 0 ? comp3.smem : 0);
+        if (3 * (need + 1024) <= smem_sm && need <= smem_max) {
+            plan.sv = full2;
+            if (L.P > 0) plan.svc = comp3;
+            plan.sv.smem = need;
+            plan.occ_v = 3;
+        }
+    }
+    if (plan.occ_v == 2) {
+        plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, ns_v, v_extra, wxb, v_hdr);
+        // two resident CTAs per SM matter more than a third stage
+        while (plan.sv.ns > 2 && (plan.sv.smem > smem_max || 2 * (plan.sv.smem + 1024) > smem_sm))
+            plan.sv = make_stage<CfgV>(L, VStage<CfgV>::FIXED, plan.sv.ns - 1, v_extra, wxb, v_hdr);
+    }
     // stress pass, in order of preference (measured on config 2: 0.647 / 0.673 / 0.775 ms):
     //   64 x 8 tiles, 2 stages, TWO resident CTAs per SM (fits up to PML 16 with <= 128 materials);
     //   64 x 16 tiles, 2 stages, one CTA with 8 consumer warps;
@@ -1225,9 +1256,14 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     p.ntxS = L.ntxS; p.ntyS = L.ntyS;
     if (int rc = plan.s16 ? encode_maps<CfgS>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)
                           : encode_maps<CfgS8>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)) return rc;
-    e = cudaFuncSetAttribute(k_velocity_tiled<CfgV>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
     int occ_v = 1, occ_s = 1;
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV>, CfgV::NT, plan.sv.smem);
+    if (plan.occ_v == 3) {
+        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 3>, CfgV::NT, plan.sv.smem);
+    } else {
+        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 2>, CfgV::NT, plan.sv.smem);
+    }
     if (plan.s16) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<CfgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, k_stress_tiled<CfgS>, CfgS::NT, plan.ss.smem);
@@ -1243,12 +1279,26 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     const char *env_w = std::getenv("BVFDTD_WAVES");
     const double waves = env_w ? std::atof(env_w) : 2.6;
     plan.zv = plan_chunks(L.nz, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, waves);
+    if (plan.svc.ns > 0 && L.P >= 8 && L.nz - 2 * L.P >= 16) {
+        // the z slabs get chunks of their own, so that every other chunk can run the compact stage plan
+        // (measured on config 2 with three resident CTAs: nine chunks of 42 planes + a short tail 0.318 ms,
+        //  six of 60 0.327, four of 84 0.334, three of 105 0.357)
+        const ZChunks in = plan_chunks(L.nz - 2 * L.P, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, env_w ? waves : 3.9);
+        if (in.n + 2 <= MAX_CHUNKS) {
+            ZChunks z;
+            z.n = in.n + 2;
+            z.b[0] = 0;
+            for (int c = 0; c <= in.n; ++c) z.b[c + 1] = L.P + in.b[c];
+            z.b[z.n] = L.nz;
+            plan.zv = z;
+        }
+    }
     plan.zs = plan_chunks(L.nz, (long long)L.ntxS * L.ntyS, (long long)std::max(1, occ_s) * sms, waves);
     parse_chunks(std::getenv("BVFDTD_ZB_V"), L.nz, plan.zv);
     parse_chunks(std::getenv("BVFDTD_ZB_S"), L.nz, plan.zs);
     if (std::getenv("BVFDTD_VERBOSE")) {
-        std::fprintf(stderr, "[bvfdtd] velocity: ns %d stage %d smem %d occ %d; stress: tile 64x%d ns %d stage %d smem %d occ %d\n[bvfdtd] z chunks velocity:",
-                     plan.sv.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.s16 ? 16 : 8, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s);
+        std::fprintf(stderr, "[bvfdtd] velocity: ns %d (compact %d) stage %d smem %d occ %d; stress: tile 64x%d ns %d stage %d smem %d occ %d\n[bvfdtd] z chunks velocity:",
+                     plan.sv.ns, plan.svc.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.s16 ? 16 : 8, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s);
         for (int c = 0; c < plan.zv.n; ++c) std::fprintf(stderr, " %d", plan.zv.b[c + 1] - plan.zv.b[c]);
         std::fprintf(stderr, "; stress:");
         for (int c = 0; c < plan.zs.n; ++c) std::fprintf(stderr, " %d", plan.zs.b[c + 1] - plan.zs.b[c]);
@@ -1266,7 +1316,9 @@ inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV
     else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    k_velocity_tiled<CfgV><<<dim3(p.ntxV, p.ntyV, plan.zv.n), CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv);
+    const dim3 grid(p.ntxV, p.ntyV, plan.zv.n);
+    if (plan.occ_v == 3) k_velocity_tiled<CfgV, 3><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
+    else k_velocity_tiled<CfgV, 2><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
     return 0;
 }
 inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {
