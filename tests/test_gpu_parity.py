@@ -185,6 +185,30 @@ def test_stepped_random_domain(bv, dims, P, wave, flags):
     sim.close()
 
 
+@pytest.mark.parametrize("dims,P,wave", [((150, 41, 70), 8, 1), ((131, 45, 66), 12, 0), ((64, 40, 52), 0, 1)])
+def test_velocity_three_cta_stage_plans(bv, dims, P, wave, monkeypatch):
+    """The velocity pass with three resident CTAs per SM and per-CTA stage plans (compact 3-stage plan
+    outside the y / z slabs, full 2-stage plan inside; z slabs in chunks of their own) is what config 2
+    runs by default; BVFDTD_OCC_V=3 forces it on a small grid with ragged tiles and several chunks: it
+    must match the oracle AND be bit-identical to the two-CTA plan (BVFDTD_OCC_V=2)."""
+    w = wl.random_domain(*dims, P, seed=60 + P, steps=90, waveform=wave)
+    monkeypatch.setenv("BVFDTD_OCC_V", "3")
+    sim, o = run_both(bv, w)
+    compare_state(sim, o)
+    peak, rms = sim.read_peak_pressure()
+    compare_map(peak, o.get("peak"))
+    compare_map(rms, o.get("rms_amp"))
+    monkeypatch.setenv("BVFDTD_OCC_V", "2")
+    two = bv.Simulation.from_workload(w)
+    two.step(w.steps)
+    for n in bv.FIELDS:
+        assert np.array_equal(sim.read_fields(n), two.read_fields(n)), n
+    pk2, rms2 = two.read_peak_pressure()
+    assert np.array_equal(peak, pk2) and np.array_equal(rms, rms2)
+    sim.close()
+    two.close()
+
+
 @pytest.mark.parametrize("dims,P,seed", [((150, 43, 38), 6, 1), ((70, 30, 61), 5, 2), ((64, 64, 40), 8, 3)])
 def test_tile_class_skipping(bv, dims, P, seed):
     """Mostly-fluid, partly lossless domains: the default path skips the shear stresses and memory
