@@ -573,6 +573,9 @@ int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, 
         return BVFDTD_OK;
     }
     void *target = dst_is_device ? dst : (void *)scratch;
+    // r_yy / r_zz are not kept where they equal r_xx (all-fluid lossy tile-planes of the tiled path): fill them in
+    if ((id == RYY || id == RZZ) && !c->dense && !(c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS))
+        tiled_fill_rii(c->plan, c->prm, c->stream);
     if (id < NSTATE) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.f[id], c->prm);
     else if (id == BVFDTD_F_SUMSQ) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.sumsq, c->prm);
     else if (id == BVFDTD_F_PRESSURE) k_pressure<<<g, b, 0, c->stream>>>((float *)target, c->prm);
@@ -591,15 +594,17 @@ int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_
         CU(cudaMemcpyAsync(scratch, src, src_bytes, cudaMemcpyHostToDevice, c->stream));
         d_src = scratch;
     }
-    k_pack<<<grid3(c->L), 128, 0, c->stream>>>(c->prm.f[id], d_src, c->prm, id <= VZ ? (int)id : -1);
-    CU(cudaGetLastError());
     if (id >= SXY && !c->dense && !(c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS)) {
         // a caller-supplied shear stress or memory variable may be non-zero where the tile-class
-        // flags assume it is identically zero: switch this context to the dense sweep
+        // flags assume it is identically zero (or equal to r_xx): switch this context to the dense
+        // sweep, after r_yy / r_zz have been filled in where only r_xx was kept
+        tiled_fill_rii(c->plan, c->prm, c->stream);
         c->dense = true;
         tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), true, c->stream);
         CU(cudaGetLastError());
     }
+    k_pack<<<grid3(c->L), 128, 0, c->stream>>>(c->prm.f[id], d_src, c->prm, id <= VZ ? (int)id : -1);
+    CU(cudaGetLastError());
     if (!src_is_device) CU(cudaStreamSynchronize(c->stream));
     return BVFDTD_OK;
 }

@@ -642,7 +642,8 @@ enum : uint32_t {
     SC_RII1 = 64u,                             // plane m-1 has lossy cells
     SC_XZ2 = 128u, SC_YZ2 = 256u,              // plane m-2: finish sxz / syz
     SC_ZS1 = 512u, SC_ZS2 = 1024u,             // plane m-1 / m-2 lies in a z slab (and inside the chunk)
-    SC_PEAK = 2048u, SC_RMS = 4096u
+    SC_PEAK = 2048u, SC_RMS = 4096u,
+    SC_RFL1 = 8192u                            // plane m-1 is lossy but holds no solid cell: r_xx = r_yy = r_zz, only r_xx moves
 };
 
 struct ShearCoef { float cU, cR; };   // dt mu_U,h and B mu_h tau_h of one shear node (readings P2, P3)
@@ -660,8 +661,8 @@ __device__ __forceinline__ void shear_update(const ShearCoef &k, float g, float 
     sn = s0 + fmaf(k.cU, g, hdt * (rn + r0));
 }
 
-// The loads of one stress iteration m (flag words of planes m, m-1, m-2 in hist, 4 bits each,
-// newest lowest).
+// The loads of one stress iteration m (flag words of planes m, m-1, m-2 in the low half of hist, 4 bits
+// each, newest lowest; their TF_SOLID bits in the high half, 1 bit each, newest at bit 16).
 template <class C>
 struct StrIssue {
     const TiledMaps *maps; const Params *p; const StagePlan *sp;
@@ -672,7 +673,7 @@ struct StrIssue {
         const uint32_t f0 = hist & 15u, f1 = (hist >> 4) & 15u, f2 = (hist >> 8) & 15u;
         uint32_t c = sens;
         if (in0) c |= SC_IN0 | ((f0 & TF_XY) ? SC_XY0 : 0u) | ((f0 & TF_XZ) ? SC_XZ0 : 0u) | ((f0 & TF_YZ) ? SC_YZ0 : 0u);
-        if (in1) c |= SC_IN1 | ((f1 & TF_RII) ? SC_RII1 : 0u) | (z_in_slab(*p, m - 1) ? SC_ZS1 : 0u);
+        if (in1) c |= SC_IN1 | ((f1 & TF_RII) ? (SC_RII1 | (((hist >> 17) & 1u) ? 0u : SC_RFL1)) : 0u) | (z_in_slab(*p, m - 1) ? SC_ZS1 : 0u);
         if (in2) c |= SC_IN2 | ((f2 & TF_XZ) ? SC_XZ2 : 0u) | ((f2 & TF_YZ) ? SC_YZ2 : 0u) | (z_in_slab(*p, m - 2) ? SC_ZS2 : 0u);
         return c;
     }
@@ -708,8 +709,11 @@ struct StrIssue {
 #pragma unroll
             for (int q = 0; q < 3; ++q) t.box4(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, SXX + q);
             if (c & SC_RII1) {
+                t.box4(SS::RII, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX);
+                if (!(c & SC_RFL1)) {
 #pragma unroll
-                for (int q = 0; q < 3; ++q) t.box4(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
+                    for (int q = 1; q < 3; ++q) t.box4(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
+                }
             }
             // phasor mode (NEXT-3) keeps its two accumulators in the peak / sumsq slots
             if (c & SC_PEAK) t.box4(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHRE : F_PEAK);
@@ -794,7 +798,24 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
                 const Q4 vii[3] = {nxx, nyy, vzz};
                 const uint32_t gq = goff - (uint32_t)p.sz;
                 Q4 tr = zero;
-                if (ctrl & SC_RII1) {
+                if (ctrl & SC_RFL1) {
+                    // no solid cell in the tile-plane: eS = bS = 0, so the three memory variables obey one and
+                    // the same recursion from the same (zero) start and only r_xx is kept in memory; the
+                    // arithmetic below is the general branch's with the terms that are exactly zero left out
+                    // (x - 0 * y = x bit for bit), so both branches give the same bits
+                    const Q4 bP = q_make(r0.z, r1.z, r2.z, r3.z);
+                    const Q4 bPth = q_mul(bP, th);
+                    const Q4 rold = q_ld(dbase + SS::RII / 4);
+                    const Q4 rn = q_sub(q_muls(rold, A), bPth);
+                    const Q4 inc = q_fmas(hdt, q_add(rn, rold), ePth);
+                    q_store<EDGE>(p.f[RXX] + gq, rn, g.nv);
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), inc);
+                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        tr = q_add(tr, sn);
+                    }
+                } else if (ctrl & SC_RII1) {
                     const Q4 bP = q_make(r0.z, r1.z, r2.z, r3.z), bS = q_make(r0.w, r1.w, r2.w, r3.w);
                     const Q4 bPth = q_mul(bP, th);
 #pragma unroll
@@ -968,7 +989,10 @@ __global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(con
             int mr = ((m_begin % MR) + MR) % MR;
             uint32_t hist = 0;       // flag words of planes m, m-1, m-2 ..., 4 bits each
             for (int m = m_begin; m < m_end; ++m) {
-                hist = (hist << 4) | (__ldg(flags + m) & 15u);
+                {
+                    const uint32_t fw = __ldg(flags + m);
+                    hist = ((hist << 4) & 0xffffu) | (fw & 15u) | (((((hist >> 16) << 1) | ((fw >> 4) & 1u)) & 0xffffu) << 16);
+                }
                 StageHdr h;
                 h.ctrl = iss.ctrl(m, hist);
                 h.az1 = h.bz1 = h.az2 = h.bz2 = 0.0f;
@@ -1008,7 +1032,7 @@ __global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__
     __syncthreads();
     uint32_t f = 0;
     if (dense) {
-        f = pass == 0 ? (TF_XY | TF_XZ | TF_YZ) : (TF_XY | TF_XZ | TF_YZ | TF_RII);
+        f = pass == 0 ? (TF_XY | TF_XZ | TF_YZ) : (TF_XY | TF_XZ | TF_YZ | TF_RII | TF_SOLID);
     } else {
         const int h = pass == 0 ? 2 : 0;
         const int EX = C::TX + 2 * h, EY = C::TY + 2 * h;
@@ -1027,6 +1051,7 @@ __global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__
             if (nxz && iny) f |= TF_XZ;      // velocity reads sxz with an x halo only
             if (nyz && inx) f |= TF_YZ;      // ... syz with a y halo only
             if (pass == 1 && (r000.bP != 0.0f || r000.bS != 0.0f)) f |= TF_RII;
+            if (pass == 1 && s000 != 0.0f) f |= TF_SOLID;
         }
     }
     if (f) atomicOr(&sf, f);
@@ -1309,6 +1334,22 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
 }
 
 inline void tiled_plan_destroy(TiledPlan &plan) { plan.ready = false; }
+
+// r_yy and r_zz of the tile-planes in which only r_xx is kept (SC_RFL1): fill them in from r_xx (before
+// they are read back, and before the context switches to the dense sweep)
+__global__ void __launch_bounds__(128) k_fill_rii(const Params p, const int ty_tile) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= p.nx) return;
+    const uint32_t fw = p.flagsS[(size_t)(i / CfgS::TX + p.ntxS * (j / ty_tile)) * (p.nz + 4) + 2 + k];
+    if (!(fw & TF_RII) || (fw & TF_SOLID)) return;
+    const long long c = p.org + i + (long long)p.px * j + p.sz * k;
+    const float r = p.f[RXX][c];
+    p.f[RYY][c] = r;
+    p.f[RZZ][c] = r;
+}
+inline void tiled_fill_rii(const TiledPlan &plan, const Params &p, cudaStream_t st) {
+    k_fill_rii<<<dim3((p.nx + 127) / 128, p.ny, p.nz), 128, 0, st>>>(p, plan.s16 ? CfgS::TY : CfgS8::TY);
+}
 
 inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st) {
     k_tile_flags<CfgV><<<dim3(p.ntxV, p.ntyV, p.nz), 128, 0, st>>>(p, flagsV, p.ntxV, 0, dense ? 1 : 0);

@@ -447,3 +447,34 @@ def test_create_and_source_validation(bv):
     sim.step(3)
     assert sim.read_fields("p").any()
     sim.close()
+
+
+def test_fluid_memory_variable_kept_once(bv):
+    """In a lossy FLUID tile-plane the tiled stress pass keeps only r_xx (r_yy = r_zz = r_xx exactly:
+    eS = bS = 0, same recursion, same zero start).  r_yy / r_zz read back must equal the oracle's and
+    the dense sweep's bit for bit, also after the context is switched to the dense sweep in mid-run
+    by writing a memory variable (the library fills r_yy / r_zz in before it switches)."""
+    w = wl.blocky_domain(134, 45, 40, 6, seed=11, steps=40)
+    # make the background a lossy fluid (brain-like) so that most tile-planes are lossy and all-fluid
+    w.table = w.table.copy()
+    w.table[0] = (1040.0, 1546.0, 0.0, 30.0, 0.0)
+    sim, o = run_both(bv, w)
+    compare_state(sim, o, rel=2e-5)
+    dense = bv.Simulation.from_workload(w, flags=bv.FLAG_DENSE)
+    dense.step(w.steps)
+    got = {n: sim.read_fields(n) for n in ("rxx", "ryy", "rzz", "sxx", "syy", "szz")}
+    assert np.abs(got["ryy"]).max() > 0
+    for n, a in got.items():
+        assert np.array_equal(a, dense.read_fields(n)), n
+    fluid_only = ~np.isin(w.index_map, np.nonzero(w.table[:, 2] > 0)[0])
+    assert np.array_equal(got["ryy"][fluid_only], got["rxx"][fluid_only])
+    # switch to the dense sweep in mid-run: write r_xy back unchanged, continue, compare with the dense twin
+    sim.write_fields("rxy", sim.read_fields("rxy"))
+    sim.step(25)
+    dense.step(25)
+    o.step(25)
+    compare_state(sim, o, rel=2e-5)
+    for n in bv.FIELDS:
+        assert np.array_equal(sim.read_fields(n), dense.read_fields(n)), n
+    sim.close()
+    dense.close()
