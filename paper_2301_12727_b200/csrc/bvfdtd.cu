@@ -122,6 +122,7 @@ struct bvfdtd_ctx {
     double f_src = 0;
     // tiled-kernel plan (tensor maps etc.)
     TiledPlan plan;
+    bool sigma_written = false;   // a normal stress was written by the caller: no sigma_xx-for-all in the velocity pass
     bool dense = false;   // tile-class skipping off (BVFDTD_FLAG_DENSE, or a shear / memory field was written)
     // kernel timing
     bool timing = false;
@@ -601,6 +602,13 @@ int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_
         tiled_fill_rii(c->plan, c->prm, c->stream);
         c->dense = true;
         tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), true, c->stream);
+        CU(cudaGetLastError());
+    }
+    if (id >= SXX && id <= SZZ && !c->dense && !c->sigma_written && !(c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS)) {
+        // a caller-supplied normal stress need not satisfy sigma_xx = sigma_yy = sigma_zz in the fluid: the
+        // velocity pass stops reading sigma_xx in place of the other two
+        c->sigma_written = true;
+        tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), false, c->stream, false);
         CU(cudaGetLastError());
     }
     k_pack<<<grid3(c->L), 128, 0, c->stream>>>(c->prm.f[id], d_src, c->prm, id <= VZ ? (int)id : -1);

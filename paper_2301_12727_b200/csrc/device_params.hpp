@@ -59,6 +59,8 @@ enum : uint32_t {
     TF_XZ = 2u,    //         ... xz ...
     TF_YZ = 4u,    //         ... yz ...
     TF_RII = 8u,   // stress: some cell of the tile-plane is lossy (r_ii can be non-zero)
+    TF_VFLUID = 8u,  // velocity (shares the bit with TF_RII, which only the stress pass uses): every cell of the
+                     // halo-extended tile-plane is a fluid, so sigma_xx = sigma_yy = sigma_zz there and one array serves
     TF_SOLID = 16u,  // stress: some cell of the tile-plane is a solid (else eS = bS = 0 and r_xx = r_yy = r_zz)
     // velocity: the same three bits, taken over the halo-extended region the pass reads
 };

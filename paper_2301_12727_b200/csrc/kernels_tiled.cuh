@@ -349,7 +349,8 @@ enum : uint32_t {
     VC_IN0 = 1u, VC_IN1 = 2u, VC_IN2 = 4u,   // plane m / m-1 / m-2 inside the chunk
     VC_XY = 8u, VC_XZ = 16u, VC_YZ = 32u,    // plane m carries non-zero sxy / sxz / syz (halo-extended tile)
     VC_WXZ = 64u, VC_WYZ = 128u,             // some plane of m-3..m carries non-zero sxz / syz
-    VC_ZS1 = 256u, VC_ZS2 = 512u             // plane m-1 / m-2 lies in a z slab (and inside the chunk)
+    VC_ZS1 = 256u, VC_ZS2 = 512u,            // plane m-1 / m-2 lies in a z slab (and inside the chunk)
+    VC_FL = 1024u                            // plane m (inside the chunk): all-fluid extended tile, sigma_xx stands for the three
 };
 
 // The loads of one velocity iteration m, derived from the chunk range and the flag words of planes
@@ -365,6 +366,7 @@ struct VelIssue {
         if (fl & TF_XY) c |= VC_XY;
         if (fl & TF_XZ) c |= VC_XZ;
         if (fl & TF_YZ) c |= VC_YZ;
+        if (in0 && (fl & TF_VFLUID)) c |= VC_FL;
         if (any & TF_XZ) c |= VC_WXZ;
         if (any & TF_YZ) c |= VC_WYZ;
         if (in1 && z_in_slab(*p, m - 1)) c |= VC_ZS1;
@@ -377,12 +379,18 @@ struct VelIssue {
         const bool xy = c & VC_XY, xz = c & VC_XZ, yz = c & VC_YZ;
         const uint32_t xbox = (uint32_t)sp->wxb * C::TY * 4;
         const int z = m + 2;
-        t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, SZZ);
+        // all-fluid extended tile: sigma_xx = sigma_yy = sigma_zz bit for bit (eS = 0, isotropic source, zero
+        // start), so ONE box of sigma_xx with both halos (rows j-1 .. j+9, in the idle sxy slot) serves D+x,
+        // D+y and D+z instead of the three boxes
+        if (c & VC_FL) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 1, z, SXX);
+        else t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, SZZ);
         if (xz) t.box4(VS::SXZ, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXZ);
         if (yz) t.box4(VS::SYZ, C::B_BYTES, &maps->boxB, x0, y0 - 2, z, SYZ);
         if (c & VC_IN0) {
-            t.box4(VS::SXX, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXX);
-            t.box4(VS::SYY, C::B_BYTES, &maps->boxB, x0, y0 - 1, z, SYY);
+            if (!(c & VC_FL)) {
+                t.box4(VS::SXX, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXX);
+                t.box4(VS::SYY, C::B_BYTES, &maps->boxB, x0, y0 - 1, z, SYY);
+            }
             if (xy) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, SXY);
             // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
             const bool use[3] = {true, xy, xz};
@@ -449,7 +457,8 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
             const float *sB_yz = reinterpret_cast<const float *>(st + VS::SYZ) + qoff;     // row j-2
             const float *psz = reinterpret_cast<const float *>(st + sp.psz) + qoff;
             // ---- z chains: push plane m ----
-            Q4 dzz = zc_push(zzz, q_ld(reinterpret_cast<const float *>(st + VS::SZZ) + qoff), c1, c2);
+            const float *sF = reinterpret_cast<const float *>(st + VS::SXY) + aoff;      // VC_FL: sigma_xx box, row j-1
+            Q4 dzz = zc_push(zzz, (ctrl & VC_FL) ? q_ld(sF + C::AX) : q_ld(reinterpret_cast<const float *>(st + VS::SZZ) + qoff), c1, c2);
             Q4 dzx = zero, dzy = zero;
             if (ctrl & VC_WXZ) dzx = zc_push(zxz, (ctrl & VC_XZ) ? q_ld(sA_xz) : zero, c1, c2);
             if (ctrl & VC_WYZ) dzy = zc_push(zyz, (ctrl & VC_YZ) ? q_ld(sB_yz + 2 * C::TX) : zero, c1, c2);
@@ -510,10 +519,16 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
 
             // ---- x-y derivative sums of plane m ----
             if (ctrl & VC_IN0) {
-                const float *sA_xx = reinterpret_cast<const float *>(st + VS::SXX) + aoff;
-                const float *sB_yy = reinterpret_cast<const float *>(st + VS::SYY) + qoff;   // row j-1
-                Q4 dxx = x_dplus(sA_xx, c1, c2);                                             // D+x sxx -> vx
-                Q4 dyy = q_d4(q_ld(sB_yy), q_ld(sB_yy + C::TX), q_ld(sB_yy + 2 * C::TX), q_ld(sB_yy + 3 * C::TX), c1, c2);   // D+y syy -> vy
+                Q4 dxx, dyy;
+                if (ctrl & VC_FL) {
+                    dxx = x_dplus(sF + C::AX, c1, c2);                                       // D+x sxx -> vx
+                    dyy = q_d4(q_ld(sF), q_ld(sF + C::AX), q_ld(sF + 2 * C::AX), q_ld(sF + 3 * C::AX), c1, c2);   // D+y (syy = sxx) -> vy
+                } else {
+                    const float *sA_xx = reinterpret_cast<const float *>(st + VS::SXX) + aoff;
+                    const float *sB_yy = reinterpret_cast<const float *>(st + VS::SYY) + qoff;   // row j-1
+                    dxx = x_dplus(sA_xx, c1, c2);                                            // D+x sxx -> vx
+                    dyy = q_d4(q_ld(sB_yy), q_ld(sB_yy + C::TX), q_ld(sB_yy + 2 * C::TX), q_ld(sB_yy + 3 * C::TX), c1, c2);   // D+y syy -> vy
+                }
                 Q4 dxy_y = zero, dxy_x = zero, dxz = zero, dyz = zero;
                 if (ctrl & VC_XY) {
                     const float *sC = reinterpret_cast<const float *>(st + VS::SXY) + aoff;  // row j-2
@@ -1024,8 +1039,11 @@ __global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(con
 // One CTA per (tile, plane).  solid(m) = mu_R > 0; a shear node is "solid" when its four cells are
 // (reading P2; out-of-grid neighbours are the replicated edge of the private index map).
 // pass 0: velocity flags (taken over the halo-extended tile the pass reads), pass 1: stress flags.
+// vfluid (pass 0 only): also set TF_VFLUID where the extended tile holds no solid cell (off once the caller
+// has written a normal stress: sigma_xx = sigma_yy = sigma_zz is then no longer guaranteed)
 template <class C>
-__global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__restrict__ flags, const int ntx, const int pass, const int dense) {
+__global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__restrict__ flags, const int ntx, const int pass, const int dense,
+                                                    const int vfluid) {
     __shared__ uint32_t sf;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, k = blockIdx.z;
     if (threadIdx.x == 0) sf = 0;
@@ -1051,12 +1069,19 @@ __global__ void __launch_bounds__(128) k_tile_flags(const Params p, uint32_t *__
             if (nxz && iny) f |= TF_XZ;      // velocity reads sxz with an x halo only
             if (nyz && inx) f |= TF_YZ;      // ... syz with a y halo only
             if (pass == 1 && (r000.bP != 0.0f || r000.bS != 0.0f)) f |= TF_RII;
-            if (pass == 1 && s000 != 0.0f) f |= TF_SOLID;
+            if (s000 != 0.0f) f |= TF_SOLID;
         }
     }
     if (f) atomicOr(&sf, f);
     __syncthreads();
-    if (threadIdx.x == 0) flags[(size_t)(blockIdx.x + ntx * blockIdx.y) * (p.nz + 4) + 2 + k] = sf;
+    if (threadIdx.x == 0) {
+        uint32_t w = sf;
+        if (pass == 0) {
+            w &= (TF_XY | TF_XZ | TF_YZ);
+            if (vfluid && !dense && !(sf & TF_SOLID)) w |= TF_VFLUID;
+        }
+        flags[(size_t)(blockIdx.x + ntx * blockIdx.y) * (p.nz + 4) + 2 + k] = w;
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1351,10 +1376,11 @@ inline void tiled_fill_rii(const TiledPlan &plan, const Params &p, cudaStream_t 
     k_fill_rii<<<dim3((p.nx + 127) / 128, p.ny, p.nz), 128, 0, st>>>(p, plan.s16 ? CfgS::TY : CfgS8::TY);
 }
 
-inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st) {
-    k_tile_flags<CfgV><<<dim3(p.ntxV, p.ntyV, p.nz), 128, 0, st>>>(p, flagsV, p.ntxV, 0, dense ? 1 : 0);
-    if (plan.s16) k_tile_flags<CfgS><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
-    else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0);
+inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV, uint32_t *flagsS, bool dense, cudaStream_t st,
+                        bool vfluid = true) {
+    k_tile_flags<CfgV><<<dim3(p.ntxV, p.ntyV, p.nz), 128, 0, st>>>(p, flagsV, p.ntxV, 0, dense ? 1 : 0, vfluid ? 1 : 0);
+    if (plan.s16) k_tile_flags<CfgS><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0, 0);
+    else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0, 0);
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
     const dim3 grid(p.ntxV, p.ntyV, plan.zv.n);

@@ -76,13 +76,15 @@ def _min_bytes(self, rms_frac: float = 0.0) -> float:
     and no shear memory variable (-60 B), a lossless cell no memory variable at all (-48 B in
     total), and in a lossy FLUID cell the three normal memory variables are one and the same number
     (eS = bS = 0: one recursion from the same zero start), so only one of them must move (-16 B):
-    fluid-lossless 82 B, fluid-lossy 90 B (SURVEY.md prints 114 = 166 - 60 + a slip; 106 with three
-    normal memory variables), solid-lossless 118 B, solid-lossy 166 B, plus
+    and its three normal stresses are one number too (the pressure), so the velocity pass needs to
+    read only one of them (-8 B; the stress pass still updates all three):
+    fluid-lossless 74 B, fluid-lossy 82 B (SURVEY.md prints 82 / 114 with three of each),
+    solid-lossless 118 B, solid-lossy 166 B, plus
     48 B per PML mask bit and 8 B per cell while the rms window is open.  Accounting only."""
     t = self.table
     solid = t[:, 2] > 0
     lossy = (t[:, 3] > 0) | ((t[:, 4] > 0) & solid)
-    per_mat = np.where(solid, np.where(lossy, 166.0, 118.0), np.where(lossy, 90.0, 82.0))
+    per_mat = np.where(solid, np.where(lossy, 166.0, 118.0), np.where(lossy, 82.0, 74.0))
     counts = np.bincount(self.index_map.ravel(), minlength=t.shape[0]).astype(np.float64)
     base = float((per_mat * counts).sum() / counts.sum())
     return base + 48.0 * self.mean_mask_bits() + 8.0 * rms_frac
