@@ -87,6 +87,9 @@ struct StagePlan {
     int bytes;             // stage size (multiple of 128)
     int ns;                // pipeline stages
     int smem;              // dynamic shared memory of the launch
+    int spw;               // velocity pass: columns of the x-profile rows kept in shared memory (TX, or 32 when the
+                           // slab part of a tile is at most 32 columns wide); 0 = TX
+    int nrho;              // velocity pass: entries of the density table in shared memory (0 = 256)
 };
 
 // z chunks of a launch: chunk c covers planes [b[c], b[c+1]).  Blocks are dispatched in blockIdx.z
@@ -297,10 +300,11 @@ __device__ __forceinline__ ThreadGeom<C> make_geom(const Params &p, const StageP
 }
 
 // x-slab profile coefficients of the tile columns, zero outside the slabs / the grid
+// (w columns per row starting at tile column `base`: the whole tile by default)
 template <class C>
-__device__ __forceinline__ void fill_xprof(float *sprof, const Params &p, int x0, int tid) {
-    for (int q = tid; q < 4 * C::TX; q += C::NT) {
-        const int a = q / C::TX, c = q % C::TX, i = x0 + c;
+__device__ __forceinline__ void fill_xprof(float *sprof, const Params &p, int x0, int tid, int w = C::TX, int base = 0) {
+    for (int q = tid; q < 4 * w; q += C::NT) {
+        const int a = q / w, c = q % w, i = x0 + base + c;
         const bool in = p.P > 0 && i < p.nx && (i < p.P || i >= p.nx - p.P);
         sprof[q] = in ? __ldg(p.prof[0][a] + i) : 0.0f;
     }
@@ -420,7 +424,7 @@ struct VelIssue {
     }
 };
 
-template <class C, bool EDGE>
+template <class C, bool EDGE, bool TRIM>
 __device__ __forceinline__ void velocity_consume(const Params &p, const StagePlan &sp, unsigned char *stages, const float *rho_tab,
                                                  const float *sprof, uint64_t *full, uint64_t *empty, int tid, int x0, int y0,
                                                  int m_begin, int m_end) {
@@ -437,6 +441,9 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
     const int qoff = ty * C::TX + 4 * tx;             // own quad inside a D / B(row 0) box
     const int aoff = ty * C::AX + 4 + 4 * tx;         // own quad inside an A / C(row 0) box
     const uint32_t zstride = (uint32_t)(p.px * p.ny);
+    // x-profile rows: width and first tile column (TRIM: only the columns that can lie in a slab are kept)
+    const int spw = (TRIM && sp.spw > 0) ? sp.spw : C::TX;
+    const int xbase = (TRIM && sp.spw > 0 && x0 >= p.P) ? max(x0, p.xhb) - x0 : 0;
 
     ZChain zxz, zyz, zzz;                             // D-z sxz, D-z syz (finish at m-1), D+z szz (finish at m-2)
     zc_clear(zxz); zc_clear(zyz); zc_clear(zzz);
@@ -538,10 +545,10 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
                 if (ctrl & VC_XZ) dxz = x_dminus(sA_xz, c1, c2);                             // D-x sxz -> vz
                 if (ctrl & VC_YZ) dyz = q_d4(q_ld(sB_yz), q_ld(sB_yz + C::TX), q_ld(sB_yz + 2 * C::TX), q_ld(sB_yz + 3 * C::TX), c1, c2);   // D-y syz -> vz
                 if (g.in_x) {
-                    const float *sp_x = sprof + 4 * tx;
-                    const Q4 ai = q_ld(sp_x), bi = q_ld(sp_x + C::TX);
+                    const float *sp_x = sprof + (4 * tx - xbase);
+                    const Q4 ai = q_ld(sp_x), bi = q_ld(sp_x + spw);
                     const float *ps = reinterpret_cast<const float *>(st + sp.psx) + g.psx_off;
-                    q_st(p.psi[0] + gxo, q_cpml(dxx, q_ld(ps), q_ld(sp_x + 2 * C::TX), q_ld(sp_x + 3 * C::TX)));
+                    q_st(p.psi[0] + gxo, q_cpml(dxx, q_ld(ps), q_ld(sp_x + 2 * spw), q_ld(sp_x + 3 * spw)));
                     if (ctrl & VC_XY) q_st(p.psi[1] + gxo, q_cpml(dxy_x, q_ld(ps + sp.xt / 4), ai, bi));
                     if (ctrl & VC_XZ) q_st(p.psi[2] + gxo, q_cpml(dxz, q_ld(ps + sp.xt / 2), ai, bi));
                 }
@@ -573,7 +580,10 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
 // a CTA uses when its tile lies outside the y slabs and its chunk outside the z slabs (spc.ns = 0:
 // every CTA uses spf).  The pass is bound by the latency of its consumer warps, not by issue slots or
 // DRAM: three resident CTAs (12 consumer warps per SM) measured 8 % faster than two.
-template <class C, int OCC>
+// TRIM: the density table and the x-profile rows are cut to what the context uses (sp.nrho, sp.spw), which
+// frees the last bytes three CTAs need with thick PMLs; the untrimmed instantiation keeps compile-time
+// strides (2 % faster on config 2).
+template <class C, int OCC, bool TRIM>
 __global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
                                                                const ZChunks zc, const StagePlan spf, const StagePlan spc) {
     using VS = VStage<C>;
@@ -582,16 +592,20 @@ __global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_cons
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
     const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
     const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
-    const bool compact = spc.ns > 0 && !tile_in_y<C>(p, y0) && !(p.P > 0 && (kz0 < p.P || kz1 > p.nz - p.P));
+    // (a compact plan without x-psi slots, spc.xt == 0, also needs a tile outside the x slabs)
+    const bool x_slab = p.P > 0 && (x0 < p.P || (x0 + C::TX > p.xhb && x0 < p.nx));
+    const bool compact = spc.ns > 0 && !tile_in_y<C>(p, y0) && !(p.P > 0 && (kz0 < p.P || kz1 > p.nz - p.P)) &&
+                         (spc.xt > 0 || !x_slab);
     const StagePlan sp = compact ? spc : spf;
     unsigned char *stages = smem;
+    const int nrho = (TRIM && sp.nrho > 0) ? sp.nrho : 256, spw_k = (TRIM && sp.spw > 0) ? sp.spw : C::TX;
     float *rho_tab = reinterpret_cast<float *>(smem + sp.ns * sp.bytes);
-    float *sprof = rho_tab + 256;
-    uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * C::TX);
+    float *sprof = rho_tab + nrho;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sprof + 4 * spw_k);
     uint64_t *empty = full + MAX_STAGES;
 
-    for (int q = tid; q < 256; q += C::NT) rho_tab[q] = p.rows[q].rho;
-    fill_xprof<C>(sprof, p, x0, tid);
+    for (int q = tid; q < nrho; q += C::NT) rho_tab[q] = p.rows[q].rho;
+    fill_xprof<C>(sprof, p, x0, tid, spw_k, (TRIM && sp.spw > 0 && x0 >= p.P) ? max(x0, p.xhb) - x0 : 0);
     if (tid == 0) {
         for (int s = 0; s < sp.ns; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], C::NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -634,8 +648,8 @@ __global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_cons
 
     // ================= consumers =================
     const bool edge = (x0 + C::TX >= p.nx) || (y0 + C::TY >= p.ny);
-    if (edge) velocity_consume<C, true>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
-    else velocity_consume<C, false>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
+    if (edge) velocity_consume<C, true, TRIM>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
+    else velocity_consume<C, false, TRIM>(p, sp, stages, rho_tab, sprof, full, empty, tid, x0, y0, m_begin, m_end);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1189,8 +1203,10 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
 }
 
 template <class C>
-inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb, int hdr_at = -1, bool yz_slots = true) {
-    StagePlan s;
+// yz_slots / x_slots: reserve the y- and z-psi (x-psi) slots (velocity pass: per-CTA compact plans)
+inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int wxb, int hdr_at = -1, bool yz_slots = true,
+                            bool x_slots = true) {
+    StagePlan s{};
     s.wxb = wxb;
     s.xb = L.P > 0 ? round128(wxb * C::TY * 4) : 0;
     s.yb = C::D_BYTES;
@@ -1201,6 +1217,7 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     const bool both = L.P > 0 && (C::TX > L.xhb || L.P > C::TX);
     s.xhi = both ? s.xb : 0;
     s.xt = both ? 2 * s.xb : s.xb;
+    if (!x_slots) s.xt = s.xhi = 0;
     s.psy = s.psx + 3 * s.xt;
     s.psz = s.psy + (L.P > 0 && yz_slots ? 3 * C::D_BYTES : 0);
     s.bytes = s.psz + (L.P > 0 && yz_slots ? 3 * C::D_BYTES : 0);
@@ -1254,10 +1271,27 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     // (the dense sweep fills every stage and is bandwidth-bound: it measured better with 2 x 3 stages; small
     // grids are launch-latency bound and lose more to the extra chunks than they gain)
     if (occ_req != 2 && !env_v && (occ_req == 3 || (!dense && L.nz - 2 * L.P >= 128))) {
-        const StagePlan full2 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, L.P > 0 ? 2 : 3, v_extra, wxb, v_hdr);
-        const StagePlan comp3 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, 3, v_extra, wxb, v_hdr, false);
+        // every byte counts against 3 (smem + 1 KB) <= 228 KB: the density table holds the materials in use,
+        // and the x-profile rows only the (at most 32) columns of a tile that can lie in a slab
+        const bool both = L.P > 0 && (CfgV::TX > L.xhb || L.P > CfgV::TX);
+        int spw = CfgV::TX, nrho = 256;
+        {
+            // (only when the untrimmed plan does not fit)
+            const StagePlan f0 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, L.P > 0 ? 2 : 3, v_extra, wxb, v_hdr);
+            if (3 * (f0.smem + 1024) > smem_sm) {
+                if (L.P > 0 && !both && wxb <= 32 && ((L.P + 3) & ~3) <= 32) spw = 32;
+                nrho = std::min(256, (p.n_mat + 31) & ~31);
+            }
+        }
+        const int extra3 = nrho * 4 + 4 * spw * 4 + bar_bytes;
+        StagePlan full2 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, L.P > 0 ? 2 : 3, extra3, wxb, v_hdr);
+        StagePlan comp3 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, 3, extra3, wxb, v_hdr, false);            // x-psi slots only
+        if (L.P > 0 && 3 * (comp3.smem + 1024) > smem_sm)
+            comp3 = make_stage<CfgV>(L, VStage<CfgV>::FIXED, 3, extra3, wxb, v_hdr, false, false);           // no psi slot at all
         const int need = std::max(full2.smem, L.P > 0 ? comp3.smem : 0);
         if (3 * (need + 1024) <= smem_sm && need <= smem_max) {
+            full2.spw = comp3.spw = spw == CfgV::TX ? 0 : spw;
+            full2.nrho = comp3.nrho = nrho == 256 ? 0 : nrho;
             plan.sv = full2;
             if (L.P > 0) plan.svc = comp3;
             plan.sv.smem = need;
@@ -1307,12 +1341,16 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     if (int rc = plan.s16 ? encode_maps<CfgS>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)
                           : encode_maps<CfgS8>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)) return rc;
     int occ_v = 1, occ_s = 1;
-    if (plan.occ_v == 3) {
-        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
-        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 3>, CfgV::NT, plan.sv.smem);
+    const bool trim_v = plan.sv.spw > 0 || plan.sv.nrho > 0;
+    if (plan.occ_v == 3 && trim_v) {
+        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 3, true>, CfgV::NT, plan.sv.smem);
+    } else if (plan.occ_v == 3) {
+        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 3, false>, CfgV::NT, plan.sv.smem);
     } else {
-        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
-        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 2>, CfgV::NT, plan.sv.smem);
+        e = cudaFuncSetAttribute(k_velocity_tiled<CfgV, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.sv.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_v, k_velocity_tiled<CfgV, 2, false>, CfgV::NT, plan.sv.smem);
     }
     if (plan.s16) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_stress_tiled<CfgS>, cudaFuncAttributeMaxDynamicSharedMemorySize, plan.ss.smem);
@@ -1384,8 +1422,10 @@ inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV
 }
 inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
     const dim3 grid(p.ntxV, p.ntyV, plan.zv.n);
-    if (plan.occ_v == 3) k_velocity_tiled<CfgV, 3><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
-    else k_velocity_tiled<CfgV, 2><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
+    if (plan.occ_v == 3 && (plan.sv.spw > 0 || plan.sv.nrho > 0))
+        k_velocity_tiled<CfgV, 3, true><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
+    else if (plan.occ_v == 3) k_velocity_tiled<CfgV, 3, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
+    else k_velocity_tiled<CfgV, 2, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
     return 0;
 }
 inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {

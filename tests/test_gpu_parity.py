@@ -185,13 +185,14 @@ def test_stepped_random_domain(bv, dims, P, wave, flags):
     sim.close()
 
 
-@pytest.mark.parametrize("dims,P,wave", [((150, 41, 70), 8, 1), ((131, 45, 66), 12, 0), ((64, 40, 52), 0, 1)])
+@pytest.mark.parametrize("dims,P,wave", [((150, 41, 70), 8, 1), ((131, 45, 66), 12, 0), ((64, 40, 52), 0, 1),
+                                         ((150, 60, 80), 24, 1), ((203, 57, 64), 20, 0)])
 def test_velocity_three_cta_stage_plans(bv, dims, P, wave, monkeypatch):
     """The velocity pass with three resident CTAs per SM and per-CTA stage plans (compact 3-stage plan
     outside the y / z slabs, full 2-stage plan inside; z slabs in chunks of their own) is what config 2
     runs by default; BVFDTD_OCC_V=3 forces it on a small grid with ragged tiles and several chunks: it
     must match the oracle AND be bit-identical to the two-CTA plan (BVFDTD_OCC_V=2)."""
-    w = wl.random_domain(*dims, P, seed=60 + P, steps=90, waveform=wave)
+    w = wl.random_domain(*dims, P, seed=60 + P, steps=90, waveform=wave, n_mat=200 if P == 20 else 6)
     monkeypatch.setenv("BVFDTD_OCC_V", "3")
     sim, o = run_both(bv, w)
     compare_state(sim, o)
