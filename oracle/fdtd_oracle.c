@@ -27,7 +27,11 @@
  * Parity pins (tests/test_oracle_pins.py, -m "not gpu"): T1 discrete dispersion relation
  * (temporal form), T2 spatial phase speed / attenuation, T2b continuum Q and phase speed,
  * T3 plate transmission, T4 discrete energy, T5 reciprocity, T6 PML reflection, T7 order of
- * convergence, T8 elastic limit and axis symmetry.  Unpinned against the paper (the paper is
+ * convergence, T8 elastic limit and axis symmetry; tests/test_oracle_source_pins.py: S1-S4 the
+ * source (sign, amplitude, delay as a time shift, burst gate, raised-cosine ramp), A1 the staggered
+ * material means on period-2 laminates (closed-form dispersion with rho arithmetic, mu harmonic,
+ * tau_s arithmetic), A2 the C-PML of a solid at oblique incidence (which profile each shear psi
+ * term takes).  Unpinned against the paper (the paper is
  * silent): the choice of ONE relaxation mechanism, the C-PML formulation, the averaging
  * rule -- "parity unpinned vs paper" for those choices; their implementation is pinned by
  * the closed forms above.
