@@ -170,6 +170,22 @@ int bvfdtd_step(bvfdtd_ctx *ctx, int64_t n);
 /* Number of steps enqueued so far (the index n of the next step). */
 int64_t bvfdtd_step_index(const bvfdtd_ctx *ctx);
 
+/* Number of steps sampled into the rms / phasor window so far (the `count` of reading P8). */
+int64_t bvfdtd_rms_count(const bvfdtd_ctx *ctx);
+
+/* Which kernels the next bvfdtd_step will run (a host-side query; tests and bench.py print it so that a
+ * parity claim names the path it holds for).  Bits of *mode: */
+enum {
+    BVFDTD_MODE_REFERENCE = 1,   /* one-thread-per-cell kernels (BVFDTD_FLAG_REFERENCE_KERNELS) */
+    BVFDTD_MODE_DENSE = 2,       /* tiled kernels, every array everywhere (BVFDTD_FLAG_DENSE, or a shear stress /
+                                    memory variable was written through bvfdtd_write_fields) */
+    BVFDTD_MODE_SIGMA_WRITTEN = 4, /* a normal stress was written by the caller: the fluid shortcuts that rely on
+                                    sigma_xx = sigma_yy = sigma_zz are off */
+    BVFDTD_MODE_FUSED = 8,       /* all-fluid tile columns run the fused single-sweep kernel */
+    BVFDTD_MODE_GRAPH = 16       /* bvfdtd_step replays a captured CUDA graph of one step */
+};
+int bvfdtd_kernel_mode(const bvfdtd_ctx *ctx, uint32_t *mode);
+
 /*
  * Copy one field out in the dense external layout.  dst_bytes must equal the field's size
  * (nx*ny*nz*4 for fp32 grid fields, nx*ny*nz for the uint8 fields, see the enum).  If

@@ -40,8 +40,9 @@ SYMBOLS = (
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
-    "bvfdtd_refocus_weights",
+    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode",
 )
+MODE_REFERENCE, MODE_DENSE, MODE_SIGMA_WRITTEN, MODE_FUSED, MODE_GRAPH = 1, 2, 4, 8, 16
 BHTE_TRACK_MAX = 1
 BHTE_WHAT = {"T": 0, "dose": 1, "tmax": 2, "rise": 3}
 
@@ -94,6 +95,9 @@ def lib():
         L.bvfdtd_step.argtypes = [vp, i64]
         L.bvfdtd_step_index.argtypes = [vp]
         L.bvfdtd_step_index.restype = i64
+        L.bvfdtd_rms_count.argtypes = [vp]
+        L.bvfdtd_rms_count.restype = i64
+        L.bvfdtd_kernel_mode.argtypes = [vp, C.POINTER(u32)]
         L.bvfdtd_read_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_write_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_read_peak_pressure.argtypes = [vp, vp, vp, i32]
@@ -294,6 +298,27 @@ class Simulation:
     @property
     def step_index(self):
         return lib().bvfdtd_step_index(self._h)
+
+    @property
+    def rms_count(self):
+        return lib().bvfdtd_rms_count(self._h)
+
+    def mode_bits(self):
+        m = C.c_uint32(0)
+        _check(lib().bvfdtd_kernel_mode(self._h, C.byref(m)), "bvfdtd_kernel_mode")
+        return m.value
+
+    def kernel_mode(self):
+        """the path the next step runs, in words (what bench.py prints as config.kernels)"""
+        m = self.mode_bits()
+        if m & MODE_REFERENCE:
+            return "reference (one thread per cell)"
+        if m & MODE_DENSE:
+            return "tiled, dense sweep"
+        s = "tiled, tile-class skipping"
+        if m & MODE_SIGMA_WRITTEN:
+            s += " (normal stresses written by the caller: fluid shortcuts off)"
+        return s
 
     def synchronize(self):
         self._stream.synchronize()

@@ -548,6 +548,18 @@ int bvfdtd_plane_span(const bvfdtd_grid *grid, uint32_t field_id, int32_t k, int
 
 int64_t bvfdtd_step_index(const bvfdtd_ctx *c) { return c ? c->step : -1; }
 
+int64_t bvfdtd_rms_count(const bvfdtd_ctx *c) { return c ? c->rms_count : -1; }
+
+int bvfdtd_kernel_mode(const bvfdtd_ctx *c, uint32_t *mode) {
+    if (!c || !mode) return BVFDTD_EINVAL;
+    uint32_t m = 0;
+    if (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) m |= BVFDTD_MODE_REFERENCE;
+    else if (c->dense) m |= BVFDTD_MODE_DENSE;
+    if (c->sigma_written) m |= BVFDTD_MODE_SIGMA_WRITTEN;
+    *mode = m;
+    return BVFDTD_OK;
+}
+
 int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, int32_t dst_is_device) {
     if (!c || !dst) return BVFDTD_EINVAL;
     const size_t need = field_bytes(c, id);
