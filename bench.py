@@ -48,17 +48,85 @@ def measured_hbm_peak():
         return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic_bytes(kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu summary."""
-    path = os.path.join(ROOT, "profiles", "traffic.csv")
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "traffic.csv")
+KERNEL_CLASSES = (("fused", "k_fluid_fused"), ("velocity", "k_velocity_tiled"), ("stress_sensor", "k_stress_tiled"))
+
+
+def kernel_source_hash():
+    """sha256 over the kernel sources and the nvcc flags of the library being timed: profiles/traffic.csv names
+    the hash it was captured for, and a capture of other code is refused."""
+    import hashlib
+    from paper_2301_12727_b200 import build as bv_build
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(bv_build.CSRC)):
+        if f.endswith((".cuh", ".cu", ".hpp", ".cpp")):
+            h.update(f.encode())
+            h.update(open(os.path.join(bv_build.CSRC, f), "rb").read())
+    h.update(" ".join(bv_build.NVCC_FLAGS).encode())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config):
+    """({kernel: dram read + write bytes per launch}, source note) from the committed ncu summary of THIS build
+    on workload `config`; ({}, why) when the capture belongs to other kernel sources or another workload."""
+    want = kernel_source_hash()
     try:
-        for line in open(path):
-            parts = [p.strip() for p in line.split(",")]
-            if parts and parts[0] == kernel:
-                return float(parts[1]) + float(parts[2])
-    except Exception:
+        lines = [ln.strip() for ln in open(TRAFFIC_CSV)]
+    except OSError:
+        return {}, "no profiles/traffic.csv"
+    have = None
+    out = {}
+    for ln in lines:
+        if ln.startswith("#"):
+            if "kernel_hash=" in ln:
+                have = ln.split("kernel_hash=")[1].split()[0]
+            continue
+        parts = [p.strip() for p in ln.split(",")]
+        if len(parts) >= 4 and parts[0] == str(config):
+            out[parts[1]] = float(parts[2]) + float(parts[3])
+    if have != want:
+        return {}, f"profiles/traffic.csv is a capture of kernel hash {have}; the library timed here is {want}: refused"
+    if not out:
+        return {}, f"profiles/traffic.csv (kernel hash {have}) holds no capture of config {config}"
+    return out, f"profiles/traffic.csv, ncu --set full capture of this build (kernel hash {have}), config {config}"
+
+
+def traffic_from_ncu(raw_csv, config):
+    """`bench.py --traffic-from <ncu -i x.ncu-rep --page raw --csv> --config C`: average dram__bytes_read.sum /
+    dram__bytes_write.sum per launch of each hot kernel into profiles/traffic.csv, stamped with the kernel hash."""
+    import csv
+    rows = list(csv.reader(open(raw_csv)))
+    hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+    names, units = rows[hdr], rows[hdr + 1]
+    col = {n: i for i, n in enumerate(names)}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    acc = {}
+    for r in rows[hdr + 2:]:
+        if len(r) <= col["dram__bytes_write.sum"]:
+            continue
+        for cls, pat in KERNEL_CLASSES:
+            if pat in r[col["Kernel Name"]]:
+                rd = float(r[col["dram__bytes_read.sum"]]) * scale[units[col["dram__bytes_read.sum"]]]
+                wr = float(r[col["dram__bytes_write.sum"]]) * scale[units[col["dram__bytes_write.sum"]]]
+                a = acc.setdefault(cls, [0.0, 0.0, 0])
+                a[0] += rd; a[1] += wr; a[2] += 1
+                break
+    want = kernel_source_hash()
+    keep = []
+    try:
+        old = [ln.rstrip("\n") for ln in open(TRAFFIC_CSV)]
+        if any(ln.startswith("#") and f"kernel_hash={want}" in ln for ln in old):
+            keep = [ln for ln in old if not ln.startswith("#") and ln.strip() and ln.split(",")[0].strip() != str(config)]
+    except OSError:
         pass
-    return None
+    with open(TRAFFIC_CSV, "w") as f:
+        f.write(f"# kernel_hash={want}  columns: config, kernel, dram__bytes_read.sum, dram__bytes_write.sum (bytes per launch, mean), launches\n")
+        for ln in keep:
+            f.write(ln + "\n")
+        for cls, (rd, wr, n) in sorted(acc.items()):
+            f.write(f"{config},{cls},{rd / n:.0f},{wr / n:.0f},{n}\n")
+    print(open(TRAFFIC_CSV).read())
+    return 0
 
 
 # ---------------------------------------------------------------------------------------------
@@ -106,26 +174,76 @@ def aggregate_rate(cells_per_rank, steps, ms_local, world, device="cpu"):
 # clocks
 # ---------------------------------------------------------------------------------------------
 class ClockSampler:
+    """SM clock and clock-event reasons sampled DURING the timed region: NVML in-process every 2 ms (a 20-step
+    run lasts ~15 ms, too short for nvidia-smi's own loop), `nvidia-smi -lms` as the fallback."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index):
-        self.index = index
-        self.proc = None
+    def __init__(self, index, uuid=None):
+        self.index, self.uuid = index, uuid
+        self.proc = self.thread = None
         self.path = os.path.join("/tmp", f"bvfdtd_clocks_{os.getpid()}.csv")
+        self.sm, self.reasons, self.sm_max, self.power = [], set(), None, []
+
+    def _nvml_loop(self, nv, h):
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake_slowdown"}
+        while not self._stop:
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                for bit, n in names.items():
+                    if r & bit:
+                        self.reasons.add(n)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def start(self):
         try:
+            import threading
+            import pynvml as nv
+            nv.nvmlInit()
+            h = None
+            if self.uuid:
+                try:
+                    h = nv.nvmlDeviceGetHandleByUUID(("GPU-" + str(self.uuid)).encode())
+                except Exception:
+                    h = None
+            if h is None:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+                ids = [v for v in vis.split(",") if v.strip().isdigit()]
+                h = nv.nvmlDeviceGetHandleByIndex(int(ids[self.index]) if self.index < len(ids) else self.index)
+            self.sm_max = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self._stop = False
+            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
+        try:
             self.f = open(self.path, "w")
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20",
                  "-i", str(self.index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.thread is not None:
+            self._stop = True
+            self.thread.join(timeout=2)
+            if self.sm:
+                out.update(sm_mhz=float(np.median(self.sm)), sm_max_mhz=self.sm_max, reasons=sorted(self.reasons),
+                           samples=len(self.sm), power_w_max=max(self.power) if self.power else None,
+                           how="NVML in-process, 2 ms period, over the timed region")
+            return out
         if self.proc is None:
             return out
         self.proc.terminate()
@@ -154,7 +272,7 @@ class ClockSampler:
             pass
         if sm:
             out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)),
-                       reasons=sorted(reasons), samples=len(sm))
+                       reasons=sorted(reasons), samples=len(sm), how="nvidia-smi -lms 20")
         return out
 
 
@@ -297,12 +415,18 @@ def ours(args):
     if args.dense:
         flags |= bv.FLAG_DENSE
 
-    # ---- device-resident timing -----------------------------------------------------------
-    sim = bv.Simulation.from_workload(w, flags=flags, device=dev)
+    # ---- device-resident timing: the call a user makes, bvfdtd_step(K) (CUDA-graph replay) ------
+    sim = bv.Simulation.from_workload(w, flags=flags, device=dev, tuning=args.tuning)
+    kernels_desc = sim.kernel_mode()
+    mode_bits = sim.mode_bits()
+    coverage = sim.fused_coverage()
     sim.step(W)
     sim.synchronize()
-    sim.enable_kernel_timing(True)
-    clocks = ClockSampler(local_rank)
+    try:
+        uuid = torch.cuda.get_device_properties(dev).uuid
+    except Exception:
+        uuid = None
+    clocks = ClockSampler(local_rank, uuid)
     clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -314,11 +438,26 @@ def ours(args):
     barrier()
     ms_local = e0.elapsed_time(e1)
     clk = clocks.stop()
-    kt = sim.kernel_times()
     value, ms = aggregate_rate(w.cells, K, ms_local, world, dev)
     peak_dev, _ = sim.read_peak_pressure_device()
     finite = bool(torch.isfinite(peak_dev).all()) and float(peak_dev.max()) > 0.0
     del peak_dev
+    sim.close()
+    del sim
+
+    # ---- the same W + K steps once more, kernel by kernel with CUDA events between the launches (the
+    #      library's own events on the context's stream): per-kernel durations for the roofline ----
+    sim = bv.Simulation.from_workload(w, flags=flags, device=dev, tuning=args.tuning)
+    sim.step(W)
+    sim.synchronize()
+    sim.enable_kernel_timing(True)
+    t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0e.record()
+    sim.step(min(K, 4096))
+    t1e.record()
+    torch.cuda.synchronize()
+    kt = sim.kernel_times()
+    ms_timed_pass = t0e.elapsed_time(t1e) / min(K, 4096)
     sim.close()
     del sim
     torch.cuda.empty_cache()
@@ -332,7 +471,7 @@ def ours(args):
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     sim = bv.Simulation(w.nx, w.ny, w.nz, w.pml, w.dx, w.dt, w.table, idx_np, w.f0, w.pml_R,
-                        w.peak_begin, w.rms_begin, w.sensor_end, flags=flags, device=dev)
+                        w.peak_begin, w.rms_begin, w.sensor_end, flags=flags, device=dev, tuning=args.tuning)
     sim.set_source(w.src_cell, w.src_amp, w.src_delay, w.waveform, w.f_src, w.n_cycles)
     sim.step(total)
     sim.read_peak_pressure(peak=True, rms=False, out_peak=peak_np)
@@ -359,17 +498,18 @@ def ours(args):
         avg_ms = kt[name]["ms"] / n
         kern[name] = {"avg_ms": avg_ms, "launches": kt[name]["launches"],
                       "algorithmic_bytes": b, "achieved_gbs": b / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else None}
-    kern["inject"] = {"avg_ms": kt["inject"]["ms"] / max(1, kt["inject"]["launches"]),
-                      "launches": kt["inject"]["launches"]}
+    for name in ("inject", "fused"):
+        kern[name] = {"avg_ms": kt[name]["ms"] / max(1, kt[name]["launches"]), "launches": kt[name]["launches"]}
     dom = "stress_sensor"
     ach_dense = kern[dom]["achieved_gbs"]
     step_bytes = vel_b + st_b
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
     min_step_bytes = w.min_bytes_per_cell_step(rms_frac=n_rms / K) * w.cells
-    have_ncu = args.config == 2 and not args.dense and not args.reference_kernels
     step_traffic = dom_traffic = None
-    if have_ncu:
-        tv, ts = ncu_traffic_bytes("velocity"), ncu_traffic_bytes("stress_sensor")
+    traffic, traffic_source = ({}, "dense / per-cell kernels: B_dense is what moves") if (args.dense or args.reference_kernels) \
+        else ncu_traffic(args.config)
+    if traffic:
+        tv, ts = traffic.get("velocity"), traffic.get("stress_sensor")
         if tv and ts:
             # the capture had both sensor maps on: take the sum-of-squares map (8 B per cell, read + write)
             # off for the timed steps outside the rms window, so bytes and times describe the same launches
@@ -389,6 +529,7 @@ def ours(args):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak_gbs, "unit": "GB/s",
                 "frac": ach / peak_gbs if ach else None,
                 "traffic": dom_traffic,
+                "traffic_source": traffic_source,
                 "rule": rule,
                 "bytes_definition": "B_dense of SURVEY.md 8(d): every array of every cell once per pass; the default "
                                     "path moves fewer bytes where shear stresses / memory variables are identically "
@@ -417,14 +558,15 @@ def ours(args):
                    "materials": int(w.table.shape[0]), "source_cells": int(w.src_cell.size),
                    "parallelism": f"replicas x{world} (no sharding)",
                    "l2": "state 2.4 GB per step >> 126 MB L2: inputs larger than L2, no flush",
-                   "kernels": "reference (one thread per cell)" if args.reference_kernels else
-                              ("tiled, dense sweep" if args.dense else "tiled, tile-class skipping"),
+                   "kernels": kernels_desc, "cuda_graph": bool(mode_bits & bv.MODE_GRAPH),
+                   "fused_tile_plane_fraction": coverage,
                    "result_finite_nonzero": finite},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d / total,
                 "d2h_bytes_per_step": d2h / total, "steps": total, "seconds": e2e_ms * 1e-3,
                 "what": "bvfdtd_create + set_source + step(W+K) + read_peak_pressure to pinned host"},
-        "gpu_launches": int(sum(kt[k]["launches"] for k in kt)),
+        "gpu_launches": int(round(sum(kt[k]["launches"] for k in kt) * K / max(1, min(K, 4096)))),
+        "ms_per_step_kernel_by_kernel": ms_timed_pass,
         "roofline": roofline,
     }
     if cpu is not None:
@@ -443,9 +585,14 @@ def main():
     ap.add_argument("--reference-kernels", action="store_true",
                     help="debug: time the one-thread-per-cell kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tuning", type=int, default=0, help="bvfdtd_opts.tuning bits (BVFDTD_TUNE_*), experiments")
+    ap.add_argument("--traffic-from", default=None,
+                    help="ncu `--page raw --csv` export of a --set full capture of this build: write profiles/traffic.csv")
     ap.add_argument("--dense", action="store_true",
                     help="BVFDTD_FLAG_DENSE: sweep every array everywhere (no tile-class skipping)")
     args = ap.parse_args()
+    if args.traffic_from:
+        return traffic_from_ncu(args.traffic_from, args.config)
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":

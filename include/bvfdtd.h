@@ -97,8 +97,19 @@ typedef struct {
     int64_t rms_begin;  /* first step index n sampled into the sum of squares (P8) */
     int64_t sensor_end; /* one past the last sampled step for both windows; < 0 = unbounded */
     uint32_t flags;     /* BVFDTD_FLAG_* */
-    uint32_t reserved;  /* must be 0 */
+    uint32_t tuning;    /* BVFDTD_TUNE_*: launch-plan requests for tests and experiments; 0 = the library's
+                           own choice.  Results never depend on it (every plan is bit-identical); any other
+                           bit set is BVFDTD_EINVAL.  The library reads no environment variable. */
 } bvfdtd_opts;
+
+enum { /* bvfdtd_opts.tuning */
+    BVFDTD_TUNE_VEL_2CTA = 1,   /* velocity pass: the two-resident-CTA plan (3 stages) */
+    BVFDTD_TUNE_VEL_3CTA = 2,   /* velocity pass: the three-resident-CTA plan with per-CTA stage plans, if it fits */
+    BVFDTD_TUNE_STRESS_8 = 4,   /* stress pass: 64 x 8 tiles */
+    BVFDTD_TUNE_STRESS_16 = 8,  /* stress pass: 64 x 16 tiles */
+    BVFDTD_TUNE_NO_GRAPH = 16,  /* bvfdtd_step launches kernel by kernel instead of replaying CUDA graphs */
+    BVFDTD_TUNE_NO_FUSED = 32   /* all-fluid tile columns run the two passes like every other tile (no fused sweep) */
+};
 
 /* Field ids for bvfdtd_read_fields / bvfdtd_write_fields. */
 enum {
@@ -216,13 +227,17 @@ const char *bvfdtd_strerror(int code);
 const char *bvfdtd_last_cuda_error(void);
 
 /* Device-time accounting for benchmarks: when enabled the library brackets every kernel of
- * bvfdtd_step with CUDA events on the context's stream; bvfdtd_kernel_times (which synchronises)
- * returns the accumulated milliseconds and launch counts per kernel (0 inject, 1 velocity,
- * 2 stress+sensor) since the last call and resets them.  At most `BVFDTD_MAX_TIMED_STEPS` steps
- * are recorded between two reads. */
+ * bvfdtd_step with CUDA events on the context's stream (and launches kernel by kernel instead of
+ * replaying CUDA graphs); bvfdtd_kernel_times (which synchronises) returns the accumulated
+ * milliseconds and launch counts per kernel (0 inject, 1 fused single sweep of the all-fluid tile
+ * columns, 2 velocity pass, 3 stress + sensor pass) since the last call and resets them.  At most
+ * `BVFDTD_MAX_TIMED_STEPS` steps are recorded between two reads. */
 enum { BVFDTD_MAX_TIMED_STEPS = 4096 };
 int bvfdtd_enable_kernel_timing(bvfdtd_ctx *ctx, int32_t on);
-int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[3], int64_t launches[3]);
+int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[4], int64_t launches[4]);
+/* How much of the grid the fused single sweep takes: 64 x 8 tile-planes it runs / all tile-planes
+ * (0 when the context is not in the fused mode, BVFDTD_MODE_FUSED).  Host-side query. */
+int bvfdtd_fused_coverage(const bvfdtd_ctx *ctx, int64_t *planes_fused, int64_t *planes_all);
 
 /* ---- host-only helpers (no CUDA device needed): the S0 constructions, exposed so that the
  * construction-parity tests can run anywhere.  Same code path bvfdtd_create uses. ---- */

@@ -26,6 +26,8 @@ FLAG_DENSE = 2
 FLAG_PHASOR = 4
 FLAG_ZLO_OPEN = 8
 FLAG_ZHI_OPEN = 16
+# bvfdtd_opts.tuning: launch-plan requests for tests and experiments (results never depend on them)
+TUNE_VEL_2CTA, TUNE_VEL_3CTA, TUNE_STRESS_8, TUNE_STRESS_16, TUNE_NO_GRAPH, TUNE_NO_FUSED = 1, 2, 4, 8, 16, 32
 
 OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 
@@ -40,7 +42,7 @@ SYMBOLS = (
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
-    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode",
+    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage",
 )
 MODE_REFERENCE, MODE_DENSE, MODE_SIGMA_WRITTEN, MODE_FUSED, MODE_GRAPH = 1, 2, 4, 8, 16
 BHTE_TRACK_MAX = 1
@@ -63,7 +65,7 @@ class Thermal(C.Structure):
 class Opts(C.Structure):
     _fields_ = [("f0", C.c_double), ("pml_R", C.c_double), ("peak_begin", C.c_int64),
                 ("rms_begin", C.c_int64), ("sensor_end", C.c_int64), ("flags", C.c_uint32),
-                ("reserved", C.c_uint32)]
+                ("tuning", C.c_uint32)]
 
 
 class BvfdtdError(RuntimeError):
@@ -98,6 +100,7 @@ def lib():
         L.bvfdtd_rms_count.argtypes = [vp]
         L.bvfdtd_rms_count.restype = i64
         L.bvfdtd_kernel_mode.argtypes = [vp, C.POINTER(u32)]
+        L.bvfdtd_fused_coverage.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.bvfdtd_read_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_write_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_read_peak_pressure.argtypes = [vp, vp, vp, i32]
@@ -225,7 +228,7 @@ class Simulation:
     """``bvfdtd_create`` .. ``bvfdtd_destroy`` around a torch-owned device workspace."""
 
     def __init__(self, nx, ny, nz, pml, dx, dt, table, index_map, f0, pml_R=1e-4, peak_begin=0,
-                 rms_begin=None, sensor_end=-1, flags=0, device="cuda:0", stream=None):
+                 rms_begin=None, sensor_end=-1, flags=0, device="cuda:0", stream=None, tuning=0):
         import torch
 
         if not torch.cuda.is_available():
@@ -249,7 +252,7 @@ class Simulation:
         arr, n = _materials(table)
         self.n_materials = n
         o = Opts(float(f0), float(pml_R), int(peak_begin), int(rms_begin), int(sensor_end),
-                 int(flags), 0)
+                 int(flags), int(tuning))
         h = C.c_void_p(None)
         with torch.cuda.device(self.device):
             rc = lib().bvfdtd_create(C.byref(h), C.byref(g), float(dx), float(dt), arr, n,
@@ -316,9 +319,17 @@ class Simulation:
         if m & MODE_DENSE:
             return "tiled, dense sweep"
         s = "tiled, tile-class skipping"
+        if m & MODE_FUSED:
+            s += ", fused sweep in all-fluid tile columns"
         if m & MODE_SIGMA_WRITTEN:
             s += " (normal stresses written by the caller: fluid shortcuts off)"
         return s
+
+    def fused_coverage(self):
+        """fraction of the 64 x 8 tile-planes the fused single sweep takes (0.0 outside the fused mode)"""
+        a, b = C.c_int64(0), C.c_int64(0)
+        _check(lib().bvfdtd_fused_coverage(self._h, C.byref(a), C.byref(b)), "bvfdtd_fused_coverage")
+        return a.value / max(1, b.value)
 
     def synchronize(self):
         self._stream.synchronize()
@@ -415,10 +426,10 @@ class Simulation:
                "bvfdtd_enable_kernel_timing")
 
     def kernel_times(self):
-        ms = (C.c_double * 3)()
-        n = (C.c_int64 * 3)()
+        ms = (C.c_double * 4)()
+        n = (C.c_int64 * 4)()
         _check(lib().bvfdtd_kernel_times(self._h, ms, n), "bvfdtd_kernel_times")
-        names = ("inject", "velocity", "stress_sensor")
+        names = ("inject", "fused", "velocity", "stress_sensor")
         return {k: {"ms": ms[i], "launches": n[i]} for i, k in enumerate(names)}
 
 

@@ -60,6 +60,7 @@ struct bvfdtd_bhte {
     char *ws = nullptr;
     BhteMap W{};
     cudaStream_t stream = nullptr;
+    int device = -1;        // owner of the workspace: every entry point runs on it (DeviceScope)
     int cur = 0;            // th[cur] holds the present state
     int zlen = 1, nchunk = 1;
     int n_mat = 0;
@@ -95,9 +96,13 @@ int bvfdtd_bhte_create(bvfdtd_bhte **out, int32_t nx, int32_t ny, int32_t nz, do
     const BhteMap W = make_map(nx, ny, nz, flags);
     if (workspace_bytes < W.total) return BVFDTD_ENOMEM;
 
+    const int ws_dev = device_of(d_workspace);
+    if (ws_dev < 0) return cuda_fail(cudaErrorInvalidDevicePointer, "d_workspace is not device memory (or no CUDA device)");
+    DeviceScope scope(ws_dev);
     bvfdtd_bhte *c = new (std::nothrow) bvfdtd_bhte;
     if (!c) return BVFDTD_ENOMEM;
     struct Guard { bvfdtd_bhte *p; ~Guard() { delete p; } } guard{c};
+    c->device = ws_dev;
     c->nx = nx; c->ny = ny; c->nz = nz; c->px = (nx + 63) / 64 * 64;
     c->flags = flags; c->dx = dx; c->dt = dt; c->T_b = T_b;
     c->ws = (char *)d_workspace; c->W = W; c->stream = (cudaStream_t)cuda_stream; c->n_mat = n_materials;
@@ -125,11 +130,15 @@ int bvfdtd_bhte_create(bvfdtd_bhte **out, int32_t nx, int32_t ny, int32_t nz, do
         const double eff = (double)ctas / (double)(waves * slots);
         if (eff > best_eff + 0.02) { best_eff = eff; best = n; }
     }
+#ifdef BVFDTD_DEV_KNOBS   // experiments only: the shipped library's launch plan does not depend on the environment
     if (const char *e = std::getenv("BVFDTD_BHTE_CHUNKS"); e && *e) best = std::max(1, std::min(max_chunks, std::atoi(e)));
+#endif
     c->zlen = (nz + best - 1) / best;
     c->nchunk = (nz + c->zlen - 1) / c->zlen;
+#ifdef BVFDTD_DEV_KNOBS
     if (std::getenv("BVFDTD_VERBOSE"))
         std::fprintf(stderr, "[bvfdtd] bhte: tiles %d chunks %d (zlen %d) occ %d slots %d\n", tiles, c->nchunk, c->zlen, occ, slots);
+#endif
 
     const size_t cells = (size_t)nx * ny * nz;
     CU(cudaMemsetAsync(c->ws, 0, W.total, c->stream));
@@ -170,6 +179,7 @@ int stage_in(bvfdtd_bhte *c, const float *src, int32_t src_is_device, const floa
 
 int bvfdtd_bhte_set_heat(bvfdtd_bhte *c, const float *Q, int32_t src_is_device) {
     if (!c || !Q) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     const float *d_src = nullptr;
     int rc = stage_in(c, Q, src_is_device, &d_src);
     if (rc) return rc;
@@ -182,6 +192,7 @@ int bvfdtd_bhte_set_heat(bvfdtd_bhte *c, const float *Q, int32_t src_is_device) 
 
 int bvfdtd_bhte_set_temperature(bvfdtd_bhte *c, const float *T, int32_t src_is_device) {
     if (!c || !T) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     const float *d_src = nullptr;
     int rc = stage_in(c, T, src_is_device, &d_src);
     if (rc) return rc;
@@ -195,6 +206,7 @@ int bvfdtd_bhte_set_temperature(bvfdtd_bhte *c, const float *T, int32_t src_is_d
 
 int bvfdtd_bhte_step(bvfdtd_bhte *c, int64_t n, double heat_scale) {
     if (!c || n < 0 || !(heat_scale >= 0.0) || !std::isfinite(heat_scale)) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     BhteParams p;
     p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.px = c->px; p.sz = c->px * c->ny;
     p.zlen = c->zlen; p.n_mat = c->n_mat;
@@ -221,6 +233,7 @@ int bvfdtd_bhte_step(bvfdtd_bhte *c, int64_t n, double heat_scale) {
 
 int bvfdtd_bhte_read(bvfdtd_bhte *c, uint32_t what, float *dst, size_t dst_bytes, int32_t dst_is_device) {
     if (!c || !dst || what > BVFDTD_BHTE_RISE) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     const size_t bytes = (size_t)c->nx * c->ny * c->nz * 4;
     if (dst_bytes < bytes) return BVFDTD_EINVAL;
     if (what == BVFDTD_BHTE_TMAX && !(c->flags & BVFDTD_BHTE_TRACK_MAX)) return BVFDTD_ESTATE;
@@ -245,6 +258,7 @@ int bvfdtd_bhte_read(bvfdtd_bhte *c, uint32_t what, float *dst, size_t dst_bytes
 
 int bvfdtd_bhte_destroy(bvfdtd_bhte *c) {
     if (!c) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     cudaStreamSynchronize(c->stream);
     delete c;
     return BVFDTD_OK;

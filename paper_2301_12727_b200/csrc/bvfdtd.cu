@@ -16,6 +16,7 @@
 #include "host_common.hpp"
 #include "kernels_ref.cuh"
 #include "kernels_tiled.cuh"
+#include "kernels_fused.cuh"
 #include "kernels_post.cuh"
 #include "kernels_rs.cuh"
 
@@ -72,7 +73,10 @@ Layout make_layout(const bvfdtd_grid &g) {
 
 // Offsets (bytes) of every region of the caller's workspace.
 struct WsMap {
-    size_t field[NSTATE], peak, sumsq, phre, phim, scratch, mat, psi[18], rows, prof, flagsV, flagsS, invz, total;
+    size_t field[NSTATE], peak, sumsq, phre, phim, alt[6], scratch, mat, psi[18], psi7_alt, rows, prof, flagsV, flagsS, flagsF,
+        invz, ctr, src, items[3], cls, total;
+    size_t zero0, zero1;      // [zero0, zero1): state, sensors, psi, flag words, counters -- what bvfdtd_create zeroes (reading P9)
+    long long src_cap;        // source cells the workspace has room for (16 bytes each); more go to a library-owned allocation
 };
 
 WsMap make_wsmap(const Layout &L) {
@@ -84,15 +88,25 @@ WsMap make_wsmap(const Layout &L) {
     w.sumsq = take(L.field_floats * 4);
     w.phre = take(L.field_floats * 4);
     w.phim = take(L.field_floats * 4);
+    for (int q = 0; q < 6; ++q) w.alt[q] = take(L.field_floats * 4);     // ping-pong copies of VX..SZZ (fused sweep)
+    for (int a = 0; a < 3; ++a) {
+        for (int t = 0; t < 6; ++t) w.psi[a * 6 + t] = take(L.psi_floats[a] * 4);
+        if (a == 1) w.psi7_alt = take(L.psi_floats[1] * 4);              // ping-pong copy of psi[7], 7th array of the y block
+    }
+    w.flagsF = take((size_t)L.flag_wordsV * 4);
+    w.flagsV = take((size_t)L.flag_wordsV * 4);          // (the words of planes -2, -1, nz, nz+1 stay zero)
+    w.flagsS = take((size_t)L.flag_wordsS * 4);
+    w.ctr = take(256);                                   // device step counter + block ticket of k_inject, index-map maximum
+    w.zero0 = 0; w.zero1 = off;
     w.scratch = take((size_t)L.nx * L.ny * L.nz * 4);
     w.mat = take(L.mat_bytes);
-    for (int a = 0; a < 3; ++a)
-        for (int t = 0; t < 6; ++t) w.psi[a * 6 + t] = take(L.psi_floats[a] * 4);
     w.rows = take(256 * sizeof(KRow));
     w.prof = take((size_t)4 * (L.nx + L.ny + L.nz) * 4);
-    w.flagsV = take((size_t)L.flag_wordsV * 4);
-    w.flagsS = take((size_t)L.flag_wordsS * 4);
     w.invz = take(256 * 4);
+    w.src_cap = 4LL * L.nx * L.ny;                       // a source plane or array fits; larger lists are library-owned
+    w.src = take((size_t)w.src_cap * 16);
+    for (int q = 0; q < 3; ++q) w.items[q] = take(fused_items_capacity(L) * sizeof(int4));   // work lists of the fused mode
+    w.cls = take((size_t)L.ntxV * L.ntyV * L.nz);
     w.total = off;
     return w;
 }
@@ -104,6 +118,7 @@ struct bvfdtd_ctx {
     WsMap W;
     char *ws = nullptr;
     cudaStream_t stream = nullptr;
+    int device = -1;      // owner of the workspace: every entry point runs on it (DeviceScope)
     double dx = 0, dt = 0;
     bvfdtd_opts opts{};
     int n_materials = 0;
@@ -118,12 +133,23 @@ struct bvfdtd_ctx {
     int64_t n_src = 0;
     long long *d_cell = nullptr;
     float *d_amp = nullptr, *d_delay = nullptr;
+    void *src_own = nullptr;     // library-owned copy of a source list too long for the workspace's source region
     int waveform = 0, n_cycles = 1;
     double f_src = 0;
     // tiled-kernel plan (tensor maps etc.)
     TiledPlan plan;
+    // fused single sweep of the all-fluid tile columns (kernels_fused.cuh); sel = which copy of the ping-pong
+    // arrays holds the current time level (0 = the primary arrays)
+    FusedPlan fplan;
+    bool ff_active = false;
+    int sel = 0;
     bool sigma_written = false;   // a normal stress was written by the caller: no sigma_xx-for-all in the velocity pass
     bool dense = false;   // tile-class skipping off (BVFDTD_FLAG_DENSE, or a shear / memory field was written)
+    // CUDA graphs of one step and of GRAPH_STEPS steps per sensor regime (peak on/off x rms on/off), built on first use
+    enum { GRAPH_STEPS = 8 };
+    cudaGraphExec_t graph[4][2][2] = {};
+    cudaStream_t cap_stream = nullptr;     // library-owned stream the graphs are captured on (the caller's may be the
+                                           // legacy default stream, which cannot be captured); nothing ever runs on it   // [regime][one step | GRAPH_STEPS steps][sel at the first step]
     // kernel timing
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -221,6 +247,72 @@ int deliver(bvfdtd_ctx *c, void *dst, const void *d_dense, size_t bytes, int dst
     return BVFDTD_OK;
 }
 
+void drop_graphs(bvfdtd_ctx *c) {
+    for (auto &a : c->graph)
+        for (auto &b : a)
+            for (cudaGraphExec_t &g : b)
+                if (g) { cudaGraphExecDestroy(g); g = nullptr; }
+}
+
+// Decide which tile columns run the fused single sweep (kernels_fused.cuh) and build the three work lists.
+// Not for the per-cell kernels, the dense sweep, the phasor sensor, z-slab contexts (their halo planes are
+// refreshed between the passes) or on request (BVFDTD_TUNE_NO_FUSED).
+int fused_setup(bvfdtd_ctx *c) {
+    const uint32_t off = BVFDTD_FLAG_REFERENCE_KERNELS | BVFDTD_FLAG_DENSE | BVFDTD_FLAG_PHASOR | BVFDTD_FLAG_ZLO_OPEN | BVFDTD_FLAG_ZHI_OPEN;
+    if ((c->opts.flags & off) || (c->opts.tuning & BVFDTD_TUNE_NO_FUSED)) return BVFDTD_OK;
+    const Layout &L = c->L;
+    int rc = fused_plan_create(c->fplan, c->plan, L, c->prm, c->ws + c->W.psi[6], (long long)(c->W.psi[7] - c->W.psi[6]));
+    if (rc == BVFDTD_EINVAL) return BVFDTD_OK;                 // the stages do not fit: stay with the two passes
+    if (rc) return cuda_fail(cudaGetLastError(), "fused_plan_create");
+    uint8_t *d_cls = (uint8_t *)(c->ws + c->W.cls);
+    k_fused_class<<<dim3(L.ntxV, L.ntyV, L.nz), 128, 0, c->stream>>>(c->prm, d_cls);
+    CU(cudaGetLastError());
+    std::vector<uint8_t> cls((size_t)L.ntxV * L.ntyV * L.nz);
+    CU(cudaMemcpyAsync(cls.data(), d_cls, cls.size(), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    int sms = 148, occ_f = 1;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_fluid_fused<CfgF>, CfgF::NT, c->fplan.smem));
+    const int sty = c->plan.s16 ? CfgS::TY : CfgS8::TY;
+    const FusedLists lists = fused_lists(L, cls, sty, sms * std::max(1, occ_f), sms * std::max(1, c->plan.occ_v_res),
+                                         sms * std::max(1, c->plan.occ_s_res));
+    const long long planes_all = (long long)L.ntxV * L.ntyV * L.nz;
+    c->fplan.planes_f = lists.planes_f;
+    c->fplan.planes_all = planes_all;
+    // worth it from a tenth of the tile-planes on (below that the extra launch costs more than it saves)
+    if (lists.planes_f * 10 < planes_all) return BVFDTD_OK;
+    const size_t cap = fused_items_capacity(L);
+    if (lists.f.size() > cap || lists.v.size() > cap || lists.s.size() > cap) return BVFDTD_OK;
+    const std::vector<int4> *src[3] = {&lists.f, &lists.v, &lists.s};
+    for (int q = 0; q < 3; ++q)
+        if (!src[q]->empty())
+            CU(cudaMemcpyAsync(c->ws + c->W.items[q], src[q]->data(), src[q]->size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaMemcpyAsync(c->ws + c->W.flagsF, lists.flags.data(), lists.flags.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    c->fplan.items_f = (const int4 *)(c->ws + c->W.items[0]); c->fplan.n_f = (int)lists.f.size();
+    c->fplan.items_v = (const int4 *)(c->ws + c->W.items[1]); c->fplan.n_v = (int)lists.v.size();
+    c->fplan.items_s = (const int4 *)(c->ws + c->W.items[2]); c->fplan.n_s = (int)lists.s.size();
+    c->ff_active = true;
+    return BVFDTD_OK;
+}
+
+// sigma_yy = sigma_zz = sigma_xx in the planes the fused sweep keeps as sigma_xx only
+int fused_fill(bvfdtd_ctx *c) {
+    if (!c->ff_active) return BVFDTD_OK;
+    k_fill_sii<<<grid3(c->L), 128, 0, c->stream>>>(c->prm);
+    CU(cudaGetLastError());
+    return BVFDTD_OK;
+}
+
+// Leave the fused mode for good: every tile column runs the two passes again, in place on the current copies.
+int fused_disable(bvfdtd_ctx *c) {
+    if (!c->ff_active) return BVFDTD_OK;
+    const int rc = fused_fill(c);
+    if (rc) return rc;
+    c->ff_active = false;
+    drop_graphs(c);
+    return BVFDTD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -305,7 +397,11 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     *out = nullptr;
     if (!grid_ok(grid) || !table || !index_map || !opts || !d_workspace) return BVFDTD_EINVAL;
     if (!(dx > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dt)) return BVFDTD_EINVAL;
-    if (!(opts->f0 > 0.0) || opts->reserved != 0) return BVFDTD_EINVAL;
+    constexpr uint32_t TUNE_ALL = BVFDTD_TUNE_VEL_2CTA | BVFDTD_TUNE_VEL_3CTA | BVFDTD_TUNE_STRESS_8 | BVFDTD_TUNE_STRESS_16 |
+                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED;
+    if (!(opts->f0 > 0.0) || (opts->tuning & ~TUNE_ALL) != 0) return BVFDTD_EINVAL;
+    if ((opts->tuning & BVFDTD_TUNE_VEL_2CTA) && (opts->tuning & BVFDTD_TUNE_VEL_3CTA)) return BVFDTD_EINVAL;
+    if ((opts->tuning & BVFDTD_TUNE_STRESS_8) && (opts->tuning & BVFDTD_TUNE_STRESS_16)) return BVFDTD_EINVAL;
     double R = opts->pml_R == 0.0 ? 1e-4 : opts->pml_R;
     if (!(R > 0.0 && R < 1.0)) return BVFDTD_EINVAL;
     if (((uintptr_t)d_workspace & 255) != 0) return BVFDTD_EINVAL;
@@ -322,6 +418,10 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     c->L = make_layout(*grid);
     c->W = make_wsmap(c->L);
     if (workspace_bytes < c->W.total) return BVFDTD_ENOMEM;
+    // the context lives on the device that owns the workspace, whatever device is current in the caller
+    c->device = device_of(d_workspace);
+    if (c->device < 0) return cuda_fail(cudaErrorInvalidDevicePointer, "d_workspace is not device memory (or no CUDA device)");
+    DeviceScope scope(c->device);
     c->ws = (char *)d_workspace;
     c->stream = (cudaStream_t)cuda_stream;
     c->dx = dx; c->dt = dt; c->opts = *opts; c->opts.pml_R = R; c->n_materials = n_materials;
@@ -342,29 +442,25 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
         for (const std::vector<float> *v : {&c->pml[a].a_int, &c->pml[a].b_int, &c->pml[a].a_half, &c->pml[a].b_half})
             prof.insert(prof.end(), v->begin(), v->end());
     }
-    // zero the whole workspace (state, sensors, psi; reading P9), then upload
-    CU(cudaMemsetAsync(c->ws, 0, c->W.total, c->stream));
-    // index map: dense upload into the scratch plane, then validated and padded into the private
-    // layout on the device (edges replicated, reading P2)
-    CU(cudaMemcpyAsync(c->ws + c->W.scratch, index_map, cells, cudaMemcpyHostToDevice, c->stream));
-    {
-        int *d_max = (int *)(c->ws + c->W.invz);      // zeroed by the memset above; the table is uploaded after the check
-        const dim3 b(128), g((L.px + 127) / 128, L.py, L.nz + 1);
-        k_pad_index_map<<<g, b, 0, c->stream>>>((uint8_t *)(c->ws + c->W.mat), (const uint8_t *)(c->ws + c->W.scratch), L.nx, L.ny, L.nz, L.px, L.py, L.sz, d_max);
-        CU(cudaGetLastError());
-        int h_max = 0;
-        CU(cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        if (h_max >= n_materials) return BVFDTD_EINVAL;
-        CU(cudaMemsetAsync(c->ws + c->W.scratch, 0, cells, c->stream));
-    }
+    // small tables first, while the stream is still empty (a pageable source is staged before cudaMemcpyAsync
+    // returns, so the vectors may die at return; it also waits for the stream's earlier work)
     CU(cudaMemcpyAsync(c->ws + c->W.rows, rows.data(), 256 * sizeof(KRow), cudaMemcpyHostToDevice, c->stream));
     CU(cudaMemcpyAsync(c->ws + c->W.prof, prof.data(), prof.size() * 4, cudaMemcpyHostToDevice, c->stream));
     float invz[256];
     for (int m = 0; m < 256; ++m) invz[m] = m < n_materials ? (float)(1.0 / (table[m].rho * table[m].cL)) : 0.0f;
     CU(cudaMemcpyAsync(c->ws + c->W.invz, invz, sizeof(invz), cudaMemcpyHostToDevice, c->stream));
-    CU(cudaStreamSynchronize(c->stream));  // host staging buffers die at return
-
+    // zero the state, the sensors, psi, the flag words and the counters (reading P9); the scratch plane, the
+    // index map and the tables are fully written below
+    CU(cudaMemsetAsync(c->ws + c->W.zero0, 0, c->W.zero1 - c->W.zero0, c->stream));
+    // index map: dense upload into the scratch plane, then validated and padded into the private
+    // layout on the device (edges replicated, reading P2)
+    CU(cudaMemcpyAsync(c->ws + c->W.scratch, index_map, cells, cudaMemcpyHostToDevice, c->stream));
+    int *d_max = (int *)(c->ws + c->W.ctr + 16);
+    {
+        const dim3 b(128), g((L.px + 127) / 128, L.py, L.nz + 1);
+        k_pad_index_map<<<g, b, 0, c->stream>>>((uint8_t *)(c->ws + c->W.mat), (const uint8_t *)(c->ws + c->W.scratch), L.nx, L.ny, L.nz, L.px, L.py, L.sz, d_max);
+        CU(cudaGetLastError());
+    }
     Params &p = c->prm;
     p.nx = L.nx; p.ny = L.ny; p.nz = L.nz; p.P = L.P;
     p.n_mat = n_materials;
@@ -380,6 +476,10 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     p.phim = (float *)(c->ws + c->W.phim);
     p.mat = (const uint8_t *)(c->ws + c->W.mat);
     for (int q = 0; q < 18; ++q) p.psi[q] = (float *)(c->ws + c->W.psi[q]);
+    // no fused sweep (yet): the passes work in place, cur == nxt
+    for (int q = 0; q < 6; ++q) { p.icur[q] = p.inxt[q] = q; p.fnxt[q] = p.f[q]; }
+    p.ipsi7_cur = 1; p.psi7_nxt = p.psi[7];
+    p.flagsF = (const uint32_t *)(c->ws + c->W.flagsF);
     p.rows = (const KRow *)(c->ws + c->W.rows);
     {
         const float *base = (const float *)(c->ws + c->W.prof);
@@ -401,13 +501,22 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
             psi_base[a] = c->ws + c->W.psi[a * 6];
             psi_stride[a] = (long long)(c->W.psi[a * 6 + 1] - c->W.psi[a * 6]);
         }
-        rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride, (opts->flags & BVFDTD_FLAG_DENSE) != 0);
+        PlanTuning tune;
+        tune.occ_v = (opts->tuning & BVFDTD_TUNE_VEL_2CTA) ? 2 : (opts->tuning & BVFDTD_TUNE_VEL_3CTA) ? 3 : 0;
+        tune.stress_ty = (opts->tuning & BVFDTD_TUNE_STRESS_8) ? 8 : (opts->tuning & BVFDTD_TUNE_STRESS_16) ? 16 : 0;
+        rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride, (opts->flags & BVFDTD_FLAG_DENSE) != 0, tune);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
         c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;
         tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);
         CU(cudaGetLastError());
-        CU(cudaStreamSynchronize(c->stream));
     }
+    // the one synchronisation of create: the largest material index of the map (validation)
+    int h_max = 0;
+    CU(cudaMemcpyAsync(&h_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (h_max >= n_materials) return BVFDTD_EINVAL;
+    rc = fused_setup(c);
+    if (rc) return rc;
     guard.c = nullptr;
     *out = c;
     return BVFDTD_OK;
@@ -416,6 +525,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
 int bvfdtd_set_source(bvfdtd_ctx *c, int64_t n_src, const int64_t *cell, const float *amp,
                       const float *delay_s, int32_t waveform, double f_src, int32_t n_cycles) {
     if (!c || n_src < 0) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     if (n_src > 0) {
         if (!cell || !amp || !delay_s || !(f_src > 0.0) || n_cycles < 1 || (waveform != 0 && waveform != 1))
             return BVFDTD_EINVAL;
@@ -434,18 +544,32 @@ int bvfdtd_set_source(bvfdtd_ctx *c, int64_t n_src, const int64_t *cell, const f
             if (!std::isfinite(amp[s]) || !std::isfinite(delay_s[s])) return BVFDTD_EINVAL;
         }
     }
-    CU(cudaStreamSynchronize(c->stream));
-    if (c->d_cell) { cudaFree(c->d_cell); cudaFree(c->d_amp); cudaFree(c->d_delay); }
-    c->d_cell = nullptr; c->d_amp = c->d_delay = nullptr;
+    // the device copy lives in the workspace's source region (room for four x-y planes of cells); only a longer
+    // list gets a library-owned allocation.  The arrays are packed on the host first, so the caller's buffers
+    // are free at return without a stream synchronisation (a pageable source is staged before
+    // cudaMemcpyAsync returns).
+    drop_graphs(c);
     c->n_src = 0;
+    c->d_cell = nullptr; c->d_amp = c->d_delay = nullptr;
+    if (c->src_own) {
+        CU(cudaStreamSynchronize(c->stream));     // a step in flight may still read the old list
+        cudaFree(c->src_own);
+        c->src_own = nullptr;
+    }
     if (n_src > 0) {
-        CU(cudaMalloc(&c->d_cell, n_src * sizeof(long long)));
-        CU(cudaMalloc(&c->d_amp, n_src * 4));
-        CU(cudaMalloc(&c->d_delay, n_src * 4));
-        CU(cudaMemcpyAsync(c->d_cell, cell, n_src * 8, cudaMemcpyHostToDevice, c->stream));
-        CU(cudaMemcpyAsync(c->d_amp, amp, n_src * 4, cudaMemcpyHostToDevice, c->stream));
-        CU(cudaMemcpyAsync(c->d_delay, delay_s, n_src * 4, cudaMemcpyHostToDevice, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
+        char *d_base = c->ws + c->W.src;
+        if (n_src > c->W.src_cap) {
+            CU(cudaMalloc(&c->src_own, (size_t)n_src * 16));
+            d_base = (char *)c->src_own;
+        }
+        std::vector<char> pack((size_t)n_src * 16);
+        std::memcpy(pack.data(), cell, (size_t)n_src * 8);
+        std::memcpy(pack.data() + (size_t)n_src * 8, amp, (size_t)n_src * 4);
+        std::memcpy(pack.data() + (size_t)n_src * 12, delay_s, (size_t)n_src * 4);
+        CU(cudaMemcpyAsync(d_base, pack.data(), pack.size(), cudaMemcpyHostToDevice, c->stream));
+        c->d_cell = (long long *)d_base;
+        c->d_amp = (float *)(d_base + (size_t)n_src * 8);
+        c->d_delay = (float *)(d_base + (size_t)n_src * 12);
         c->n_src = n_src; c->waveform = waveform; c->f_src = f_src; c->n_cycles = n_cycles;
     }
     return BVFDTD_OK;
@@ -455,15 +579,45 @@ namespace {
 
 enum { PH_INJECT = 1, PH_VELOCITY = 2, PH_STRESS = 4, PH_ALL = 7 };
 
-// The passes of step c->step selected by `phases`; the step counter advances with the stress pass.
-int run_phases(bvfdtd_ctx *c, int phases) {
-    const Layout &L = c->L;
-    const bool ref = (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) != 0;
-    const int64_t step = c->step;
+__global__ void k_set_counter(long long *d_ctr, long long step) {
+    d_ctr[0] = step;
+    d_ctr[1] = 0;      // block ticket of k_inject
+}
+
+// sensor regime of step n: bit 0 running peak on, bit 1 sum of squares (or phasor) on (reading P8)
+int regime_of(const bvfdtd_ctx *c, int64_t step) {
     const bool in_end = c->opts.sensor_end < 0 || step < c->opts.sensor_end;
+    return (in_end && step >= c->opts.peak_begin ? 1 : 0) | (in_end && step >= c->opts.rms_begin ? 2 : 0);
+}
+// number of steps from `step` on (at most n) that share its regime
+int64_t regime_run(const bvfdtd_ctx *c, int64_t step, int64_t n) {
+    int64_t run = n;
+    for (int64_t edge : {c->opts.peak_begin, c->opts.rms_begin, c->opts.sensor_end})
+        if (edge > step) run = std::min(run, edge - step);
+    return run;
+}
+
+// the cur / nxt copies of the ping-pong arrays for a step that starts with copy `sel` current
+void select_copies(const bvfdtd_ctx *c, Params &p, int sel, bool pingpong) {
+    for (int q = 0; q < 6; ++q) {
+        float *prim = (float *)(c->ws + c->W.field[q]), *alt = (float *)(c->ws + c->W.alt[q]);
+        p.f[q] = sel ? alt : prim;
+        p.icur[q] = sel ? F_ALT + q : q;
+        p.fnxt[q] = pingpong ? (sel ? prim : alt) : p.f[q];
+        p.inxt[q] = pingpong ? (sel ? q : F_ALT + q) : p.icur[q];
+    }
+    float *p7 = (float *)(c->ws + c->W.psi[7]), *p7a = (float *)(c->ws + c->W.psi7_alt);
+    p.psi[7] = sel ? p7a : p7;
+    p.ipsi7_cur = sel ? PSI7_ALT : 1;
+    p.psi7_nxt = pingpong ? (sel ? p7 : p7a) : p.psi[7];
+}
+
+// kernel parameters of step `step` when copy `sel` of the ping-pong arrays is current
+Params step_params(const bvfdtd_ctx *c, int64_t step, int regime, int sel) {
     Params p = c->prm;
-    p.do_peak = in_end && step >= c->opts.peak_begin;
-    p.do_rms = in_end && step >= c->opts.rms_begin;
+    select_copies(c, p, sel, c->ff_active);
+    p.do_peak = regime & 1;
+    p.do_rms = (regime >> 1) & 1;
     p.do_phasor = 0; p.ph_cos = p.ph_sin = 0.0f;
     if (c->opts.flags & BVFDTD_FLAG_PHASOR) {
         // NEXT-3: the window [rms_begin, sensor_end) accumulates the phasor at f0; no peak / rms
@@ -474,40 +628,101 @@ int run_phases(bvfdtd_ctx *c, int phases) {
             p.ph_cos = (float)std::cos(wt); p.ph_sin = (float)std::sin(wt);
         }
     }
+    return p;
+}
+
+// after a step of the fused mode the other copy is current
+void flip_copies(bvfdtd_ctx *c, int64_t steps) {
+    if (!c->ff_active || !(steps & 1)) return;
+    c->sel ^= 1;
+    select_copies(c, c->prm, c->sel, false);
+}
+
+// Enqueue the passes of one step selected by `phases`.  d_ctr != nullptr: the injection takes the step index
+// from the device counter (graph replay); ev != nullptr: five events bracket the four kernels (inject, fused sweep,
+// velocity pass, stress pass).
+int enqueue_passes(bvfdtd_ctx *c, const Params &p, int phases, int64_t step, long long *d_ctr, cudaEvent_t *ev, cudaStream_t st) {
+    const Layout &L = c->L;
+    const bool ref = (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) != 0;
+    if (ev) CU(cudaEventRecord(ev[0], st));
+    if ((phases & PH_INJECT) && c->n_src > 0) {
+        const int tb = 128;
+        k_inject<<<(unsigned)((c->n_src + tb - 1) / tb), tb, 0, st>>>(
+            p, c->n_src, c->d_cell, c->d_amp, c->d_delay, c->waveform, c->f_src, c->n_cycles, c->dt, (long long)step, d_ctr);
+    }
+    if (ev) CU(cudaEventRecord(ev[1], st));
+    const dim3 rb(32, 4, 2), rg((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
+    const bool ff = c->ff_active;       // (only whole steps run in the fused mode: bvfdtd_step_phase leaves it first)
+    if (ff && (phases & PH_VELOCITY)) fused_launch(c->fplan, p, st);
+    if (ev) CU(cudaEventRecord(ev[2], st));
+    if (phases & PH_VELOCITY) {
+        if (ref) k_velocity_ref<<<rg, rb, 0, st>>>(p);
+        else if (tiled_velocity(c->plan, p, st, ff ? c->fplan.items_v : nullptr, c->fplan.n_v)) return cuda_fail(cudaGetLastError(), "tiled_velocity");
+    }
+    if (ev) CU(cudaEventRecord(ev[3], st));
+    if (phases & PH_STRESS) {
+        if (ref) k_stress_ref<<<rg, rb, 0, st>>>(p);
+        else if (tiled_stress(c->plan, p, st, ff ? c->fplan.items_s : nullptr, c->fplan.n_s)) return cuda_fail(cudaGetLastError(), "tiled_stress");
+    }
+    if (ev) CU(cudaEventRecord(ev[4], st));
+    return BVFDTD_OK;
+}
+
+// The passes of step c->step selected by `phases`; the step counter advances with the stress pass.
+int run_phases(bvfdtd_ctx *c, int phases) {
+    const int64_t step = c->step;
+    const Params p = step_params(c, step, regime_of(c, step), c->sel);
     const bool timed = phases == PH_ALL && c->timing && c->timed_steps < BVFDTD_MAX_TIMED_STEPS;
     cudaEvent_t *ev = nullptr;
     if (timed) {
-        if (c->ev.size() < (size_t)(c->timed_steps + 1) * 4) {
-            for (int q = 0; q < 4; ++q) { cudaEvent_t e; CU(cudaEventCreate(&e)); c->ev.push_back(e); }
+        if (c->ev.size() < (size_t)(c->timed_steps + 1) * 5) {
+            for (int q = 0; q < 5; ++q) { cudaEvent_t e; CU(cudaEventCreate(&e)); c->ev.push_back(e); }
         }
-        ev = &c->ev[c->timed_steps * 4];
-        CU(cudaEventRecord(ev[0], c->stream));
+        ev = &c->ev[c->timed_steps * 5];
     }
-    if ((phases & PH_INJECT) && c->n_src > 0) {
-        const int tb = 128;
-        k_inject<<<(unsigned)((c->n_src + tb - 1) / tb), tb, 0, c->stream>>>(
-            p, c->n_src, c->d_cell, c->d_amp, c->d_delay, c->waveform, c->f_src, c->n_cycles,
-            (double)step * c->dt);
-    }
-    if (timed) CU(cudaEventRecord(ev[1], c->stream));
-    const dim3 rb(32, 4, 2), rg((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
-    if (phases & PH_VELOCITY) {
-        if (ref) k_velocity_ref<<<rg, rb, 0, c->stream>>>(p);
-        else if (tiled_velocity(c->plan, p, c->stream)) return cuda_fail(cudaGetLastError(), "tiled_velocity");
-    }
-    if (timed) CU(cudaEventRecord(ev[2], c->stream));
-    if (phases & PH_STRESS) {
-        if (ref) k_stress_ref<<<rg, rb, 0, c->stream>>>(p);
-        else if (tiled_stress(c->plan, p, c->stream)) return cuda_fail(cudaGetLastError(), "tiled_stress");
-    }
-    if (timed) { CU(cudaEventRecord(ev[3], c->stream)); c->timed_steps++; }
+    const int rc = enqueue_passes(c, p, phases, step, nullptr, ev, c->stream);
+    if (rc) return rc;
+    if (timed) c->timed_steps++;
     if (phases & PH_STRESS) {
         if (p.do_rms || p.do_phasor) c->rms_count++;
         c->step++;
         c->phase_done = 0;
+        flip_copies(c, 1);
     } else {
         c->phase_done |= phases;
     }
+    return BVFDTD_OK;
+}
+
+// bvfdtd_step replays CUDA graphs unless the caller asked for per-kernel timing, the phasor sensor is on (its
+// cos / sin change every step) or the context says no (BVFDTD_TUNE_NO_GRAPH)
+bool graph_ok(const bvfdtd_ctx *c) {
+    return !c->timing && !(c->opts.flags & BVFDTD_FLAG_PHASOR) && !(c->opts.tuning & BVFDTD_TUNE_NO_GRAPH);
+}
+
+
+// the graph of `len` (1 or GRAPH_STEPS) consecutive steps in sensor regime `regime`, captured on first use
+int get_graph(bvfdtd_ctx *c, int regime, int len, cudaGraphExec_t *out) {
+    cudaGraphExec_t &slot = c->graph[regime][len == 1 ? 0 : 1][c->sel];
+    if (!slot) {
+        long long *d_ctr = (long long *)(c->ws + c->W.ctr);
+        if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+        CU(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed));
+        int rc = BVFDTD_OK;
+        for (int s = 0; s < len && rc == BVFDTD_OK; ++s) {
+            // (in the fused mode consecutive steps alternate between the two copies of the ping-pong arrays)
+            const Params p = step_params(c, 0, regime, c->ff_active ? (c->sel ^ (s & 1)) : c->sel);
+            rc = enqueue_passes(c, p, PH_ALL, 0, d_ctr, nullptr, c->cap_stream);
+        }
+        cudaGraph_t g = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+        if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+        const cudaError_t e2 = cudaGraphInstantiate(&slot, g, 0);
+        cudaGraphDestroy(g);
+        if (e2 != cudaSuccess) { slot = nullptr; return cuda_fail(e2, "cudaGraphInstantiate"); }
+    }
+    *out = slot;
     return BVFDTD_OK;
 }
 
@@ -516,6 +731,31 @@ int run_phases(bvfdtd_ctx *c, int phases) {
 int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
     if (!c || n < 0) return BVFDTD_EINVAL;
     if (c->phase_done != 0) return BVFDTD_ESTATE;   // a step begun with bvfdtd_step_phase must be finished first
+    DeviceScope scope(c->device);
+    if (n >= 2 && graph_ok(c)) {
+        // one graph launch per GRAPH_STEPS steps (per step for the remainder) instead of three kernel launches
+        // per step: the small grids are launch-bound
+        if (c->n_src > 0) k_set_counter<<<1, 1, 0, c->stream>>>((long long *)(c->ws + c->W.ctr), (long long)c->step);
+        int64_t left = n;
+        while (left > 0) {
+            const int regime = regime_of(c, c->step);
+            int64_t run = regime_run(c, c->step, left);
+            left -= run;
+            while (run > 0) {
+                const int len = run >= bvfdtd_ctx::GRAPH_STEPS ? (int)bvfdtd_ctx::GRAPH_STEPS : 1;
+                cudaGraphExec_t g = nullptr;
+                const int rc = get_graph(c, regime, len, &g);
+                if (rc) return rc;
+                CU(cudaGraphLaunch(g, c->stream));
+                c->step += len;
+                if (regime & 2) c->rms_count += len;
+                flip_copies(c, len);
+                run -= len;
+            }
+        }
+        CU(cudaGetLastError());
+        return BVFDTD_OK;
+    }
     for (int64_t s = 0; s < n; ++s) {
         int rc = run_phases(c, PH_ALL);
         if (rc) return rc;
@@ -526,11 +766,14 @@ int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
 
 int bvfdtd_step_phase(bvfdtd_ctx *c, int32_t phase) {
     if (!c || phase < 0 || phase > 2) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     // the passes of one step run in order: inject (0), velocity (1), stress + sensor (2)
     const int bit = 1 << phase;
     const int before = bit - 1;                       // every earlier pass must have run, this one not
     if ((c->phase_done & before) != before || (c->phase_done & bit)) return BVFDTD_ESTATE;
-    int rc = run_phases(c, bit);
+    int rc = fused_disable(c);          // single passes run on every tile column
+    if (rc) return rc;
+    rc = run_phases(c, bit);
     if (rc) return rc;
     CU(cudaGetLastError());
     return BVFDTD_OK;
@@ -556,12 +799,15 @@ int bvfdtd_kernel_mode(const bvfdtd_ctx *c, uint32_t *mode) {
     if (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) m |= BVFDTD_MODE_REFERENCE;
     else if (c->dense) m |= BVFDTD_MODE_DENSE;
     if (c->sigma_written) m |= BVFDTD_MODE_SIGMA_WRITTEN;
+    if (graph_ok(c)) m |= BVFDTD_MODE_GRAPH;
+    if (c->ff_active) m |= BVFDTD_MODE_FUSED;
     *mode = m;
     return BVFDTD_OK;
 }
 
 int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, int32_t dst_is_device) {
     if (!c || !dst) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     const size_t need = field_bytes(c, id);
     if (need == 0 || dst_bytes != need) return BVFDTD_EINVAL;
     const Layout &L = c->L;
@@ -589,6 +835,11 @@ int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, 
     // r_yy / r_zz are not kept where they equal r_xx (all-fluid lossy tile-planes of the tiled path): fill them in
     if ((id == RYY || id == RZZ) && !c->dense && !(c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS))
         tiled_fill_rii(c->plan, c->prm, c->stream);
+    // ... and sigma_yy / sigma_zz where the fused sweep keeps sigma_xx only
+    if (id == SYY || id == SZZ || id == BVFDTD_F_PRESSURE) {
+        const int rcf = fused_fill(c);
+        if (rcf) return rcf;
+    }
     if (id < NSTATE) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.f[id], c->prm);
     else if (id == BVFDTD_F_SUMSQ) k_unpack<<<g, b, 0, c->stream>>>((float *)target, c->prm.sumsq, c->prm);
     else if (id == BVFDTD_F_PRESSURE) k_pressure<<<g, b, 0, c->stream>>>((float *)target, c->prm);
@@ -600,8 +851,15 @@ int bvfdtd_read_fields(bvfdtd_ctx *c, uint32_t id, void *dst, size_t dst_bytes, 
 
 int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_bytes, int32_t src_is_device) {
     if (!c || !src || id >= NSTATE) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     if (src_bytes != field_bytes(c, id)) return BVFDTD_EINVAL;
     const float *d_src = (const float *)src;
+    if (id >= SXX) {
+        // a caller-supplied stress or memory variable ends the fused mode (it relies on sigma_xx = sigma_yy =
+        // sigma_zz, r_xx = r_yy = r_zz and zero shear stresses in its tile columns)
+        const int rcf = fused_disable(c);
+        if (rcf) return rcf;
+    }
     if (!src_is_device) {
         float *scratch = (float *)(c->ws + c->W.scratch);
         CU(cudaMemcpyAsync(scratch, src, src_bytes, cudaMemcpyHostToDevice, c->stream));
@@ -631,6 +889,7 @@ int bvfdtd_write_fields(bvfdtd_ctx *c, uint32_t id, const void *src, size_t src_
 
 int bvfdtd_read_peak_pressure(bvfdtd_ctx *c, float *peak, float *rms_amp, int32_t dst_is_device) {
     if (!c) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     const Layout &L = c->L;
     const size_t bytes = (size_t)L.nx * L.ny * L.nz * 4;
     float *scratch = (float *)(c->ws + c->W.scratch);
@@ -654,6 +913,7 @@ int bvfdtd_read_peak_pressure(bvfdtd_ctx *c, float *peak, float *rms_amp, int32_
 
 int bvfdtd_read_phasor(bvfdtd_ctx *c, float *re, float *im, int32_t dst_is_device) {
     if (!c || !re || !im) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     if (!(c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
     const Layout &L = c->L;
     const size_t bytes = (size_t)L.nx * L.ny * L.nz * 4;
@@ -672,6 +932,7 @@ int bvfdtd_read_phasor(bvfdtd_ctx *c, float *re, float *im, int32_t dst_is_devic
 
 int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) {
     if (!c || !plane_sum || !plane_max) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     if (c->rms_count <= 0 || (c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
     const Layout &L = c->L;
     double *d_out = (double *)(c->ws + c->W.scratch);          // 2 nz doubles of the dense scratch plane
@@ -687,6 +948,7 @@ int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) 
 
 int bvfdtd_heat_source(bvfdtd_ctx *c, const double *absorbed_fraction, double scale, float *Q) {
     if (!c || !absorbed_fraction || !Q || !(scale >= 0.0) || !std::isfinite(scale)) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     if (c->rms_count <= 0 || (c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
     // Q = scale a 2 alphaL I,  I = p_amp^2 / (2 rho cL) = sumsq / (count rho cL): one fp32 factor per material
     float coef[256];
@@ -732,6 +994,7 @@ int bvfdtd_refocus_weights(int64_t n_pts, const float *p_re, const float *p_im, 
     if (n_pts <= 0 || n_pts > (1 << 30) || n_elem <= 0 || n_elem > 65535 || !p_re || !p_im || !element || !area || !w_pts || !delay_s)
         return BVFDTD_EINVAL;
     if (!(f > 0.0) || !std::isfinite(u0)) return BVFDTD_EINVAL;
+    DeviceScope scope(device_of(p_re));      // the caller's arrays say which device the launch belongs to
     cudaStream_t st = (cudaStream_t)cuda_stream;
     float2 *d_unit = nullptr;
     int *d_bad = nullptr;
@@ -758,6 +1021,7 @@ int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight
     if (n_src <= 0 || n_rcv <= 0 || n_src > (1 << 30) || n_rcv > (1 << 30) || !src_xyz || !src_weight || !rcv_xyz || !p_re || !p_im)
         return BVFDTD_EINVAL;
     if (!(f > 0.0) || !(c0 > 0.0) || !(rho0 > 0.0) || (amp == nullptr) != (delay_s == nullptr)) return BVFDTD_EINVAL;
+    DeviceScope scope(device_of(p_re));      // the caller's arrays say which device the launch belongs to
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const double w = 2.0 * 3.14159265358979323846 * f, k = w / c0;
     // pack the sources as float4 (x, y, z, 0) on the device
@@ -779,13 +1043,14 @@ int bvfdtd_enable_kernel_timing(bvfdtd_ctx *c, int32_t on) {
     return BVFDTD_OK;
 }
 
-int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[3], int64_t launches[3]) {
+int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[4], int64_t launches[4]) {
     if (!c || !ms || !launches) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     CU(cudaStreamSynchronize(c->stream));
-    for (int q = 0; q < 3; ++q) { ms[q] = 0.0; launches[q] = 0; }
+    for (int q = 0; q < 4; ++q) { ms[q] = 0.0; launches[q] = 0; }
     for (int64_t s = 0; s < c->timed_steps; ++s) {
-        cudaEvent_t *ev = &c->ev[s * 4];
-        for (int q = 0; q < 3; ++q) {
+        cudaEvent_t *ev = &c->ev[s * 5];
+        for (int q = 0; q < 4; ++q) {
             float t = 0.0f;
             CU(cudaEventElapsedTime(&t, ev[q], ev[q + 1]));
             ms[q] += t;
@@ -793,17 +1058,31 @@ int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[3], int64_t launches[3]) {
         }
     }
     if (c->n_src == 0) { ms[0] = 0.0; launches[0] = 0; }
+    if (!c->ff_active || c->fplan.n_f == 0) { ms[1] = 0.0; launches[1] = 0; }
+    if (c->ff_active && c->fplan.n_v == 0) { ms[2] = 0.0; launches[2] = 0; }
+    if (c->ff_active && c->fplan.n_s == 0) { ms[3] = 0.0; launches[3] = 0; }
     c->timed_steps = 0;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_fused_coverage(const bvfdtd_ctx *c, int64_t *planes_fused, int64_t *planes_all) {
+    if (!c || !planes_fused || !planes_all) return BVFDTD_EINVAL;
+    *planes_fused = c->ff_active ? c->fplan.planes_f : 0;
+    *planes_all = (int64_t)c->L.ntxV * c->L.ntyV * c->L.nz;
     return BVFDTD_OK;
 }
 
 int bvfdtd_destroy(bvfdtd_ctx *c) {
     if (!c) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
     cudaStreamSynchronize(c->stream);
-    if (c->d_cell) { cudaFree(c->d_cell); cudaFree(c->d_amp); cudaFree(c->d_delay); }
+    drop_graphs(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->src_own) cudaFree(c->src_own);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     tiled_plan_destroy(c->plan);
     delete c;
+    (void)cudaGetLastError();
     return BVFDTD_OK;
 }
 

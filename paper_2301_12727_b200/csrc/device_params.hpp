@@ -51,6 +51,16 @@ struct Params {
     float ph_cos, ph_sin;  // cos / sin of w0 (n + 1) dt for this step
     // tile-class flags: one word per (tile, plane + 2), planes -2..nz+1
     const uint32_t *flagsV, *flagsS;
+    // Ping-pong of the arrays the fused fluid sweep reads with a halo while other CTAs of the same launch write
+    // them (vx, vy, vz, sigma_xx, sigma_yy, sigma_zz and the y-psi of D+y sigma_yy): every kernel of a step reads
+    // the time level it starts from in the "cur" copy and writes its results to the "nxt" copy; the host swaps
+    // the two after the step.  f[0..5] and psi[7] always name the cur copies.  Without the fused sweep
+    // cur == nxt and the passes work in place, as before.
+    int icur[6], inxt[6];     // array index of VX..SZZ inside the 4-D field tensor map
+    float *fnxt[6];           // where the step writes VX..SZZ
+    int ipsi7_cur;            // array index of psi[7] inside the y-psi tensor map (1, or 6 for the alternate)
+    float *psi7_nxt;
+    const uint32_t *flagsF;   // fused sweep: one word per (64 x 8 tile, plane + 2)
 };
 
 // tile-class flag bits
@@ -63,6 +73,15 @@ enum : uint32_t {
                      // halo-extended tile-plane is a fluid, so sigma_xx = sigma_yy = sigma_zz there and one array serves
     TF_SOLID = 16u,  // stress: some cell of the tile-plane is a solid (else eS = bS = 0 and r_xx = r_yy = r_zz)
     // velocity: the same three bits, taken over the halo-extended region the pass reads
+};
+
+// fused-sweep flag bits (flagsF; kernels_fused.cuh)
+enum : uint32_t {
+    FF_FLUID4 = 1u,   // S0: no solid cell within 4 cells (x, y) of the 64 x 8 tile in this plane
+    FF_LOSSY = 2u,    // S0: some cell of the tile-plane is lossy (r_xx moves)
+    FF_RUN = 4u,      // host: the plane belongs to a run of the fused sweep
+    FF_WYY = 8u,      // host: a y-neighbour tile runs the two passes here and reads sigma_yy: write it too
+    FF_WZZ = 16u      // host: a plane within reach of the z stencil runs the two passes: write sigma_zz too
 };
 
 }  // namespace bvfdtd

@@ -55,10 +55,9 @@ __device__ __forceinline__ float pml_term(const Params &p, const SlabIdx &s, int
     return cpml(d, p.psi[axis * 6 + term], s.q[axis], a, b);
 }
 
-// S1 (reading P7): additive isotropic stress injection at t_n = n dt
-__global__ void k_inject(Params p, long long n_src, const long long *__restrict__ cell,
-                         const float *__restrict__ amp, const float *__restrict__ delay,
-                         int waveform, double f_src, int n_cycles, double t_n) {
+__device__ __forceinline__ void inject_cells(const Params &p, long long n_src, const long long *__restrict__ cell,
+                                             const float *__restrict__ amp, const float *__restrict__ delay,
+                                             int waveform, double f_src, int n_cycles, double t_n) {
     const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (s >= n_src) return;
     const double t = t_n - (double)delay[s];
@@ -79,6 +78,33 @@ __global__ void k_inject(Params p, long long n_src, const long long *__restrict_
     p.f[SXX][c] -= add;
     p.f[SYY][c] -= add;
     p.f[SZZ][c] -= add;
+}
+
+// S1 (reading P7): additive isotropic stress injection at t_n = n dt.
+// The step index n is the host's `step`, or -- when the step is replayed from a CUDA graph, whose kernel
+// arguments are frozen -- the device counter d_ctr[0], which the last block to finish advances by one
+// (every block has read the counter before it can finish, so the update races with no reader).
+__global__ void k_inject(Params p, long long n_src, const long long *__restrict__ cell,
+                         const float *__restrict__ amp, const float *__restrict__ delay,
+                         int waveform, double f_src, int n_cycles, double dt, long long step, long long *d_ctr) {
+    if (d_ctr) {
+        __shared__ long long s_step;
+        if (threadIdx.x == 0) s_step = *reinterpret_cast<volatile long long *>(d_ctr);
+        __syncthreads();
+        step = s_step;
+    }
+    inject_cells(p, n_src, cell, amp, delay, waveform, f_src, n_cycles, (double)step * dt);
+    if (d_ctr) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            unsigned int *done = reinterpret_cast<unsigned int *>(d_ctr + 1);
+            if (atomicAdd(done, 1u) == gridDim.x - 1) {
+                *done = 0u;
+                *reinterpret_cast<volatile long long *>(d_ctr) = step + 1;
+            }
+        }
+    }
 }
 
 // S2 (Eq. 1 rows 1-3; readings P1, P2, P4, P5)

@@ -107,12 +107,16 @@ struct TiledPlan {
     StagePlan sv, ss;
     StagePlan svc{};       // compact velocity stage plan (ns = 0: unused), see k_velocity_tiled
     int occ_v = 2;         // register budget of the velocity instantiation in use (2 or 3 resident CTAs)
+    int occ_v_res = 1, occ_s_res = 1;   // resident CTAs per SM the occupancy query reports for the two passes
     bool s16 = true;       // stress pass runs 64 x 16 tiles (else 64 x 8)
     ZChunks zv, zs;        // z chunks of the velocity / stress launch
     bool ready = false;
 };
 
-enum { F_PEAK = NSTATE, F_SUMSQ = NSTATE + 1, F_PHRE = NSTATE + 2, F_PHIM = NSTATE + 3, NGRID = NSTATE + 4 };
+enum { F_PEAK = NSTATE, F_SUMSQ = NSTATE + 1, F_PHRE = NSTATE + 2, F_PHIM = NSTATE + 3, NGRID = NSTATE + 4,
+       F_ALT = NGRID,            // alternates of VX..SZZ (ping-pong of the fused sweep, device_params.hpp)
+       NGRID_ALL = NGRID + 6 };
+enum { PSI7_ALT = 6 };          // array index of the alternate of psi[7] inside the y-psi block
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers: mbarrier + TMA
@@ -386,14 +390,14 @@ struct VelIssue {
         // all-fluid extended tile: sigma_xx = sigma_yy = sigma_zz bit for bit (eS = 0, isotropic source, zero
         // start), so ONE box of sigma_xx with both halos (rows j-1 .. j+9, in the idle sxy slot) serves D+x,
         // D+y and D+z instead of the three boxes
-        if (c & VC_FL) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 1, z, SXX);
-        else t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, SZZ);
+        if (c & VC_FL) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 1, z, p->icur[SXX]);
+        else t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, p->icur[SZZ]);
         if (xz) t.box4(VS::SXZ, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXZ);
         if (yz) t.box4(VS::SYZ, C::B_BYTES, &maps->boxB, x0, y0 - 2, z, SYZ);
         if (c & VC_IN0) {
             if (!(c & VC_FL)) {
-                t.box4(VS::SXX, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXX);
-                t.box4(VS::SYY, C::B_BYTES, &maps->boxB, x0, y0 - 1, z, SYY);
+                t.box4(VS::SXX, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, p->icur[SXX]);
+                t.box4(VS::SYY, C::B_BYTES, &maps->boxB, x0, y0 - 1, z, p->icur[SYY]);
             }
             if (xy) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, SXY);
             // psi of the x-y derivatives of plane m: x terms 0..2, y terms 0..2
@@ -406,14 +410,14 @@ struct VelIssue {
                     if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, q);
                     if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, q);
                 }
-                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, q);
+                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, q == 1 ? p->ipsi7_cur : q);
             }
         }
         if (c & VC_IN1) {
-            t.box4(VS::VXO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, VX);
-            t.box4(VS::VYO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, VY);
+            t.box4(VS::VXO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VX]);
+            t.box4(VS::VYO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VY]);
         }
-        if (c & VC_IN2) t.box4(VS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, VZ);
+        if (c & VC_IN2) t.box4(VS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, p->icur[VZ]);
         if (c & VC_ZS1) {
             const int kc = z_compact(*p, m - 1);
             if (c & VC_WXZ) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, kc, 0);
@@ -505,8 +509,8 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
                     if (wall_y) oy = zero;
                 }
                 const uint32_t gq = goff - (uint32_t)p.sz;
-                q_store<EDGE>(p.f[VX] + gq, ox, g.nv);
-                q_store<EDGE>(p.f[VY] + gq, oy, g.nv);
+                q_store<EDGE>(p.fnxt[VX] + gq, ox, g.nv);
+                q_store<EDGE>(p.fnxt[VY] + gq, oy, g.nv);
             }
             if (ctrl & VC_IN2) {
                 // finish vz at plane m-2
@@ -518,7 +522,7 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
                                      dt2 * rcp_newton(rho_prev[2] + rho_j[2]), dt2 * rcp_newton(rho_prev[3] + rho_j[3]));
                 Q4 oz = q_fma(cz, q_add(pvz2, dzz), q_ld(reinterpret_cast<const float *>(st + VS::VZO) + qoff));
                 if (m - 2 == p.nz - 1) oz = zero;
-                q_store<EDGE>(p.f[VZ] + (goff - 2u * (uint32_t)p.sz), oz, g.nv);
+                q_store<EDGE>(p.fnxt[VZ] + (goff - 2u * (uint32_t)p.sz), oz, g.nv);
             }
             pvz2 = pvz1;
 #pragma unroll
@@ -556,7 +560,7 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
                     const float *ps = reinterpret_cast<const float *>(st + sp.psy) + qoff;
                     const Q4 ai = q_set(g.ay_i), bi = q_set(g.by_i);
                     if (ctrl & VC_XY) q_store<EDGE>(p.psi[6] + gyo, q_cpml(dxy_y, q_ld(ps), ai, bi), g.nv);
-                    q_store<EDGE>(p.psi[7] + gyo, q_cpml(dyy, q_ld(ps + DQ), q_set(g.ay_h), q_set(g.by_h)), g.nv);
+                    q_store<EDGE>(p.psi7_nxt + gyo, q_cpml(dyy, q_ld(ps + DQ), q_set(g.ay_h), q_set(g.by_h)), g.nv);
                     if (ctrl & VC_YZ) q_store<EDGE>(p.psi[8] + gyo, q_cpml(dyz, q_ld(ps + 2 * DQ), ai, bi), g.nv);
                 }
                 pvx = q_add(dxx, dxy_y);
@@ -585,12 +589,17 @@ __device__ __forceinline__ void velocity_consume(const Params &p, const StagePla
 // strides (2 % faster on config 2).
 template <class C, int OCC, bool TRIM>
 __global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_constant__ TiledMaps maps, const Params p,
-                                                               const ZChunks zc, const StagePlan spf, const StagePlan spc) {
+                                                               const ZChunks zc, const StagePlan spf, const StagePlan spc,
+                                                               const int4 *__restrict__ items) {
     using VS = VStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
+    // a block is (tile, z chunk) of the launch grid, or -- with a work list (the tile columns the fused sweep does
+    // not take) -- item blockIdx.x = (tile x, tile y, first plane, one past the last plane)
+    int bx = blockIdx.x, by = blockIdx.y, kz0, kz1;
+    if (items) { const int4 it = __ldg(items + blockIdx.x); bx = it.x; by = it.y; kz0 = it.z; kz1 = it.w; }
+    else { kz0 = zc.b[blockIdx.z]; kz1 = zc.b[blockIdx.z + 1]; }
+    const int x0 = bx * C::TX, y0 = by * C::TY;
     const int m_begin = kz0 - 2, m_end = kz1 + 2;   // iterations m in [m_begin, m_end)
     // (a compact plan without x-psi slots, spc.xt == 0, also needs a tile outside the x slabs)
     const bool x_slab = p.P > 0 && (x0 < p.P || (x0 + C::TX > p.xhb && x0 < p.nx));
@@ -616,7 +625,7 @@ __global__ void __launch_bounds__(C::NT, OCC) k_velocity_tiled(const __grid_cons
     if (tid >= C::NC) {
         // ================= producer warp =================
         if (tid == C::NC) {
-            const uint32_t *flags = p.flagsV + (size_t)(blockIdx.x + p.ntxV * blockIdx.y) * (p.nz + 4) + 2;
+            const uint32_t *flags = p.flagsV + (size_t)(bx + p.ntxV * by) * (p.nz + 4) + 2;
             VelIssue<C> iss;
             iss.maps = &maps; iss.p = &p; iss.sp = &sp;
             iss.tX = make_tilex<C>(p, x0); iss.tY = tile_in_y<C>(p, y0); iss.jy0 = tile_jy0<C>(p, y0);
@@ -712,9 +721,9 @@ struct StrIssue {
         const uint32_t c = ctrl(m, hist);
         const uint32_t xbox = (uint32_t)sp->wxb * C::TY * 4;
         const int z = m + 2;
-        t.box4(SS::VXB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VX);
-        t.box4(SS::VYB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VY);
-        t.box4(SS::VZB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, VZ);
+        t.box4(SS::VXB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, p->inxt[VX]);
+        t.box4(SS::VYB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, p->inxt[VY]);
+        t.box4(SS::VZB, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 2, z, p->inxt[VZ]);
         if (c & SC_IN0) {
             // psi of the x-y derivatives of plane m: x terms 3 (D-x vx), 4 (D+x vy), 5 (D+x vz);
             // y terms 3 (D+y vx), 4 (D-y vy), 5 (D+y vz)
@@ -736,7 +745,7 @@ struct StrIssue {
         }
         if (c & SC_IN1) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) t.box4(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, SXX + q);
+            for (int q = 0; q < 3; ++q) t.box4(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[SXX + q]);
             if (c & SC_RII1) {
                 t.box4(SS::RII, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX);
                 if (!(c & SC_RFL1)) {
@@ -841,7 +850,7 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
 #pragma unroll
                     for (int q = 0; q < 3; ++q) {
                         const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), inc);
-                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        q_store<EDGE>(p.fnxt[SXX + q] + gq, sn, g.nv);
                         tr = q_add(tr, sn);
                     }
                 } else if (ctrl & SC_RII1) {
@@ -855,7 +864,7 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
                         const Q4 rold = q_ld(dbase + SS::RII / 4 + q * DQ);
                         const Q4 rn = q_sub(q_muls(rold, A), eR);
                         const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), q_fmas(hdt, q_add(rn, rold), eU));
-                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        q_store<EDGE>(p.fnxt[SXX + q] + gq, sn, g.nv);
                         q_store<EDGE>(p.f[RXX + q] + gq, rn, g.nv);
                         tr = q_add(tr, sn);
                     }
@@ -864,7 +873,7 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
                     for (int q = 0; q < 3; ++q) {
                         const Q4 eU = q_fnma(eS, q_sub(th, vii[q]), ePth);
                         const Q4 sn = q_add(q_ld(dbase + SS::SII / 4 + q * DQ), eU);
-                        q_store<EDGE>(p.f[SXX + q] + gq, sn, g.nv);
+                        q_store<EDGE>(p.fnxt[SXX + q] + gq, sn, g.nv);
                         tr = q_add(tr, sn);
                     }
                 }
@@ -972,7 +981,7 @@ __device__ __forceinline__ void stress_consume(const Params &p, const StagePlan 
 
 template <class C>
 __global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(const __grid_constant__ TiledMaps maps, const Params p,
-                                                           const ZChunks zc, const StagePlan sp) {
+                                                           const ZChunks zc, const StagePlan sp, const int4 *__restrict__ items) {
     using SS = SStage<C>;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *stages = smem;
@@ -986,8 +995,10 @@ __global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(con
     uint64_t *empty = full + MAX_STAGES;
 
     const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY;
-    const int kz0 = zc.b[blockIdx.z], kz1 = zc.b[blockIdx.z + 1];
+    int bx = blockIdx.x, by = blockIdx.y, kz0, kz1;      // (tile, z chunk) of the grid, or an item of the work list
+    if (items) { const int4 it = __ldg(items + blockIdx.x); bx = it.x; by = it.y; kz0 = it.z; kz1 = it.w; }
+    else { kz0 = zc.b[blockIdx.z]; kz1 = zc.b[blockIdx.z + 1]; }
+    const int x0 = bx * C::TX, y0 = by * C::TY;
     const int m_begin = kz0 - 2, m_end = kz1 + 2;
 
     for (int q = tid; q < NM; q += C::NT) {
@@ -1006,7 +1017,7 @@ __global__ void __launch_bounds__(C::NT, C::TY >= 16 ? 1 : 2) k_stress_tiled(con
     if (tid >= C::NC) {
         // ================= producer warp =================
         if (tid == C::NC) {
-            const uint32_t *flags = p.flagsS + (size_t)(blockIdx.x + p.ntxS * blockIdx.y) * (p.nz + 4) + 2;
+            const uint32_t *flags = p.flagsS + (size_t)(bx + p.ntxS * by) * (p.nz + 4) + 2;
             StrIssue<C> iss;
             iss.maps = &maps; iss.p = &p; iss.sp = &sp;
             iss.tX = make_tilex<C>(p, x0); iss.tY = tile_in_y<C>(p, y0); iss.jy0 = tile_jy0<C>(p, y0);
@@ -1163,7 +1174,7 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
     const long long fstride = (const char *)p.f[1] - (const char *)p.f[0];
     {
         void *base = (void *)(p.f[0] + (L.org - 2 * L.sz));      // cell (0,0,-2)
-        const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), (cuuint64_t)NGRID};
+        const cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 4), (cuuint64_t)NGRID_ALL};
         const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
         struct { CUtensorMap *m; cuuint32_t bx, by; } boxes[4] = {
             {&maps.boxA, (cuuint32_t)C::AX, (cuuint32_t)C::TY}, {&maps.boxB, (cuuint32_t)C::TX, (cuuint32_t)C::BY},
@@ -1187,7 +1198,7 @@ inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, co
             if (int rc = encode(&maps.psx, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[0], d, s, b, "psi x box")) return rc;
         }
         {   // y slabs: (px, 2P, nz, 6)
-            const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)(2 * L.P), (cuuint64_t)L.nz, 6};
+            const cuuint64_t d[4] = {(cuuint64_t)L.px, (cuuint64_t)(2 * L.P), (cuuint64_t)L.nz, 7};   // 6 terms + the alternate of psi[7]
             const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * 2 * L.P * 4, (cuuint64_t)psi_stride[1]};
             const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::TY, 1, 1};
             if (int rc = encode(&maps.psy, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_base[1], d, s, b, "psi y box")) return rc;
@@ -1226,7 +1237,24 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
     return s;
 }
 
-inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const psi_base[3], const long long psi_stride[3], bool dense) {
+// launch-plan requests (bvfdtd_opts.tuning; 0 = the library's own choice).  The library reads no environment
+// variable; a build with -DBVFDTD_DEV_KNOBS additionally honours BVFDTD_NS_V / _NS_S / _WAVES / _ZB_V / _ZB_S /
+// _VERBOSE for experiments.
+struct PlanTuning {
+    int occ_v = 0;      // 0 auto, 2 or 3 resident CTAs of the velocity pass
+    int stress_ty = 0;  // 0 auto, 8 or 16 rows per stress tile
+};
+inline const char *dev_knob(const char *name) {
+#ifdef BVFDTD_DEV_KNOBS
+    return std::getenv(name);
+#else
+    (void)name;
+    return nullptr;
+#endif
+}
+
+inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const psi_base[3], const long long psi_stride[3], bool dense,
+                             const PlanTuning &tune = PlanTuning{}) {
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -1252,7 +1280,7 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const char *env_v = std::getenv("BVFDTD_NS_V"), *env_s = std::getenv("BVFDTD_NS_S"), *env_ty = std::getenv("BVFDTD_STRESS_TY");
+    const char *env_v = dev_knob("BVFDTD_NS_V"), *env_s = dev_knob("BVFDTD_NS_S");
     int ns_v = env_v ? std::atoi(env_v) : 3, ns_s = env_s ? std::atoi(env_s) : 0;
     ns_v = std::max(2, std::min(MAX_STAGES, ns_v));
     const int v_extra = 256 * 4 + 4 * CfgV::TX * 4 + bar_bytes;
@@ -1264,8 +1292,7 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     //   THREE resident CTAs per SM (124 registers): 3 stages where the CTA needs no y- / z-psi slots
     //   (compact plan), 2 stages elsewhere;  needs 3 (smem + 1 KB) <= 228 KB;
     //   two resident CTAs (141 registers), up to 3 stages (thick PMLs).
-    const char *env_occ = std::getenv("BVFDTD_OCC_V");
-    const int occ_req = env_occ ? std::atoi(env_occ) : 0;
+    const int occ_req = tune.occ_v;
     plan.svc = StagePlan{};
     plan.occ_v = 2;
     // (the dense sweep fills every stage and is bandwidth-bound: it measured better with 2 x 3 stages; small
@@ -1311,7 +1338,7 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     const int nm = (p.n_mat + 31) & ~31;
     auto s_extra16 = [&](int ns) { return (ns + 2) * CfgS::M_BYTES + nm * 24 + 4 * CfgS::TX * 4 + bar_bytes; };
     auto s_extra8 = [&](int ns) { return (ns + 2) * CfgS8::M_BYTES + nm * 24 + 4 * CfgS8::TX * 4 + bar_bytes; };
-    const int ty_req = env_ty ? std::atoi(env_ty) : 0;
+    const int ty_req = tune.stress_ty;
     bool chosen = false;
     // (the dense sweep, whose every iteration fills the whole stage, measured better on the 64 x 16 tile)
     if (ty_req != 16 && (!ns_s || ns_s == 2) && !(dense && ty_req != 8)) {
@@ -1364,7 +1391,8 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
         (void)cudaGetLastError();
         return BVFDTD_ECUDA;
     }
-    const char *env_w = std::getenv("BVFDTD_WAVES");
+    plan.occ_v_res = occ_v; plan.occ_s_res = occ_s;
+    const char *env_w = dev_knob("BVFDTD_WAVES");
     const double waves = env_w ? std::atof(env_w) : 2.6;
     plan.zv = plan_chunks(L.nz, (long long)L.ntxV * L.ntyV, (long long)std::max(1, occ_v) * sms, waves);
     if (plan.svc.ns > 0 && L.P >= 8 && L.nz - 2 * L.P >= 16) {
@@ -1382,9 +1410,9 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
         }
     }
     plan.zs = plan_chunks(L.nz, (long long)L.ntxS * L.ntyS, (long long)std::max(1, occ_s) * sms, waves);
-    parse_chunks(std::getenv("BVFDTD_ZB_V"), L.nz, plan.zv);
-    parse_chunks(std::getenv("BVFDTD_ZB_S"), L.nz, plan.zs);
-    if (std::getenv("BVFDTD_VERBOSE")) {
+    parse_chunks(dev_knob("BVFDTD_ZB_V"), L.nz, plan.zv);
+    parse_chunks(dev_knob("BVFDTD_ZB_S"), L.nz, plan.zs);
+    if (dev_knob("BVFDTD_VERBOSE")) {
         std::fprintf(stderr, "[bvfdtd] velocity: ns %d (compact %d) stage %d smem %d occ %d; stress: tile 64x%d ns %d stage %d smem %d occ %d\n[bvfdtd] z chunks velocity:",
                      plan.sv.ns, plan.svc.ns, plan.sv.bytes, plan.sv.smem, occ_v, plan.s16 ? 16 : 8, plan.ss.ns, plan.ss.bytes, plan.ss.smem, occ_s);
         for (int c = 0; c < plan.zv.n; ++c) std::fprintf(stderr, " %d", plan.zv.b[c + 1] - plan.zv.b[c]);
@@ -1420,17 +1448,21 @@ inline void tiled_flags(const TiledPlan &plan, const Params &p, uint32_t *flagsV
     if (plan.s16) k_tile_flags<CfgS><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0, 0);
     else k_tile_flags<CfgS8><<<dim3(p.ntxS, p.ntyS, p.nz), 128, 0, st>>>(p, flagsS, p.ntxS, 1, dense ? 1 : 0, 0);
 }
-inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    const dim3 grid(p.ntxV, p.ntyV, plan.zv.n);
+// items != nullptr: a work list of n_items (tile, z range) entries replaces the (tiles) x (chunks) grid
+inline int tiled_velocity(TiledPlan &plan, const Params &p, cudaStream_t st, const int4 *items = nullptr, int n_items = 0) {
+    if (items && n_items == 0) return 0;
+    const dim3 grid = items ? dim3(n_items) : dim3(p.ntxV, p.ntyV, plan.zv.n);
     if (plan.occ_v == 3 && (plan.sv.spw > 0 || plan.sv.nrho > 0))
-        k_velocity_tiled<CfgV, 3, true><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
-    else if (plan.occ_v == 3) k_velocity_tiled<CfgV, 3, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
-    else k_velocity_tiled<CfgV, 2, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc);
+        k_velocity_tiled<CfgV, 3, true><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc, items);
+    else if (plan.occ_v == 3) k_velocity_tiled<CfgV, 3, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc, items);
+    else k_velocity_tiled<CfgV, 2, false><<<grid, CfgV::NT, plan.sv.smem, st>>>(plan.mv, p, plan.zv, plan.sv, plan.svc, items);
     return 0;
 }
-inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st) {
-    if (plan.s16) k_stress_tiled<CfgS><<<dim3(p.ntxS, p.ntyS, plan.zs.n), CfgS::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss);
-    else k_stress_tiled<CfgS8><<<dim3(p.ntxS, p.ntyS, plan.zs.n), CfgS8::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss);
+inline int tiled_stress(TiledPlan &plan, const Params &p, cudaStream_t st, const int4 *items = nullptr, int n_items = 0) {
+    if (items && n_items == 0) return 0;
+    const dim3 grid = items ? dim3(n_items) : dim3(p.ntxS, p.ntyS, plan.zs.n);
+    if (plan.s16) k_stress_tiled<CfgS><<<grid, CfgS::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss, items);
+    else k_stress_tiled<CfgS8><<<grid, CfgS8::NT, plan.ss.smem, st>>>(plan.ms, p, plan.zs, plan.ss, items);
     return 0;
 }
 

@@ -414,6 +414,44 @@ def blocky_domain(nx, ny, nz, pml, seed, steps=20, waveform=1, f0=500e3, dx=1e-3
                     n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
 
 
+def fluid_domain(nx, ny, nz, pml, seed, steps=40, waveform=1, f0=500e3, dx=1e-3 / 3.0, solid_boxes=2) -> Workload:
+    """Mostly fluid: lossless water with blobs of three other fluids (two lossy, different densities and speeds)
+    and a few solid boxes well inside the grid.  Most 64 x 8 tile columns have no solid cell within reach of
+    their stencils over long z runs -- the layout on which the fused single sweep (kernels_fused.cuh) takes
+    over from the two passes -- next to tile columns, and z ranges, that keep the two passes."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 5000 + seed))
+    table = np.array([WATER,
+                      (1040.0, 1546.0, 0.0, 30.0, 0.0),           # lossy fluid (brain-like)
+                      (920.0, 1450.0, 0.0, 0.0, 0.0),             # lossless light fluid
+                      (1100.0, 1600.0, 0.0, 60.0, 0.0),           # lossy heavy fluid
+                      (1900.0, 2800.0, 1500.0, 200.0, 200.0),     # lossy solid
+                      (1700.0, 2500.0, 1300.0, 0.0, 0.0)], dtype=np.float64)
+    dt, spp = snapped_dt(dx, f0, table[:, 1].max())
+    idx = np.zeros((nz, ny, nx), dtype=np.uint8)
+    dims = np.array([nz, ny, nx])
+    for b in range(8):
+        lo = np.array([rng.integers(0, max(1, d - 4)) for d in dims])
+        ext = np.array([rng.integers(3, max(4, d // 2)) for d in dims])
+        hi = np.minimum(dims, lo + ext)
+        idx[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] = 1 + b % 3
+    for b in range(solid_boxes):
+        lo = np.array([rng.integers(d // 4, max(d // 4 + 1, d // 2)) for d in dims])
+        ext = np.array([rng.integers(3, max(4, d // 5)) for d in dims])
+        hi = np.minimum(dims, lo + ext)
+        idx[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] = 4 + b % 2
+    lo = pml
+    n = 10
+    ci = rng.integers(lo, nx - lo, size=n)
+    cj = rng.integers(lo, ny - lo, size=n)
+    ck = rng.integers(lo, nz - lo, size=n)
+    cells = np.unique((ci + nx * (cj + ny * ck)).astype(np.int64))
+    amp = (0.5 + rng.random(cells.size)).astype(np.float32)
+    delay = (rng.random(cells.size) * 0.5 / f0).astype(np.float32)
+    return Workload(f"fluid_{nx}x{ny}x{nz}_p{pml}_s{seed}", nx, ny, nz, pml, dx, dt, f0, spp,
+                    steps, table, idx, cells, amp, delay, waveform=waveform, f_src=f0,
+                    n_cycles=3, peak_begin=0, rms_begin=max(0, steps // 2))
+
+
 # ----------------------------------------------------------------------------------------
 # transducer surface decompositions (inputs of the Rayleigh-Sommerfeld step, PAPER.md:L95)
 # ----------------------------------------------------------------------------------------

@@ -120,11 +120,11 @@ def test_invalid_rows_rejected(bv):
 
 
 def test_workspace_bytes(bv):
-    # 19 grid arrays (15 state, peak, sumsq, 2 phasor accumulators) + a dense scratch plane + the
-    # index map; padding and PML overhead below 25 % at config 2 size
+    # 25 grid arrays (15 state, peak, sumsq, 2 phasor accumulators, the 6 ping-pong copies of the fused sweep)
+    # + a dense scratch plane + the index map; padding and PML overhead below 25 % at config 2 size
     nx, ny, nz, P = 300, 300, 450, 16
     n = bv.workspace_bytes(nx, ny, nz, P)
-    dense = nx * ny * nz * (20 * 4 + 1)
+    dense = nx * ny * nz * (26 * 4 + 1)
     assert dense < n < 1.25 * dense
     with pytest.raises(bv.BvfdtdError):
         bv.workspace_bytes(20, 64, 64, 8)        # dim < 2*pml + 8
@@ -139,3 +139,37 @@ def test_no_gpu_means_loud_failure(bv):
     w = wl.make(0)
     with pytest.raises(RuntimeError):
         bv.Simulation.from_workload(w)
+
+
+def test_tuning_bits_validated_before_any_device_call(bv):
+    """bvfdtd_opts.tuning: unknown bits and contradictory requests are BVFDTD_EINVAL (checked with the other
+    argument rules, before the library touches CUDA)."""
+    import ctypes as C
+    w = wl.make(0)
+    g = bv.Grid(w.nx, w.ny, w.nz, w.pml)
+    arr, n = bv._materials(w.table)
+    for tuning in (64, 1 << 31, bv.TUNE_VEL_2CTA | bv.TUNE_VEL_3CTA, bv.TUNE_STRESS_8 | bv.TUNE_STRESS_16):
+        o = bv.Opts(w.f0, 1e-4, 0, 0, -1, 0, tuning)
+        h = C.c_void_p(None)
+        rc = bv.lib().bvfdtd_create(C.byref(h), C.byref(g), w.dx, w.dt, arr, n, w.index_map.ctypes.data, C.byref(o),
+                                    C.c_void_p(4096), 1 << 40, None)
+        assert rc == bv.EINVAL and not h.value
+
+
+def test_library_reads_no_environment_variable():
+    """the launch plan of the shipped library must not depend on the caller's environment: every getenv in csrc/
+    sits inside an #ifdef BVFDTD_DEV_KNOBS block, and the build does not define that macro"""
+    csrc = os.path.join(ROOT, "paper_2301_12727_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        guarded = 0
+        for line in open(os.path.join(csrc, f)):
+            t = line.strip()
+            if t.startswith("#ifdef BVFDTD_DEV_KNOBS"):
+                guarded += 1
+            elif t.startswith("#endif") and guarded:
+                guarded -= 1
+            elif t.startswith("#else") and guarded:
+                guarded = 0
+            if "getenv(" in line:
+                assert guarded, (f, line)
+    assert "BVFDTD_DEV_KNOBS" not in " ".join(bv_build.NVCC_FLAGS)

@@ -62,9 +62,9 @@ def compare_map(got, ref, rel=REL_PEAK):
     return e
 
 
-def run_both(bv, w, steps=None, flags=0, state=None):
+def run_both(bv, w, steps=None, flags=0, state=None, tuning=0):
     steps = w.steps if steps is None else steps
-    sim = bv.Simulation.from_workload(w, flags=flags)
+    sim = bv.Simulation.from_workload(w, flags=flags, tuning=tuning)
     o = orc.Oracle.from_workload(w)
     if state is not None:
         for n, a in state.items():
@@ -187,20 +187,18 @@ def test_stepped_random_domain(bv, dims, P, wave, flags):
 
 @pytest.mark.parametrize("dims,P,wave", [((150, 41, 70), 8, 1), ((131, 45, 66), 12, 0), ((64, 40, 52), 0, 1),
                                          ((150, 60, 80), 24, 1), ((203, 57, 64), 20, 0)])
-def test_velocity_three_cta_stage_plans(bv, dims, P, wave, monkeypatch):
+def test_velocity_three_cta_stage_plans(bv, dims, P, wave):
     """The velocity pass with three resident CTAs per SM and per-CTA stage plans (compact 3-stage plan
     outside the y / z slabs, full 2-stage plan inside; z slabs in chunks of their own) is what config 2
-    runs by default; BVFDTD_OCC_V=3 forces it on a small grid with ragged tiles and several chunks: it
-    must match the oracle AND be bit-identical to the two-CTA plan (BVFDTD_OCC_V=2)."""
+    runs by default; bvfdtd_opts.tuning = BVFDTD_TUNE_VEL_3CTA forces it on a small grid with ragged tiles and
+    several chunks: it must match the oracle AND be bit-identical to the two-CTA plan (BVFDTD_TUNE_VEL_2CTA)."""
     w = wl.random_domain(*dims, P, seed=60 + P, steps=90, waveform=wave, n_mat=200 if P == 20 else 6)
-    monkeypatch.setenv("BVFDTD_OCC_V", "3")
-    sim, o = run_both(bv, w)
+    sim, o = run_both(bv, w, tuning=bv.TUNE_VEL_3CTA)
     compare_state(sim, o)
     peak, rms = sim.read_peak_pressure()
     compare_map(peak, o.get("peak"))
     compare_map(rms, o.get("rms_amp"))
-    monkeypatch.setenv("BVFDTD_OCC_V", "2")
-    two = bv.Simulation.from_workload(w)
+    two = bv.Simulation.from_workload(w, tuning=bv.TUNE_VEL_2CTA)
     two.step(w.steps)
     for n in bv.FIELDS:
         assert np.array_equal(sim.read_fields(n), two.read_fields(n)), n
