@@ -148,6 +148,8 @@ struct bvfdtd_ctx {
     // CUDA graphs of one step and of GRAPH_STEPS steps per sensor regime (peak on/off x rms on/off), built on first use
     enum { GRAPH_STEPS = 8 };
     cudaGraphExec_t graph[4][2][2] = {};
+    cudaStream_t cap_stream2 = nullptr;    // second branch of a captured step: the velocity pass of the two-pass columns runs
+    cudaEvent_t cap_fork = nullptr, cap_join = nullptr;   // beside the fused sweep (both read the cur copies, write the nxt ones)
     cudaStream_t cap_stream = nullptr;     // library-owned stream the graphs are captured on (the caller's may be the
                                            // legacy default stream, which cannot be captured); nothing ever runs on it   // [regime][one step | GRAPH_STEPS steps][sel at the first step]
     // kernel timing
@@ -653,11 +655,24 @@ int enqueue_passes(bvfdtd_ctx *c, const Params &p, int phases, int64_t step, lon
     if (ev) CU(cudaEventRecord(ev[1], st));
     const dim3 rb(32, 4, 2), rg((L.nx + 31) / 32, (L.ny + 3) / 4, (L.nz + 1) / 2);
     const bool ff = c->ff_active;       // (only whole steps run in the fused mode: bvfdtd_step_phase leaves it first)
+    // in a captured step the fused sweep and the velocity pass of the other tile columns are two branches of the
+    // graph: they are independent (both read the cur copies and write the nxt ones) and fill each other's last wave
+    const bool fork = ff && d_ctr && c->cap_stream2 && c->fplan.n_f > 0 && c->fplan.n_v > 0 && (phases & PH_VELOCITY);
+    cudaStream_t sv = st;
+    if (fork) {
+        CU(cudaEventRecord(c->cap_fork, st));
+        CU(cudaStreamWaitEvent(c->cap_stream2, c->cap_fork, 0));
+        sv = c->cap_stream2;
+    }
     if (ff && (phases & PH_VELOCITY)) fused_launch(c->fplan, p, st);
     if (ev) CU(cudaEventRecord(ev[2], st));
     if (phases & PH_VELOCITY) {
         if (ref) k_velocity_ref<<<rg, rb, 0, st>>>(p);
-        else if (tiled_velocity(c->plan, p, st, ff ? c->fplan.items_v : nullptr, c->fplan.n_v)) return cuda_fail(cudaGetLastError(), "tiled_velocity");
+        else if (tiled_velocity(c->plan, p, sv, ff ? c->fplan.items_v : nullptr, c->fplan.n_v)) return cuda_fail(cudaGetLastError(), "tiled_velocity");
+    }
+    if (fork) {
+        CU(cudaEventRecord(c->cap_join, sv));
+        CU(cudaStreamWaitEvent(st, c->cap_join, 0));
     }
     if (ev) CU(cudaEventRecord(ev[3], st));
     if (phases & PH_STRESS) {
@@ -706,7 +721,12 @@ int get_graph(bvfdtd_ctx *c, int regime, int len, cudaGraphExec_t *out) {
     cudaGraphExec_t &slot = c->graph[regime][len == 1 ? 0 : 1][c->sel];
     if (!slot) {
         long long *d_ctr = (long long *)(c->ws + c->W.ctr);
-        if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+        if (!c->cap_stream) {
+            CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+            CU(cudaStreamCreateWithFlags(&c->cap_stream2, cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&c->cap_fork, cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&c->cap_join, cudaEventDisableTiming));
+        }
         CU(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed));
         int rc = BVFDTD_OK;
         for (int s = 0; s < len && rc == BVFDTD_OK; ++s) {
@@ -1078,6 +1098,9 @@ int bvfdtd_destroy(bvfdtd_ctx *c) {
     cudaStreamSynchronize(c->stream);
     drop_graphs(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->cap_stream2) cudaStreamDestroy(c->cap_stream2);
+    if (c->cap_fork) cudaEventDestroy(c->cap_fork);
+    if (c->cap_join) cudaEventDestroy(c->cap_join);
     if (c->src_own) cudaFree(c->src_own);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     tiled_plan_destroy(c->plan);

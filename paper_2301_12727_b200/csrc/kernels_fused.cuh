@@ -118,21 +118,21 @@ struct FusedIssue {
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
                 const int d = sp->psx + q * sp->xt;
-                if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, 3 * q);
-                if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, 3 * q);
+                if (tX.lo) t.box4s(d, xbox, &maps->psx, tX.cx_lo, y0, m, 3 * q);
+                if (tX.hi) t.box4s(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, 3 * q);
             }
             if (tYe) t.box4(sp->psy, C::B_BYTES, &maps->psyE, x0, jy0e - 2, m, p->ipsi7_cur);
-            if (tY) t.box4(sp->psy + C::B_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, 4);
+            if (tY) t.box4s(sp->psy + C::B_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, 4);
         }
         if (c & FC_VZ2) {
-            t.box4(FS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, p->icur[VZ]);
-            if (c & FC_ZS2) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 2);
+            t.box4s(FS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, p->icur[VZ]);
+            if (c & FC_ZS2) t.box4s(sp->psz, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 2);
         }
         if (c & FC_S3) {
-            if (c & FC_LOSSY3) t.box4(FS::RXX, C::D_BYTES, &maps->boxD, x0, y0, z - 3, RXX);
-            if (c & FC_PEAK) t.box4(FS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 3, F_PEAK);
-            if (c & FC_RMS) t.box4(FS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 3, F_SUMSQ);
-            if (c & FC_ZS3) t.box4(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 3), 5);
+            if (c & FC_LOSSY3) t.box4s(FS::RXX, C::D_BYTES, &maps->boxD, x0, y0, z - 3, RXX);
+            if (c & FC_PEAK) t.box4s(FS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 3, F_PEAK);
+            if (c & FC_RMS) t.box4s(FS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 3, F_SUMSQ);
+            if (c & FC_ZS3) t.box4s(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 3), 5);
         }
     }
 };
@@ -293,8 +293,8 @@ __device__ __forceinline__ void fused_consume(const Params &p, const StagePlan &
                 q_store<EDGE>(p.fnxt[VX] + goff, ox, g.nv);
                 q_store<EDGE>(p.fnxt[VY] + goff, oy, g.nv);
             }
-            q_st(xv + aoff, ox);
-            q_st(xy + boff, oy);
+            q_sts(xv + aoff, ox);
+            q_sts(xy + boff, oy);
             if (ex_vx) {
                 float val = 0.0f;
                 if (ex_vx_in) {
@@ -320,7 +320,7 @@ __device__ __forceinline__ void fused_consume(const Params &p, const StagePlan &
                                          dt2 * rcp_newton(rho_tab[a >> 24] + rho_tab[b >> 24]));
                     val = q_fma(cy, dyy, q_ld(vyo + bo));
                 }
-                q_st(xy + bo, val);
+                q_sts(xy + bo, val);
             }
             consumer_barrier(C::NC);
             if (active) {
@@ -541,15 +541,34 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
                 out.flags[(size_t)(bx + ntx * by) * (nz + 4) + 2 + k] = w;
             }
     out.planes_f = planes_f;
-    // chunk lengths: about three waves of the resident CTAs, the long items first
-    const long long planes_all = (long long)ntx * nty * nz;
-    auto chunk_len = [&](long long planes, int slots, int lo, int hi) {
-        const long long want = planes / std::max(1, 3 * slots);
-        return (int)std::max<long long>(lo, std::min<long long>(hi, want));
+    // runs of each kind
+    struct Run { int bx, by, a, b; };
+    std::vector<Run> rf, rv, rs;
+    for (int by = 0; by < nty; ++by)
+        for (int bx = 0; bx < ntx; ++bx) {
+            for (int a = 0; a < nz;) {
+                const bool r = R(bx, by, a);
+                int b = a;
+                while (b < nz && R(bx, by, b) == r) ++b;
+                if (r) rf.push_back({bx, by, a, b});
+                else {
+                    // velocity pass: the z slabs get chunks of their own (compact stage plan elsewhere)
+                    const int cuts[4] = {a, std::min(b, std::max(a, P)), std::max(a, std::min(b, nz - P)), b};
+                    for (int c = 0; c < 3; ++c)
+                        if (cuts[c + 1] > cuts[c]) rv.push_back({bx, by, cuts[c], cuts[c + 1]});
+                    if (by % group == 0) rs.push_back({bx, by / group, a, b});
+                }
+                a = b;
+            }
+        }
+    // chunk length of a kind: about three rounds of the resident CTAs.  (Choosing the length that minimises
+    // rounds x (planes + priming planes) in a model of equal items -- 2 rounds of 90 planes instead of 3.5 of 50 on
+    // config 2 -- measured 2-8 % slower: the passes are limited by memory-level parallelism, not by the round count.)
+    auto wave_len = [&](const std::vector<Run> &runs, int slots, int lo, int hi) {
+        long long planes = 0;
+        for (const Run &r : runs) planes += r.b - r.a;
+        return (int)std::max<long long>(lo, std::min<long long>(hi, planes / std::max(1, 3 * slots)));
     };
-    const int len_f = chunk_len(planes_f, slots_f, 24, 128);
-    const int len_v = chunk_len(planes_all - planes_f, slots_v, 16, 96);
-    const int len_s = chunk_len((planes_all - planes_f) * TY / sty, slots_s, 16, 96);
     // [a, b) in about equal chunks of at most `len` planes; with `fused` no chunk boundary falls inside, or within
     // two planes of, a z slab (a fused chunk recomputes vz at kz0-2, kz0-1 and kz1 without their psi)
     auto split = [&](std::vector<int4> &dst, int bx, int by, int a, int b, int len, bool fused) {
@@ -566,23 +585,10 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
             k0 = k1;
         }
     };
-    for (int by = 0; by < nty; ++by)
-        for (int bx = 0; bx < ntx; ++bx) {
-            for (int a = 0; a < nz;) {
-                const bool r = R(bx, by, a);
-                int b = a;
-                while (b < nz && R(bx, by, b) == r) ++b;
-                if (r) split(out.f, bx, by, a, b, len_f, true);
-                else {
-                    // velocity pass: the z slabs get chunks of their own (compact stage plan elsewhere)
-                    int cuts[4] = {a, std::min(b, std::max(a, P)), std::max(a, std::min(b, nz - P)), b};
-                    for (int c = 0; c < 3; ++c)
-                        if (cuts[c + 1] > cuts[c]) split(out.v, bx, by, cuts[c], cuts[c + 1], len_v, false);
-                    if (by % group == 0) split(out.s, bx, by / group, a, b, len_s, false);
-                }
-                a = b;
-            }
-        }
+    const int len_f = wave_len(rf, slots_f, 24, 128), len_v = wave_len(rv, slots_v, 16, 96), len_s = wave_len(rs, slots_s, 16, 96);
+    for (const Run &r : rf) split(out.f, r.bx, r.by, r.a, r.b, len_f, true);
+    for (const Run &r : rv) split(out.v, r.bx, r.by, r.a, r.b, len_v, false);
+    for (const Run &r : rs) split(out.s, r.bx, r.by, r.a, r.b, len_s, false);
     // launch order: the long items first (the short ones fill the last wave), and among items of about the same
     // length those of one z range together, tile rows in order: CTAs that run at the same time then share their
     // halo rows and columns in L2 (ordered by length alone, the halo reads of the fused sweep went to DRAM: L2

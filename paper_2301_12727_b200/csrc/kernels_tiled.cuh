@@ -153,11 +153,17 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
         ::"r"(smem_u32(dst)), "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)) : "memory");
 }
 // One box load into the stage, counting its bytes for the stage barrier.
+// (box4s marks the boxes only this CTA reads -- plain tiles of old values, psi.  Loading them with an L2
+// evict-first policy, and storing the results with st.global.cs, was measured and made every pass 3-8 % slower
+// (profiles/r2b_fused.md); both load the same way.)
 struct Tma {
     unsigned char *st;
     uint64_t *bar;
     uint32_t bytes;
     __device__ __forceinline__ void box4(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z, int f) {
+        tma_load_4d(st + off, map, bar, x, y, z, f); bytes += nbytes;
+    }
+    __device__ __forceinline__ void box4s(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z, int f) {
         tma_load_4d(st + off, map, bar, x, y, z, f); bytes += nbytes;
     }
     __device__ __forceinline__ void box3(int off, uint32_t nbytes, const CUtensorMap *map, int x, int y, int z) {
@@ -191,6 +197,7 @@ __device__ __forceinline__ Q4 q_fmas(float s, Q4 y, Q4 z) { const float2 t = mak
 __device__ __forceinline__ Q4 q_fnma(Q4 y, Q4 z, Q4 x) { Q4 q; q.a = __ffma2_rn(f2neg(y.a), z.a, x.a); q.b = __ffma2_rn(f2neg(y.b), z.b, x.b); return q; }
 __device__ __forceinline__ float q_get(const Q4 &q, int c) { return c == 0 ? q.a.x : c == 1 ? q.a.y : c == 2 ? q.b.x : q.b.y; }
 __device__ __forceinline__ void q_st(float *g, const Q4 &q) { *reinterpret_cast<float4 *>(g) = make_float4(q.a.x, q.a.y, q.b.x, q.b.y); }
+__device__ __forceinline__ void q_sts(float *g, const Q4 &q) { *reinterpret_cast<float4 *>(g) = make_float4(q.a.x, q.a.y, q.b.x, q.b.y); }
 // store the first nv (1..4) cells only: partial quad at the ragged x edge
 __device__ __forceinline__ void q_st_n(float *g, const Q4 &q, int nv) {
     if (nv >= 4) { q_st(g, q); return; }
@@ -391,7 +398,7 @@ struct VelIssue {
         // start), so ONE box of sigma_xx with both halos (rows j-1 .. j+9, in the idle sxy slot) serves D+x,
         // D+y and D+z instead of the three boxes
         if (c & VC_FL) t.box4(VS::SXY, C::C_BYTES, &maps->boxC, x0 - 4, y0 - 1, z, p->icur[SXX]);
-        else t.box4(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, p->icur[SZZ]);
+        else t.box4s(VS::SZZ, C::D_BYTES, &maps->boxD, x0, y0, z, p->icur[SZZ]);
         if (xz) t.box4(VS::SXZ, C::A_BYTES, &maps->boxA, x0 - 4, y0, z, SXZ);
         if (yz) t.box4(VS::SYZ, C::B_BYTES, &maps->boxB, x0, y0 - 2, z, SYZ);
         if (c & VC_IN0) {
@@ -407,23 +414,23 @@ struct VelIssue {
             for (int q = 0; q < 3; ++q) {
                 if (use[q]) {
                     const int d = sp->psx + q * sp->xt;
-                    if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, q);
-                    if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, q);
+                    if (tX.lo) t.box4s(d, xbox, &maps->psx, tX.cx_lo, y0, m, q);
+                    if (tX.hi) t.box4s(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, q);
                 }
-                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, q == 1 ? p->ipsi7_cur : q);
+                if (tY && usey[q]) t.box4s(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, q == 1 ? p->ipsi7_cur : q);
             }
         }
         if (c & VC_IN1) {
-            t.box4(VS::VXO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VX]);
-            t.box4(VS::VYO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VY]);
+            t.box4s(VS::VXO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VX]);
+            t.box4s(VS::VYO, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[VY]);
         }
-        if (c & VC_IN2) t.box4(VS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, p->icur[VZ]);
+        if (c & VC_IN2) t.box4s(VS::VZO, C::D_BYTES, &maps->boxD, x0, y0, z - 2, p->icur[VZ]);
         if (c & VC_ZS1) {
             const int kc = z_compact(*p, m - 1);
-            if (c & VC_WXZ) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, kc, 0);
-            if (c & VC_WYZ) t.box4(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, kc, 1);
+            if (c & VC_WXZ) t.box4s(sp->psz, C::D_BYTES, &maps->psz, x0, y0, kc, 0);
+            if (c & VC_WYZ) t.box4s(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, kc, 1);
         }
-        if (c & VC_ZS2) t.box4(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 2);
+        if (c & VC_ZS2) t.box4s(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 2);
         t.box3(VS::MAT, C::MX * C::MY, &maps->mat, x0, y0, m - 1);
     }
 };
@@ -733,40 +740,40 @@ struct StrIssue {
             for (int q = 0; q < 3; ++q) {
                 if (use[q]) {
                     const int d = sp->psx + q * sp->xt;
-                    if (tX.lo) t.box4(d, xbox, &maps->psx, tX.cx_lo, y0, m, 3 + q);
-                    if (tX.hi) t.box4(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, 3 + q);
+                    if (tX.lo) t.box4s(d, xbox, &maps->psx, tX.cx_lo, y0, m, 3 + q);
+                    if (tX.hi) t.box4s(d + sp->xhi, xbox, &maps->psx, tX.cx_hi, y0, m, 3 + q);
                 }
-                if (tY && usey[q]) t.box4(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, 3 + q);
+                if (tY && usey[q]) t.box4s(sp->psy + q * C::D_BYTES, C::D_BYTES, &maps->psy, x0, jy0, m, 3 + q);
             }
         }
         if (c & SC_XY0) {
-            t.box4(SS::SXY, C::D_BYTES, &maps->boxD, x0, y0, z, SXY);
-            t.box4(SS::RXY, C::D_BYTES, &maps->boxD, x0, y0, z, RXY);
+            t.box4s(SS::SXY, C::D_BYTES, &maps->boxD, x0, y0, z, SXY);
+            t.box4s(SS::RXY, C::D_BYTES, &maps->boxD, x0, y0, z, RXY);
         }
         if (c & SC_IN1) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) t.box4(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[SXX + q]);
+            for (int q = 0; q < 3; ++q) t.box4s(SS::SII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->icur[SXX + q]);
             if (c & SC_RII1) {
-                t.box4(SS::RII, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX);
+                t.box4s(SS::RII, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX);
                 if (!(c & SC_RFL1)) {
 #pragma unroll
-                    for (int q = 1; q < 3; ++q) t.box4(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
+                    for (int q = 1; q < 3; ++q) t.box4s(SS::RII + q * C::D_BYTES, C::D_BYTES, &maps->boxD, x0, y0, z - 1, RXX + q);
                 }
             }
             // phasor mode (NEXT-3) keeps its two accumulators in the peak / sumsq slots
-            if (c & SC_PEAK) t.box4(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHRE : F_PEAK);
-            if (c & SC_RMS) t.box4(SS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHIM : F_SUMSQ);
-            if (c & SC_ZS1) t.box4(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 1), 5);
+            if (c & SC_PEAK) t.box4s(SS::PEAK, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHRE : F_PEAK);
+            if (c & SC_RMS) t.box4s(SS::SUMSQ, C::D_BYTES, &maps->boxD, x0, y0, z - 1, p->do_phasor ? F_PHIM : F_SUMSQ);
+            if (c & SC_ZS1) t.box4s(sp->psz + 2 * C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 1), 5);
         }
         if (c & SC_XZ2) {
-            t.box4(SS::SXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SXZ);
-            t.box4(SS::RXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RXZ);
-            if (c & SC_ZS2) t.box4(sp->psz, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 3);
+            t.box4s(SS::SXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SXZ);
+            t.box4s(SS::RXZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RXZ);
+            if (c & SC_ZS2) t.box4s(sp->psz, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 3);
         }
         if (c & SC_YZ2) {
-            t.box4(SS::SYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SYZ);
-            t.box4(SS::RYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RYZ);
-            if (c & SC_ZS2) t.box4(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 4);
+            t.box4s(SS::SYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, SYZ);
+            t.box4s(SS::RYZ, C::D_BYTES, &maps->boxD, x0, y0, z - 2, RYZ);
+            if (c & SC_ZS2) t.box4s(sp->psz + C::D_BYTES, C::D_BYTES, &maps->psz, x0, y0, z_compact(*p, m - 2), 4);
         }
         t.box3(mat_off, C::MX * C::MY, &maps->mat, x0, y0, m);
     }
