@@ -467,21 +467,26 @@ def ours(args):
     pinned_idx = torch.from_numpy(w.index_map.copy()).pin_memory()
     pinned_peak = torch.empty(w.index_map.shape, dtype=torch.float32).pin_memory()
     idx_np, peak_np = pinned_idx.numpy(), pinned_peak.numpy()
-    barrier()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    sim = bv.Simulation(w.nx, w.ny, w.nz, w.pml, w.dx, w.dt, w.table, idx_np, w.f0, w.pml_R,
-                        w.peak_begin, w.rms_begin, w.sensor_end, flags=flags, device=dev, tuning=args.tuning)
-    sim.set_source(w.src_cell, w.src_amp, w.src_delay, w.waveform, w.f_src, w.n_cycles)
-    sim.step(total)
-    sim.read_peak_pressure(peak=True, rms=False, out_peak=peak_np)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
+    def e2e_pass():
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sim = bv.Simulation(w.nx, w.ny, w.nz, w.pml, w.dx, w.dt, w.table, idx_np, w.f0, w.pml_R,
+                            w.peak_begin, w.rms_begin, w.sensor_end, flags=flags, device=dev, tuning=args.tuning)
+        sim.set_source(w.src_cell, w.src_amp, w.src_delay, w.waveform, w.f_src, w.n_cycles)
+        sim.step(total)
+        sim.read_peak_pressure(peak=True, rms=False, out_peak=peak_np)
+        torch.cuda.synchronize()
+        dt_s = time.perf_counter() - t0
+        sim.close()
+        return dt_s
+
+    e2e_cold_s = e2e_pass()          # first pass: the allocator's cudaMalloc of the workspace, first graph instantiation
+    e2e_s = e2e_pass()               # timed pass (the warm-up rule applies to this leg too)
     e2e_ms = reduce_max(e2e_s * 1e3, dev)
     h2d = w.index_map.nbytes + 256 * 32 + 4 * 4 * (w.nx + w.ny + w.nz) + w.src_cell.size * 16
     d2h = peak_np.nbytes
     e2e_value = world * w.cells * total / (e2e_ms * 1e-3) / 1e9
-    sim.close()
 
     if rank != 0:
         return 0
@@ -564,7 +569,9 @@ def ours(args):
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d / total,
                 "d2h_bytes_per_step": d2h / total, "steps": total, "seconds": e2e_ms * 1e-3,
-                "what": "bvfdtd_create + set_source + step(W+K) + read_peak_pressure to pinned host"},
+                "seconds_first_pass": e2e_cold_s,
+                "what": "bvfdtd_create + set_source + step(W+K) + read_peak_pressure to pinned host, wall clock; "
+                        "second of two identical passes (the first also pays the workspace cudaMalloc)"},
         "gpu_launches": int(round(sum(kt[k]["launches"] for k in kt) * K / max(1, min(K, 4096)))),
         "ms_per_step_kernel_by_kernel": ms_timed_pass,
         "roofline": roofline,

@@ -108,7 +108,9 @@ enum { /* bvfdtd_opts.tuning */
     BVFDTD_TUNE_STRESS_8 = 4,   /* stress pass: 64 x 8 tiles */
     BVFDTD_TUNE_STRESS_16 = 8,  /* stress pass: 64 x 16 tiles */
     BVFDTD_TUNE_NO_GRAPH = 16,  /* bvfdtd_step launches kernel by kernel instead of replaying CUDA graphs */
-    BVFDTD_TUNE_NO_FUSED = 32   /* all-fluid tile columns run the two passes like every other tile (no fused sweep) */
+    BVFDTD_TUNE_NO_FUSED = 32,  /* all-fluid tile columns run the two passes like every other tile (no fused sweep) */
+    BVFDTD_TUNE_FUSED = 64      /* use the fused sweep wherever it applies, also on grids the library judges too small
+                                   for it to pay (under 6 M cells) or with few all-fluid tile columns */
 };
 
 /* Field ids for bvfdtd_read_fields / bvfdtd_write_fields. */

@@ -27,7 +27,7 @@ FLAG_PHASOR = 4
 FLAG_ZLO_OPEN = 8
 FLAG_ZHI_OPEN = 16
 # bvfdtd_opts.tuning: launch-plan requests for tests and experiments (results never depend on them)
-TUNE_VEL_2CTA, TUNE_VEL_3CTA, TUNE_STRESS_8, TUNE_STRESS_16, TUNE_NO_GRAPH, TUNE_NO_FUSED = 1, 2, 4, 8, 16, 32
+TUNE_VEL_2CTA, TUNE_VEL_3CTA, TUNE_STRESS_8, TUNE_STRESS_16, TUNE_NO_GRAPH, TUNE_NO_FUSED, TUNE_FUSED = 1, 2, 4, 8, 16, 32, 64
 
 OK, EINVAL, ENOMEM, ESTABILITY, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
 

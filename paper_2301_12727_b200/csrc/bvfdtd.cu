@@ -263,6 +263,9 @@ int fused_setup(bvfdtd_ctx *c) {
     const uint32_t off = BVFDTD_FLAG_REFERENCE_KERNELS | BVFDTD_FLAG_DENSE | BVFDTD_FLAG_PHASOR | BVFDTD_FLAG_ZLO_OPEN | BVFDTD_FLAG_ZHI_OPEN;
     if ((c->opts.flags & off) || (c->opts.tuning & BVFDTD_TUNE_NO_FUSED)) return BVFDTD_OK;
     const Layout &L = c->L;
+    // small grids are launch-bound and L2-resident: a third kernel per step costs more than the bytes it saves
+    // (config 1, 128^3: 22 Gcell/s with the two passes, 17.7 fused); BVFDTD_TUNE_FUSED forces the fused mode
+    if ((long long)L.nx * L.ny * L.nz < 6000000LL && !(c->opts.tuning & BVFDTD_TUNE_FUSED)) return BVFDTD_OK;
     int rc = fused_plan_create(c->fplan, c->plan, L, c->prm, c->ws + c->W.psi[6], (long long)(c->W.psi[7] - c->W.psi[6]));
     if (rc == BVFDTD_EINVAL) return BVFDTD_OK;                 // the stages do not fit: stay with the two passes
     if (rc) return cuda_fail(cudaGetLastError(), "fused_plan_create");
@@ -282,7 +285,8 @@ int fused_setup(bvfdtd_ctx *c) {
     c->fplan.planes_f = lists.planes_f;
     c->fplan.planes_all = planes_all;
     // worth it from a tenth of the tile-planes on (below that the extra launch costs more than it saves)
-    if (lists.planes_f * 10 < planes_all) return BVFDTD_OK;
+    if (lists.planes_f * 10 < planes_all && !(c->opts.tuning & BVFDTD_TUNE_FUSED)) return BVFDTD_OK;
+    if (lists.planes_f == 0) return BVFDTD_OK;
     const size_t cap = fused_items_capacity(L);
     if (lists.f.size() > cap || lists.v.size() > cap || lists.s.size() > cap) return BVFDTD_OK;
     const std::vector<int4> *src[3] = {&lists.f, &lists.v, &lists.s};
@@ -400,10 +404,11 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     if (!grid_ok(grid) || !table || !index_map || !opts || !d_workspace) return BVFDTD_EINVAL;
     if (!(dx > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dt)) return BVFDTD_EINVAL;
     constexpr uint32_t TUNE_ALL = BVFDTD_TUNE_VEL_2CTA | BVFDTD_TUNE_VEL_3CTA | BVFDTD_TUNE_STRESS_8 | BVFDTD_TUNE_STRESS_16 |
-                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED;
+                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED | BVFDTD_TUNE_FUSED;
     if (!(opts->f0 > 0.0) || (opts->tuning & ~TUNE_ALL) != 0) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_VEL_2CTA) && (opts->tuning & BVFDTD_TUNE_VEL_3CTA)) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_STRESS_8) && (opts->tuning & BVFDTD_TUNE_STRESS_16)) return BVFDTD_EINVAL;
+    if ((opts->tuning & BVFDTD_TUNE_NO_FUSED) && (opts->tuning & BVFDTD_TUNE_FUSED)) return BVFDTD_EINVAL;
     double R = opts->pml_R == 0.0 ? 1e-4 : opts->pml_R;
     if (!(R > 0.0 && R < 1.0)) return BVFDTD_EINVAL;
     if (((uintptr_t)d_workspace & 255) != 0) return BVFDTD_EINVAL;

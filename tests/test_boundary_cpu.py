@@ -148,7 +148,8 @@ def test_tuning_bits_validated_before_any_device_call(bv):
     w = wl.make(0)
     g = bv.Grid(w.nx, w.ny, w.nz, w.pml)
     arr, n = bv._materials(w.table)
-    for tuning in (64, 1 << 31, bv.TUNE_VEL_2CTA | bv.TUNE_VEL_3CTA, bv.TUNE_STRESS_8 | bv.TUNE_STRESS_16):
+    for tuning in (128, 1 << 31, bv.TUNE_VEL_2CTA | bv.TUNE_VEL_3CTA, bv.TUNE_STRESS_8 | bv.TUNE_STRESS_16,
+                   bv.TUNE_FUSED | bv.TUNE_NO_FUSED):
         o = bv.Opts(w.f0, 1e-4, 0, 0, -1, 0, tuning)
         h = C.c_void_p(None)
         rc = bv.lib().bvfdtd_create(C.byref(h), C.byref(g), w.dx, w.dt, arr, n, w.index_map.ctypes.data, C.byref(o),

@@ -1,6 +1,7 @@
 """GPU parity on the configurations of BASELINE.json at their FULL sizes, from the zero state, in the
-default launch configuration (the one bench.py times: tiled kernels, tile-class skipping, sigma_xx-for-all
-in fluid velocity tiles, r_xx-only in lossy fluid, fused injection) -- nothing is written through
+default launch configuration (the one bench.py times: CUDA-graph replay, the fused single sweep in the all-fluid
+tile columns, elsewhere the two tiled passes with tile-class skipping, sigma_xx-for-all in fluid velocity tiles and
+r_xx-only in lossy fluid) -- nothing is written through
 `bvfdtd_write_fields` except, where stated, the three velocities (which leaves every optimisation on).
 
   * config 2, all 3000 steps (the oracle needs ~9 min on the box's 16 cores): north_star's bars
@@ -30,6 +31,7 @@ from test_gpu_parity import GROUPS, compare_map
 
 pytestmark = pytest.mark.gpu
 
+DEFAULT_MODE = "tiled, tile-class skipping, fused sweep in all-fluid tile columns"
 CACHE = os.environ.get("BVFDTD_ORACLE_CACHE", "/tmp/bvfdtd_oracle_cache")
 OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
 
@@ -132,22 +134,35 @@ def compare_full(sim, ref, rel=1e-4, rel_max=10.0, rel_block=10.0):
 def _run_and_compare(bv, w, steps, state=None, tag=None):
     ref = OracleResult(w, steps, state)
     sim = bv.Simulation.from_workload(w)
-    assert sim.kernel_mode() == "tiled, tile-class skipping"
+    # the default path on these grids: tile-class skipping, the fused sweep in the all-fluid tile columns, graphs
+    assert sim.kernel_mode() == DEFAULT_MODE and sim.mode_bits() & bv.MODE_GRAPH
     for n, a in (state or {}).items():
         assert n in ("vx", "vy", "vz")                # anything else would switch optimisations off
         sim.write_fields(n, a)
-    assert sim.kernel_mode() == "tiled, tile-class skipping"
+    assert sim.kernel_mode() == DEFAULT_MODE
     sim.step(steps)
     rep = compare_full(sim, ref)
     peak, rms = sim.read_peak_pressure()
     out = {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "steps": steps, "fields": rep,
            "peak_max_rel": compare_map(peak, ref.get("peak")), "oracle_seconds": ref.seconds,
-           "oracle_threads": os.cpu_count(), "kernel_mode": sim.kernel_mode()}
+           "oracle_threads": os.cpu_count(), "kernel_mode": sim.kernel_mode(), "fused_tile_plane_fraction": sim.fused_coverage()}
     if 0 <= w.rms_begin < steps:
         assert sim.rms_count == ref.rms_count
         out["rms_max_rel"] = compare_map(rms, ref.get("rms_amp"))
     out["worst_rel_l2"] = max(v["rel_l2"] for v in rep.values())
+    # the same run on the two passes alone (no fused sweep, no graph): the default path must equal it bit for bit
+    keep = {n: sim.read_fields(n) for n in ("p", "vz", "rxx")}
     sim.close()
+    two = bv.Simulation.from_workload(w, tuning=bv.TUNE_NO_FUSED | bv.TUNE_NO_GRAPH)
+    for n, a in (state or {}).items():
+        two.write_fields(n, a)
+    two.step(steps)
+    for n, a in keep.items():
+        assert np.array_equal(a, two.read_fields(n)), n
+    pk2, _ = two.read_peak_pressure(rms=False)
+    assert np.array_equal(peak, pk2)
+    out["bit_identical_to_two_pass_path"] = True
+    two.close()
     print(json.dumps({k: v for k, v in out.items() if k != "fields"}))
     if tag:
         try:
@@ -184,7 +199,7 @@ def test_config2_short_run_velocity_state_only(bv):
     for n, a in st.items():
         sim.write_fields(n, a)
     sim.step(8)
-    assert sim.kernel_mode() == "tiled, tile-class skipping"
+    assert sim.kernel_mode() == DEFAULT_MODE
     compare_full(sim, ref, rel=1e-5)
     peak, rms = sim.read_peak_pressure()
     compare_map(peak, ref.get("peak"), rel=1e-4)

@@ -44,7 +44,7 @@ CASES = [  # dims, P, seed, waveform, steps, velocity start
 def test_fused_matches_oracle_and_two_pass(bv, dims, P, seed, wave, steps, vstart):
     w = wl.fluid_domain(*dims, P, seed=seed, steps=steps, waveform=wave)
     st = wl.random_state(w, 70 + seed, fields=("vx", "vy", "vz")) if vstart else {}
-    f = bv.Simulation.from_workload(w)
+    f = bv.Simulation.from_workload(w, tuning=bv.TUNE_FUSED)        # (small grid: the library would not fuse by itself)
     assert f.mode_bits() & bv.MODE_FUSED, "the fused sweep should take this domain"
     assert f.fused_coverage() > 0.2
     two = bv.Simulation.from_workload(w, tuning=bv.TUNE_NO_FUSED)
@@ -81,7 +81,7 @@ def test_fused_matches_oracle_and_two_pass(bv, dims, P, seed, wave, steps, vstar
 
 def test_fused_step_phase_leaves_the_fused_mode(bv):
     w = wl.fluid_domain(150, 60, 70, 8, seed=6, steps=30)
-    f = bv.Simulation.from_workload(w)
+    f = bv.Simulation.from_workload(w, tuning=bv.TUNE_FUSED)
     two = bv.Simulation.from_workload(w, tuning=bv.TUNE_NO_FUSED)
     f.step(11); two.step(11)
     assert f.mode_bits() & bv.MODE_FUSED
