@@ -240,6 +240,13 @@ int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[4], int64_t launches[4]);
 /* How much of the grid the fused single sweep takes: 64 x 8 tile-planes it runs / all tile-planes
  * (0 when the context is not in the fused mode, BVFDTD_MODE_FUSED).  Host-side query. */
 int bvfdtd_fused_coverage(const bvfdtd_ctx *ctx, int64_t *planes_fused, int64_t *planes_all);
+/* The work lists of the fused mode, for tests: which = 0 fused sweep, 1 velocity pass, 2 stress pass.  items
+ * (HOST, capacity entries of 4 int32: tile x, tile y, first plane, one past the last plane) receives at most
+ * `capacity` entries, *n_items the length of the list (0 outside the fused mode), tile_rows[0] the rows of the
+ * tiles the list counts in (8, or 16 for the stress pass on 64 x 16 tiles; tiles are 64 cells wide).  Lists 0 and
+ * 1, and lists 0 and 2, each cover every tile-plane of the grid exactly once. */
+int bvfdtd_work_items(bvfdtd_ctx *ctx, int32_t which, int32_t *items, int64_t capacity, int64_t *n_items,
+                      int32_t tile_rows[1]);
 
 /* ---- host-only helpers (no CUDA device needed): the S0 constructions, exposed so that the
  * construction-parity tests can run anywhere.  Same code path bvfdtd_create uses. ---- */

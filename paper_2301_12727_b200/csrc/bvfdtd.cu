@@ -1090,6 +1090,20 @@ int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[4], int64_t launches[4]) {
     return BVFDTD_OK;
 }
 
+int bvfdtd_work_items(bvfdtd_ctx *c, int32_t which, int32_t *items, int64_t capacity, int64_t *n_items, int32_t tile_rows[1]) {
+    if (!c || which < 0 || which > 2 || !n_items || capacity < 0 || (capacity > 0 && !items)) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
+    const int n = !c->ff_active ? 0 : which == 0 ? c->fplan.n_f : which == 1 ? c->fplan.n_v : c->fplan.n_s;
+    *n_items = n;
+    if (tile_rows) tile_rows[0] = which == 2 ? (c->plan.s16 ? CfgS::TY : CfgS8::TY) : CfgF::TY;
+    const int64_t m = std::min<int64_t>(n, capacity);
+    if (m > 0) {
+        CU(cudaMemcpyAsync(items, c->ws + c->W.items[which], (size_t)m * sizeof(int4), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return BVFDTD_OK;
+}
+
 int bvfdtd_fused_coverage(const bvfdtd_ctx *c, int64_t *planes_fused, int64_t *planes_all) {
     if (!c || !planes_fused || !planes_all) return BVFDTD_EINVAL;
     *planes_fused = c->ff_active ? c->fplan.planes_f : 0;

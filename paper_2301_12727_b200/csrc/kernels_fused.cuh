@@ -517,6 +517,7 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
                 if (P > 0) {
                     if (ra > 0 && ra < P + 2) ra = P + 2;
                     if (rb < nz && rb > nz - P - 1) rb = nz - P - 1;
+                    if ((ra > nz - P - 1 && ra < nz) || (rb > 0 && rb < P + 2)) rb = ra;   // the run lies inside a slab: dropped
                 }
                 if (rb - ra >= LMIN)
                     for (int by = gy; by < g1; ++by)
@@ -553,7 +554,11 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
                 if (r) rf.push_back({bx, by, a, b});
                 else {
                     // velocity pass: the z slabs get chunks of their own (compact stage plan elsewhere)
-                    const int cuts[4] = {a, std::min(b, std::max(a, P)), std::max(a, std::min(b, nz - P)), b};
+                    // (a cut that would leave a piece under 8 planes is not made: a chunk costs 4 priming planes)
+                    int cuts[4] = {a, std::min(b, std::max(a, P)), std::max(a, std::min(b, nz - P)), b};
+                    if (cuts[1] - cuts[0] < 8 || cuts[2] - cuts[1] < 8) cuts[1] = cuts[0];
+                    if (cuts[3] - cuts[2] < 8 || cuts[2] - cuts[1] < 8) cuts[2] = cuts[3];
+                    if (cuts[2] < cuts[1]) cuts[1] = cuts[2] = cuts[0];
                     for (int c = 0; c < 3; ++c)
                         if (cuts[c + 1] > cuts[c]) rv.push_back({bx, by, cuts[c], cuts[c + 1]});
                     if (by % group == 0) rs.push_back({bx, by / group, a, b});

@@ -112,3 +112,53 @@ def test_fused_on_config2_layout_short(bv):
     pb, rb = two.read_peak_pressure()
     assert np.array_equal(pa, pb) and np.array_equal(ra, rb)
     f.close(); two.close()
+
+
+def _check_lists(sim, nx, ny, nz, P):
+    """lists 0 + 1 and 0 + 2 cover every tile-plane exactly once; no boundary of a fused item lies inside, or within
+    two planes of, a z slab (the chunk would recompute vz there without the psi it does not own)"""
+    cover = {}
+    for which in (0, 1, 2):
+        it, rows = sim.work_items(which)
+        cnt = np.zeros(((ny + rows - 1) // rows, (nx + 63) // 64, nz), np.int32)
+        for bx, by, a, b in it:
+            assert 0 <= a < b <= nz
+            cnt[by, bx, a:b] += 1
+            if which == 0 and P > 0:
+                for e in (a, b):
+                    assert e in (0, nz) or P + 2 <= e <= nz - P - 1, (bx, by, a, b)
+        cover[which] = (cnt, rows)
+    f, v, st = cover[0][0], cover[1][0], cover[2][0]
+    assert ((f + v) == 1).all()
+    g = cover[2][1] // 8
+    assert ((f[::g] + st) == 1).all()
+    if g > 1 and f.shape[0] % g == 0:
+        assert (f[::g] == f[1::g]).all()          # a 64 x 16 stress tile is fused as a whole
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_work_lists_partition_the_grid(bv, cfg):
+    w = wl.make(cfg, steps=2)
+    sim = bv.Simulation.from_workload(w)
+    assert sim.mode_bits() & bv.MODE_FUSED
+    _check_lists(sim, w.nx, w.ny, w.nz, w.pml)
+    sim.close()
+
+
+def test_fused_run_that_would_start_inside_the_top_slab(bv):
+    """a solid box just below the top z slab leaves an all-fluid run that starts INSIDE the slab (config 3 has such
+    tile columns): it must stay with the two passes"""
+    nx, ny, nz, P = 150, 80, 110, 24
+    w = wl.fluid_domain(nx, ny, nz, P, seed=7, steps=24, solid_boxes=0)
+    w.index_map[76:86, 30:50, 30:100] = 4            # no fused plane in 73..88: the run above would start at 89 > nz-P-1 = 85
+    w.index_map[16:22, 28:52, 90:140] = 5            # ... and here the run below would end at 13 < P+2 = 26
+    st = wl.random_state(w, 77, fields=("vx", "vy", "vz"))
+    f = bv.Simulation.from_workload(w, tuning=bv.TUNE_FUSED)
+    two = bv.Simulation.from_workload(w, tuning=bv.TUNE_NO_FUSED)
+    assert f.mode_bits() & bv.MODE_FUSED
+    _check_lists(f, nx, ny, nz, P)
+    for n, a in st.items():
+        f.write_fields(n, a); two.write_fields(n, a)
+    f.step(24); two.step(24)
+    _same(f, two, bv)
+    f.close(); two.close()
