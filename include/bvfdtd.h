@@ -240,6 +240,10 @@ int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[4], int64_t launches[4]);
 /* How much of the grid the fused single sweep takes: 64 x 8 tile-planes it runs / all tile-planes
  * (0 when the context is not in the fused mode, BVFDTD_MODE_FUSED).  Host-side query. */
 int bvfdtd_fused_coverage(const bvfdtd_ctx *ctx, int64_t *planes_fused, int64_t *planes_all);
+/* Self-check (compute-sanitizer is not available everywhere): the number of non-zero floats in the zero gaps of
+ * the private layout of all 25 grid arrays (x beyond nx, the two extra rows, the two planes before and after: the
+ * zero ghost of reading P4, which no kernel may write).  0 on a healthy context.  Synchronises the stream. */
+int bvfdtd_padding_nonzeros(bvfdtd_ctx *ctx, int64_t *count);
 /* The work lists of the fused mode, for tests: which = 0 fused sweep, 1 velocity pass, 2 stress pass.  items
  * (HOST, capacity entries of 4 int32: tile x, tile y, first plane, one past the last plane) receives at most
  * `capacity` entries, *n_items the length of the list (0 outside the fused mode), tile_rows[0] the rows of the

@@ -42,7 +42,7 @@ SYMBOLS = (
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
-    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage", "bvfdtd_work_items",
+    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage", "bvfdtd_work_items", "bvfdtd_padding_nonzeros",
 )
 MODE_REFERENCE, MODE_DENSE, MODE_SIGMA_WRITTEN, MODE_FUSED, MODE_GRAPH = 1, 2, 4, 8, 16
 BHTE_TRACK_MAX = 1
@@ -101,6 +101,7 @@ def lib():
         L.bvfdtd_rms_count.restype = i64
         L.bvfdtd_kernel_mode.argtypes = [vp, C.POINTER(u32)]
         L.bvfdtd_fused_coverage.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+        L.bvfdtd_padding_nonzeros.argtypes = [vp, C.POINTER(i64)]
         L.bvfdtd_work_items.argtypes = [vp, i32, vp, i64, C.POINTER(i64), C.POINTER(i32)]
         L.bvfdtd_read_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
         L.bvfdtd_write_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
@@ -331,6 +332,12 @@ class Simulation:
         a, b = C.c_int64(0), C.c_int64(0)
         _check(lib().bvfdtd_fused_coverage(self._h, C.byref(a), C.byref(b)), "bvfdtd_fused_coverage")
         return a.value / max(1, b.value)
+
+    def padding_nonzeros(self):
+        """non-zero floats in the zero gaps of the private layout (0 unless a kernel wrote out of bounds)"""
+        n = C.c_int64(0)
+        _check(lib().bvfdtd_padding_nonzeros(self._h, C.byref(n)), "bvfdtd_padding_nonzeros")
+        return n.value
 
     def work_items(self, which):
         """(items (n, 4) int32: tile x, tile y, kz0, kz1; rows per tile) of work list 0 fused / 1 velocity / 2 stress"""

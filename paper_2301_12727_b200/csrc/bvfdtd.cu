@@ -227,6 +227,21 @@ __global__ void k_mask(uint8_t *__restrict__ dst, Params p, int open_lo, int ope
     dst[i + (long long)p.nx * (j + (long long)p.ny * k)] = m;
 }
 
+// counts the non-zero floats of a field allocation that lie OUTSIDE the grid cells (the zero gaps of the private
+// layout, device_params.hpp): no kernel may ever write there
+__global__ void k_padding_nonzeros(const float *__restrict__ f, long long n_floats, Params p, unsigned long long *count) {
+    const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (q >= n_floats) return;
+    const long long r = q - p.org;                 // offset from cell (0,0,0)
+    bool cell = false;
+    if (r >= 0) {
+        const long long k = r / p.sz, rem = r - k * p.sz;
+        const long long j = rem / p.px, i = rem - j * p.px;
+        cell = k < p.nz && j < p.ny && i < p.nx;
+    }
+    if (!cell && f[q] != 0.0f) atomicAdd(count, 1ULL);
+}
+
 dim3 grid3(const Layout &L) { return dim3((L.nx + 127) / 128, L.ny, L.nz); }
 
 size_t field_bytes(const bvfdtd_ctx *c, uint32_t id) {
@@ -1087,6 +1102,24 @@ int bvfdtd_kernel_times(bvfdtd_ctx *c, double ms[4], int64_t launches[4]) {
     if (c->ff_active && c->fplan.n_v == 0) { ms[2] = 0.0; launches[2] = 0; }
     if (c->ff_active && c->fplan.n_s == 0) { ms[3] = 0.0; launches[3] = 0; }
     c->timed_steps = 0;
+    return BVFDTD_OK;
+}
+
+int bvfdtd_padding_nonzeros(bvfdtd_ctx *c, int64_t *count) {
+    if (!c || !count) return BVFDTD_EINVAL;
+    DeviceScope scope(c->device);
+    unsigned long long *d_count = (unsigned long long *)(c->ws + c->W.ctr + 32);
+    CU(cudaMemsetAsync(d_count, 0, 8, c->stream));
+    const long long n = c->L.field_floats;
+    for (int a = 0; a < NGRID_ALL; ++a) {
+        const float *f = (const float *)(c->ws + c->W.field[0] + (size_t)a * (c->W.field[1] - c->W.field[0]));
+        k_padding_nonzeros<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(f, n, c->prm, d_count);
+    }
+    CU(cudaGetLastError());
+    unsigned long long h = 0;
+    CU(cudaMemcpyAsync(&h, d_count, 8, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    *count = (int64_t)h;
     return BVFDTD_OK;
 }
 

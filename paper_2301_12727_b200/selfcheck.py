@@ -26,6 +26,7 @@ def _run(w, steps, flags=0, tuning=0, split=None):
     out["peak"], out["rms"] = sim.read_peak_pressure()
     mode = sim.kernel_mode()
     cov = sim.fused_coverage()
+    assert sim.padding_nonzeros() == 0, "a kernel wrote into the zero gaps of the layout"
     sim.close()
     return out, mode, cov
 
@@ -37,6 +38,9 @@ def _case(name, w, steps, flags=0, tuning=0, split=None, want_fused=False):
     assert float(np.abs(got["p"]).max()) > 0.0, name
     for n in ref:
         assert np.array_equal(ref[n], got[n]), (name, n)
+    again, _, _ = _run(w, steps, flags=flags, tuning=tuning, split=split)      # run to run: no race shows
+    for n in got:
+        assert np.array_equal(again[n], got[n]), (name, n, "not deterministic")
     if want_fused:
         assert "fused" in mode and cov > 0.2, (name, mode, cov)
     print(f"selfcheck {name}: ok ({mode}; fused tile-plane fraction {cov:.2f})")

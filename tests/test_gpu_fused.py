@@ -68,6 +68,7 @@ def test_fused_matches_oracle_and_two_pass(bv, dims, P, seed, wave, steps, vstar
     compare_map(peak, o.get("peak"))
     compare_map(rms, o.get("rms_amp"))
     _same(f, two, bv)
+    assert f.padding_nonzeros() == 0 and two.padding_nonzeros() == 0      # nothing wrote into the zero ghost cells
     # leaving the fused mode in the middle of a run (a caller writes a stress): sigma_yy / sigma_zz are filled in
     # and the run continues on the two passes, bit-identical to the context that never fused
     sxx = f.read_fields("sxx")
