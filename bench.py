@@ -373,17 +373,87 @@ def reference_arm(args):
 
 
 # ---------------------------------------------------------------------------------------------
+# the kernels beyond the hot path: `--next`, and "next_rows" of the default line
+# ---------------------------------------------------------------------------------------------
+def next_rows(dev):
+    """One row per NEXT kernel, timed with CUDA events after warm-up.
+    NEXT-1 k_rayleigh: config 2's focused bowl (aperture 64 mm, F# 1) decomposed at lambda/4 on the
+    whole 300 x 300 entry plane; SFU-bound, 3 MUFU operations (rsqrt, sin, cos) per (source, receiver) pair: peak =
+    the MUFU rate measured by bvfdtd_probe_mufu on this device / 3.
+    NEXT-4 k_bhte: thermal step on config 2's grid; HBM-bound, 21 B per cell-step (rise read + write, Q, dose read +
+    write, material byte), 29 B with the running maximum; peak = the measured copy bandwidth."""
+    import math
+    import torch
+    from paper_2301_12727_b200 import binding as bv
+    from paper_2301_12727_b200 import workloads as wl
+    rows = []
+    f, c0, rho0 = 500e3, 1500.0, 1000.0
+    pos, area = wl.bowl_elements(64e-3, 64e-3, c0 / f / 4)
+    dx = 1e-3 / 3.0
+    xs = (np.arange(300) - 149.5) * dx
+    X, Y = np.meshgrid(xs, xs)
+    rcv = np.stack([X.ravel(), Y.ravel(), np.full(X.size, 15e-3)], axis=1)
+    s = torch.from_numpy(pos.astype(np.float32)).to(dev)
+    wg = torch.from_numpy(np.stack([0.01 * area, np.zeros_like(area)], axis=1).astype(np.float32)).to(dev)
+    r = torch.from_numpy(rcv.astype(np.float32)).to(dev)
+    out = torch.empty((4, r.shape[0]), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev).cuda_stream
+
+    def launch():
+        bv._check(bv.lib().bvfdtd_rayleigh(s.shape[0], s.data_ptr(), wg.data_ptr(), r.shape[0], r.data_ptr(), f, c0, rho0,
+                                           out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), out[3].data_ptr(),
+                                           stream), "bvfdtd_rayleigh")
+    for _ in range(3):
+        launch()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    reps = 20
+    e0.record()
+    for _ in range(reps):
+        launch()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    pairs = float(s.shape[0]) * float(r.shape[0])
+    mufu = bv.probe_mufu(dev)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    rows.append({"kernel": "k_rayleigh", "workload": f"{s.shape[0]} bowl elements x {r.shape[0]} receivers", "ms": ms,
+                 "value": pairs / (ms * 1e-3) / 1e9, "unit": "Gpair/s",
+                 "roofline": {"bound": "alu", "achieved": pairs / (ms * 1e-3) / 1e9, "peak": mufu / 3.0 / 1e9, "unit": "Gpair/s",
+                              "frac": pairs / (ms * 1e-3) / (mufu / 3.0),
+                              "peak_source": f"MUFU rate measured by bvfdtd_probe_mufu ({mufu / 1e12:.2f} Top/s = "
+                                             f"{mufu / sms / 1.965e9:.1f} per SM per clock at 1965 MHz) / 3 MUFU per pair"}})
+    del s, wg, r, out
+    hbm, _ = measured_hbm_peak()
+    tw = wl.thermal_config2()
+    cells = tw["nx"] * tw["ny"] * tw["nz"]
+    for track_max in (False, True):
+        th = bv.Bhte(tw["nx"], tw["ny"], tw["nz"], tw["dx"], tw["dt"], tw["table"], tw["index_map"], track_max=track_max, device=dev)
+        th.set_heat(tw["Q"])
+        th.step(5, tw["duty"])
+        torch.cuda.synchronize()
+        reps = 50
+        e0.record()
+        th.step(reps, tw["duty"])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        b = 29.0 if track_max else 21.0
+        gbs = cells * b / (ms * 1e-3) / 1e9
+        rows.append({"kernel": "k_bhte<%s>" % ("true" if track_max else "false"),
+                     "workload": "thermal step on config 2's grid (300x300x450, 128 materials), %d launches" % reps,
+                     "ms": ms, "value": cells / (ms * 1e-3) / 1e9, "unit": "Gcell-updates/s",
+                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+                                  "bytes_per_cell_step": b}})
+        th.close()
+        del th
+        torch.cuda.empty_cache()
+    return rows
+
+
+# ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
-def kernel_bytes(w, rms_on):
-    """Algorithmic bytes per launch: per cell 49 B (S2) and
-    109 B + 8 (peak) + 8 (sumsq when on) (S3+S4), plus 24 B per PML mask bit in each pass."""
-    bits = w.mean_mask_bits()
-    vel = (49.0 + 24.0 * bits) * w.cells
-    st = (109.0 + 8.0 + (8.0 if rms_on else 0.0) + 24.0 * bits) * w.cells
-    return vel, st
-
-
 def ours(args):
     import torch
     from paper_2301_12727_b200 import build as bv_build
@@ -563,6 +633,7 @@ def ours(args):
                 "kernels": kern}
 
     cpu = cpu_baseline_leg(wl.make(args.config)) if (world == 1 and not args.no_cpu_baseline) else None
+    nxt = next_rows(dev) if (world == 1 and args.config == 2 and not args.no_next and not args.no_cpu_baseline) else None
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -587,6 +658,8 @@ def ours(args):
     }
     if cpu is not None:
         line["cpu_baseline"] = cpu
+    if nxt is not None:
+        line["next_rows"] = nxt            # SURVEY.md 8(f) kernels beyond the hot path (also: bench.py --next)
     print(json.dumps(line), flush=True)
     return 0
 
@@ -601,6 +674,8 @@ def main():
     ap.add_argument("--reference-kernels", action="store_true",
                     help="debug: time the one-thread-per-cell kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--next", action="store_true", help="time only the kernels beyond the hot path (SURVEY.md 8(f)), one JSON line")
+    ap.add_argument("--no-next", action="store_true", help="leave next_rows out of the default line")
     ap.add_argument("--tuning", type=int, default=0, help="bvfdtd_opts.tuning bits (BVFDTD_TUNE_*), experiments")
     ap.add_argument("--traffic-from", default=None,
                     help="ncu `--page raw --csv` export of a --set full capture of this build: write profiles/traffic.csv")
@@ -613,6 +688,12 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return reference_arm(args)
+    if args.next:
+        import torch
+        from paper_2301_12727_b200 import build as bv_build
+        bv_build.build()
+        print(json.dumps({"next_rows": next_rows(torch.device("cuda", 0))}), flush=True)
+        return 0
     return ours(args)
 
 

@@ -287,7 +287,8 @@ int bvfdtd_read_phasor(bvfdtd_ctx *ctx, float *re, float *im, int32_t dst_is_dev
  * of every cell (rho, cL = the table row of the cell's own material; rms_amp of reading P8) reduced
  * over the cells OUTSIDE the PML mask of every z plane, on the device (fp32 per cell, fp64 sums in a
  * fixed order).  plane_sum, plane_max: HOST arrays of nz doubles (W/m^2); planes inside the z slabs
- * give 0.  BVFDTD_ESTATE when no step has been sampled into the rms window yet.  Synchronises the
+ * give 0.  BVFDTD_ESTATE when no step has been sampled into the rms window yet, and on z-slab contexts
+ * (BVFDTD_FLAG_ZLO_OPEN / _ZHI_OPEN: their outer planes are interior planes of the whole domain).  Synchronises the
  * context's stream.
  *
  * bvfdtd_energy_loss (host only): z_m = the interior plane on which max_water is largest (first on
@@ -305,7 +306,8 @@ int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const 
  *     P(r) = (j rho0 c0 k / 2 pi) sum_s W_s exp(-j k |r - r_s|) / |r - r_s|,  k = 2 pi f / c0,
  * W_s = u_s A_s the complex normal velocity times the element area (m^3/s).
  *   src_xyz     DEVICE, n_src x 3 fp32 (m);   src_weight  DEVICE, n_src x 2 fp32 (Re, Im of W_s)
- *   rcv_xyz     DEVICE, n_rcv x 3 fp32 (m); no receiver may coincide with a source element
+ *   rcv_xyz     DEVICE, n_rcv x 3 fp32 (m); a receiver that coincides with a source point gets the sum over the
+ *               other source points (that pair has no finite value and is left out)
  *   p_re, p_im  DEVICE, n_rcv fp32 each (Pa)
  *   amp, delay_s  DEVICE, n_rcv fp32 each, or both NULL: the same field as the (amplitude, delay)
  *               pair bvfdtd_set_source takes for a CW source, p(t) = amp sin(2 pi f (t - delay)),
@@ -313,6 +315,10 @@ int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const 
  *   cuda_stream the launch is asynchronous on this stream
  * fp32 arithmetic, one thread per receiver; no context is needed.
  */
+/* Measured MUFU (special-function unit) rate of the current device in operations per second: a short probe
+ * kernel of independent sin.approx chains, timed with CUDA events.  bvfdtd_rayleigh spends three MUFU operations
+ * per (source, receiver) pair, so its roofline is this rate / 3.  Synchronises. */
+int bvfdtd_probe_mufu(double *ops_per_second, void *cuda_stream);
 int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv,
                     const float *rcv_xyz, double f, double c0, double rho0, float *p_re, float *p_im,
                     float *amp, float *delay_s, void *cuda_stream);
@@ -404,6 +410,13 @@ int bvfdtd_heat_source(bvfdtd_ctx *ctx, const double *absorbed_fraction, double 
  * workspaces of two ranks (device-to-device, NCCL send/recv or a peer-to-peer put).
  */
 int bvfdtd_step_phase(bvfdtd_ctx *ctx, int32_t phase);
+/* The same pass (phase 1 velocity or 2 stress + sensor) over the z planes [k0, k1) only, so that a rank can run the
+ * planes that read no halo plane while the halo exchange is in flight and the others after it:
+ *     velocity / stress at plane k read planes k-2 .. k+2 of the exchanged arrays.
+ * The ranges of one pass may come in any order, must not overlap and must add up to all nz planes; the pass (and, for
+ * phase 2, the step) is complete when they do.  Results do not depend on the split (the kernels are bit-identical
+ * under any z chunking).  BVFDTD_ESTATE out of order, on overlap, or with BVFDTD_FLAG_REFERENCE_KERNELS. */
+int bvfdtd_step_phase_planes(bvfdtd_ctx *ctx, int32_t phase, int32_t k0, int32_t k1);
 int bvfdtd_plane_span(const bvfdtd_grid *grid, uint32_t field_id, int32_t k, int32_t n_planes,
                       size_t *offset_bytes, size_t *bytes);
 

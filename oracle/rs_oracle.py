@@ -12,7 +12,8 @@ source, e^{+j w t} convention,
     P(r) = (j rho0 c0 k / 2 pi) sum_s W_s exp(-j k R_s) / R_s,   R_s = |r - r_s|,  k = 2 pi f / c0,
 
 with W_s = u_s A_s.  The function below is that double sum written out (one receiver at a time, numpy
-over the sources, fp64), nothing else.
+over the sources, fp64), nothing else.  A receiver that coincides with a source point (R_s = 0) takes the sum
+over the OTHER source points: the point-element term has no finite value there (reading).
 """
 from __future__ import annotations
 
@@ -27,7 +28,8 @@ def rayleigh(src_xyz, src_weight, rcv_xyz, f, c0=1500.0, rho0=1000.0):
     out = np.zeros(r.shape[0], dtype=np.complex128)
     for n in range(r.shape[0]):
         R = np.sqrt(((r[n] - s) ** 2).sum(axis=1))
-        out[n] = (w * np.exp(-1j * k * R) / R).sum()
+        ok = R > 0.0
+        out[n] = (w[ok] * np.exp(-1j * k * R[ok]) / R[ok]).sum()
     return 1j * rho0 * c0 * k / (2.0 * np.pi) * out
 
 

@@ -38,10 +38,10 @@ SYMBOLS = (
     "bvfdtd_read_peak_pressure", "bvfdtd_destroy", "bvfdtd_strerror", "bvfdtd_last_cuda_error",
     "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
     "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
-    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_read_phasor",
+    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_probe_mufu", "bvfdtd_read_phasor",
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
-    "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_plane_span",
+    "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_step_phase_planes", "bvfdtd_plane_span",
     "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage", "bvfdtd_work_items", "bvfdtd_padding_nonzeros",
 )
 MODE_REFERENCE, MODE_DENSE, MODE_SIGMA_WRITTEN, MODE_FUSED, MODE_GRAPH = 1, 2, 4, 8, 16
@@ -119,6 +119,7 @@ def lib():
         L.bvfdtd_plane_intensity.argtypes = [vp, vp, vp]
         L.bvfdtd_read_phasor.argtypes = [vp, vp, vp, i32]
         L.bvfdtd_rayleigh.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
+        L.bvfdtd_probe_mufu.argtypes = [C.POINTER(dbl), vp]
         L.bvfdtd_energy_loss.argtypes = [vp, vp, vp, i32, i32, C.POINTER(i32), C.POINTER(dbl), C.POINTER(dbl)]
         L.bvfdtd_max_courant.restype = dbl
         L.bvfdtd_bhte_workspace_bytes.argtypes = [i32, i32, i32, u32, C.POINTER(C.c_size_t)]
@@ -131,6 +132,7 @@ def lib():
         L.bvfdtd_bhte_destroy.argtypes = [vp]
         L.bvfdtd_heat_source.argtypes = [vp, vp, dbl, vp]
         L.bvfdtd_step_phase.argtypes = [vp, i32]
+        L.bvfdtd_step_phase_planes.argtypes = [vp, i32, i32, i32]
         L.bvfdtd_refocus_weights.argtypes = [i64, vp, vp, vp, vp, i32, dbl, dbl, vp, vp, vp, vp]
         L.bvfdtd_plane_span.argtypes = [C.POINTER(Grid), u32, i32, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         _lib = L
@@ -226,6 +228,15 @@ def rayleigh(src_xyz, src_weight, rcv_xyz, f, c0=1500.0, rho0=1000.0, device="cu
     return (p, o[2], o[3]) if want_source else p
 
 
+def probe_mufu(device="cuda:0"):
+    """measured special-function-unit rate of the device (operations per second)"""
+    import torch
+    v = C.c_double(0.0)
+    with torch.cuda.device(torch.device(device)):
+        _check(lib().bvfdtd_probe_mufu(C.byref(v), torch.cuda.current_stream().cuda_stream), "bvfdtd_probe_mufu")
+    return v.value
+
+
 class Simulation:
     """``bvfdtd_create`` .. ``bvfdtd_destroy`` around a torch-owned device workspace."""
 
@@ -299,6 +310,10 @@ class Simulation:
     def step_phase(self, phase):
         """NEXT-5: one pass of the current step (0 inject, 1 velocity, 2 stress + sensor), in order."""
         _check(lib().bvfdtd_step_phase(self._h, int(phase)), "bvfdtd_step_phase")
+
+    def step_phase_planes(self, phase, k0, k1):
+        """NEXT-5: pass 1 or 2 over the planes [k0, k1) only (the ranges of a pass must add up to all planes)."""
+        _check(lib().bvfdtd_step_phase_planes(self._h, int(phase), int(k0), int(k1)), "bvfdtd_step_phase_planes")
 
     @property
     def step_index(self):

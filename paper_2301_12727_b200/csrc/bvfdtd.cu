@@ -127,6 +127,8 @@ struct bvfdtd_ctx {
     PmlAxis pml[3];
     Params prm{};
     int64_t step = 0;
+    int phase_planes = 0; // planes of the pass in progress already run through bvfdtd_step_phase_planes
+    int range_slot = 0;   // next slice of the work-list regions bvfdtd_step_phase_planes writes (round robin of 4)
     int phase_done = 0;   // passes of the current step already run through bvfdtd_step_phase (bit 0 inject, 1 velocity)
     int64_t rms_count = 0;
     // source
@@ -770,7 +772,7 @@ int get_graph(bvfdtd_ctx *c, int regime, int len, cudaGraphExec_t *out) {
 
 int bvfdtd_step(bvfdtd_ctx *c, int64_t n) {
     if (!c || n < 0) return BVFDTD_EINVAL;
-    if (c->phase_done != 0) return BVFDTD_ESTATE;   // a step begun with bvfdtd_step_phase must be finished first
+    if (c->phase_done != 0 || c->phase_planes != 0) return BVFDTD_ESTATE;   // a step begun with bvfdtd_step_phase must be finished first
     DeviceScope scope(c->device);
     if (n >= 2 && graph_ok(c)) {
         // one graph launch per GRAPH_STEPS steps (per step for the remainder) instead of three kernel launches
@@ -810,12 +812,55 @@ int bvfdtd_step_phase(bvfdtd_ctx *c, int32_t phase) {
     // the passes of one step run in order: inject (0), velocity (1), stress + sensor (2)
     const int bit = 1 << phase;
     const int before = bit - 1;                       // every earlier pass must have run, this one not
-    if ((c->phase_done & before) != before || (c->phase_done & bit)) return BVFDTD_ESTATE;
+    if ((c->phase_done & before) != before || (c->phase_done & bit) || c->phase_planes != 0) return BVFDTD_ESTATE;
     int rc = fused_disable(c);          // single passes run on every tile column
     if (rc) return rc;
     rc = run_phases(c, bit);
     if (rc) return rc;
     CU(cudaGetLastError());
+    return BVFDTD_OK;
+}
+
+int bvfdtd_step_phase_planes(bvfdtd_ctx *c, int32_t phase, int32_t k0, int32_t k1) {
+    if (!c || (phase != 1 && phase != 2) || k0 < 0 || k1 <= k0 || k1 > c->L.nz) return BVFDTD_EINVAL;
+    if (c->opts.flags & BVFDTD_FLAG_REFERENCE_KERNELS) return BVFDTD_ESTATE;      // the per-cell kernels sweep whole grids
+    DeviceScope scope(c->device);
+    const int bit = 1 << phase, before = bit - 1;
+    if ((c->phase_done & before) != before || (c->phase_done & bit)) return BVFDTD_ESTATE;
+    if (c->phase_planes + (k1 - k0) > c->L.nz) return BVFDTD_ESTATE;              // ranges of one pass must not overlap
+    int rc = fused_disable(c);
+    if (rc) return rc;
+    // the pass over planes [k0, k1) of every tile column, as a work list in a slice of the list region
+    const Layout &L = c->L;
+    const bool vel = phase == 1;
+    const int ntx = vel ? L.ntxV : L.ntxS, nty = vel ? L.ntyV : c->prm.ntyS;
+    const int nchunk = (k1 - k0 + 47) / 48;
+    std::vector<int4> items;
+    items.reserve((size_t)ntx * nty * nchunk);
+    for (int ch = 0; ch < nchunk; ++ch) {
+        const int a = k0 + (int)((long long)(k1 - k0) * ch / nchunk), b = k0 + (int)((long long)(k1 - k0) * (ch + 1) / nchunk);
+        for (int by = 0; by < nty; ++by)
+            for (int bx = 0; bx < ntx; ++bx) items.push_back(make_int4(bx, by, a, b));
+    }
+    const size_t slice = fused_items_capacity(L) / 4;
+    if (items.size() > slice) return BVFDTD_EINVAL;
+    int4 *d_items = (int4 *)(c->ws + c->W.items[vel ? 1 : 2]) + slice * (size_t)(c->range_slot++ & 3);
+    CU(cudaMemcpyAsync(d_items, items.data(), items.size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    const int64_t step = c->step;
+    const Params p = step_params(c, step, regime_of(c, step), c->sel);
+    if (vel) tiled_velocity(c->plan, p, c->stream, d_items, (int)items.size());
+    else tiled_stress(c->plan, p, c->stream, d_items, (int)items.size());
+    CU(cudaGetLastError());
+    c->phase_planes += k1 - k0;
+    if (c->phase_planes == L.nz) {
+        c->phase_planes = 0;
+        if (vel) c->phase_done |= bit;
+        else {
+            if (p.do_rms || p.do_phasor) c->rms_count++;
+            c->step++;
+            c->phase_done = 0;
+        }
+    }
     return BVFDTD_OK;
 }
 
@@ -974,6 +1019,9 @@ int bvfdtd_plane_intensity(bvfdtd_ctx *c, double *plane_sum, double *plane_max) 
     if (!c || !plane_sum || !plane_max) return BVFDTD_EINVAL;
     DeviceScope scope(c->device);
     if (c->rms_count <= 0 || (c->opts.flags & BVFDTD_FLAG_PHASOR)) return BVFDTD_ESTATE;
+    // a z-slab context holds interior planes where an undivided box has its z slabs: the reduction skips [0, P)
+    // and [nz - P, nz), so it is refused there (reduce the owned planes of the slabs on the caller's side)
+    if (c->opts.flags & (BVFDTD_FLAG_ZLO_OPEN | BVFDTD_FLAG_ZHI_OPEN)) return BVFDTD_ESTATE;
     const Layout &L = c->L;
     double *d_out = (double *)(c->ws + c->W.scratch);          // 2 nz doubles of the dense scratch plane
     k_plane_intensity<<<L.nz, 256, 0, c->stream>>>(c->prm, (const float *)(c->ws + c->W.invz), (float)(1.0 / (double)c->rms_count), d_out);
@@ -1073,6 +1121,31 @@ int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight
                                                               (float)(rho0 * c0 * k / (2.0 * 3.14159265358979323846)), (float)w, p_re, p_im, amp, delay_s);
     CU(cudaGetLastError());
     CU(cudaFreeAsync(d_src, st));
+    return BVFDTD_OK;
+}
+
+int bvfdtd_probe_mufu(double *ops_per_second, void *cuda_stream) {
+    if (!ops_per_second) return BVFDTD_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float *d_out = nullptr;
+    CU(cudaMalloc(&d_out, 4));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int iters = 1 << 14, blocks = 2 * sms;
+    k_mufu_probe<<<blocks, 1024, 0, st>>>(d_out, 64);                  // warm-up
+    CU(cudaEventRecord(e0, st));
+    k_mufu_probe<<<blocks, 1024, 0, st>>>(d_out, iters);
+    CU(cudaEventRecord(e1, st));
+    CU(cudaEventSynchronize(e1));
+    float ms = 0.0f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    CU(cudaGetLastError());
+    *ops_per_second = 4.0 * iters * 1024.0 * blocks / (ms * 1e-3);
     return BVFDTD_OK;
 }
 

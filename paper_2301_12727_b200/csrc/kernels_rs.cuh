@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(128) k_rayleigh(const int n_src, const float4 
                 const float4 s = spos[q];
                 const float dx = x - s.x, dy = y - s.y, dz = z - s.z;
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                const float ir = rs_rsqrt(r2);
+                const float ir = r2 > 0.0f ? rs_rsqrt(r2) : 0.0f;   // a receiver ON a source point: that pair adds nothing
                 const float turns = (r2 * ir) * inv_lambda;                 // k R / 2 pi
                 const float ph = -6.283185307179586f * (turns - rintf(turns));   // -k R reduced to [-pi, pi]
                 const float sn = rs_sin(ph), cs = rs_cos(ph);
@@ -70,6 +70,14 @@ __global__ void __launch_bounds__(128) k_rayleigh(const int n_src, const float4 
         amp[r] = sqrtf(re * re + im * im);
         delay[r] = a / omega;
     }
+}
+
+// MUFU throughput probe: the roofline denominator of k_rayleigh is measured, not assumed.  Every thread runs
+// four independent chains of sin.approx (1024 threads x 2 blocks per SM hide the latency); ops = 4 * iters per thread.
+__global__ void __launch_bounds__(1024) k_mufu_probe(float *__restrict__ out, const int iters) {
+    float a0 = threadIdx.x * 1e-3f, a1 = a0 + 0.25f, a2 = a0 + 0.5f, a3 = a0 + 0.75f;
+    for (int i = 0; i < iters; ++i) { a0 = rs_sin(a0); a1 = rs_sin(a1); a2 = rs_sin(a2); a3 = rs_sin(a3); }
+    if (a0 + a1 + a2 + a3 == 12345.0f) out[0] = a0;     // keeps the chains alive
 }
 
 }  // namespace bvfdtd

@@ -105,19 +105,38 @@ def _view(ws, span):
 
 def exchange_distributed(ws, plan, rank, world, group=None):
     """One halo exchange of the fields in `plan` with both z neighbours (torch.distributed
-    point-to-point, batched; `ws` is the rank's workspace as a flat uint8 tensor)."""
+    point-to-point, batched; `ws` is the rank's workspace as a flat uint8 tensor).  With a backend
+    that cannot move device memory (gloo) the blocks are staged through pinned host buffers."""
+    import torch
     import torch.distributed as dist
-    ops = []
+    staged = ws.is_cuda and dist.get_backend(group) != "nccl"
+    ops, back = [], []
+
+    def buf(span, recv):
+        v = _view(ws, span)
+        if not staged:
+            return v
+        h = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+        if recv:
+            back.append((v, h))
+        else:
+            h.copy_(v, non_blocking=True)
+        return h
+
     for e in plan:
         if "send_lo" in e:
-            ops.append(dist.P2POp(dist.isend, _view(ws, e["send_lo"]), rank - 1, group))
-            ops.append(dist.P2POp(dist.irecv, _view(ws, e["recv_lo"]), rank - 1, group))
+            ops.append(dist.P2POp(dist.isend, buf(e["send_lo"], False), rank - 1, group))
+            ops.append(dist.P2POp(dist.irecv, buf(e["recv_lo"], True), rank - 1, group))
         if "send_hi" in e:
-            ops.append(dist.P2POp(dist.isend, _view(ws, e["send_hi"]), rank + 1, group))
-            ops.append(dist.P2POp(dist.irecv, _view(ws, e["recv_hi"]), rank + 1, group))
+            ops.append(dist.P2POp(dist.isend, buf(e["send_hi"], False), rank + 1, group))
+            ops.append(dist.P2POp(dist.irecv, buf(e["recv_hi"], True), rank + 1, group))
+    if staged:
+        torch.cuda.current_stream(ws.device).synchronize()      # the device-to-host copies of the send blocks
     if ops:
         for r in dist.batch_isend_irecv(ops):
             r.wait()
+    for v, h in back:
+        v.copy_(h, non_blocking=True)
 
 
 def exchange_local(workspaces, plans):
@@ -144,21 +163,76 @@ class _Slab:
         return a[lo:lo + (self.meta["z1"] - self.meta["z0"])]
 
 
-class SlabRank(_Slab):
-    """One rank of a torch.distributed z-slab run (one process per GPU)."""
+def split_ranges(nz_local, lo, hi):
+    """(interior, boundary) plane ranges of a pass: a pass at plane k reads planes k-2 .. k+2 of the exchanged
+    arrays, so the planes [lo + 2, nz - hi - 2) read no halo plane and can run while the exchange is in flight;
+    the owned planes next to an interface run after it.  The halo planes themselves ([0, lo) and [nz - hi, nz)) are
+    in the boundary ranges too: what a pass computes there is overwritten by the next exchange, but every plane must
+    be swept for the pass to complete."""
+    i0 = lo + HALO if lo else 0
+    i1 = nz_local - hi - HALO if hi else nz_local
+    boundary = []
+    if i0 > 0:
+        boundary.append((0, i0))
+    if i1 < nz_local:
+        boundary.append((i1, nz_local))
+    return (i0, i1), boundary
 
-    def __init__(self, w, rank, world, device, group=None, flags=0):
+
+class SlabRank(_Slab):
+    """One rank of a torch.distributed z-slab run (one process per GPU).  Per step, with overlap:
+
+        inject -> [ exchange of the six stresses  ||  velocity pass on the planes that read no halo ]
+               -> velocity pass on the planes next to the interfaces
+               -> [ exchange of the three velocities  ||  stress pass on the planes that read no halo ]
+               -> stress pass on the planes next to the interfaces
+
+    The passes run on the simulation's stream, the exchanges on a side stream of the same device; events order
+    them (the exchange waits for what it sends, the boundary planes wait for what was received)."""
+
+    def __init__(self, w, rank, world, device, group=None, flags=0, overlap=True):
+        import torch
+        self._torch = torch
+        torch.cuda.set_device(torch.device(device))     # NCCL point-to-point runs on the current device
         super().__init__(w, rank, world, device, flags)
         self.group = group
+        self.overlap = overlap
+        self.main = self.sim._stream
+        self.side = torch.cuda.Stream(device=self.sim.device)
+        self.interior, self.boundary = split_ranges(self.w.nz, self.meta["lo"], self.meta["hi"])
+
+    def _exchange(self, plan):
+        torch = self._torch
+        self.side.wait_stream(self.main)                # what is sent was written on the main stream
+        with torch.cuda.stream(self.side):
+            exchange_distributed(self.sim.workspace, plan, self.rank, self.world, self.group)
+
+    def _pass(self, phase, plan):
+        if not self.overlap or self.world == 1:
+            self._exchange(plan)
+            self.main.wait_stream(self.side)
+            self.sim.step_phase(phase)
+            return
+        # the interior planes are enqueued first; the exchange then runs beside them
+        mark = self._torch.cuda.Event()
+        mark.record(self.main)                          # everything the exchange sends is complete here
+        i0, i1 = self.interior
+        if i1 > i0:
+            self.sim.step_phase_planes(phase, i0, i1)
+        self.side.wait_event(mark)
+        with self._torch.cuda.stream(self.side):
+            exchange_distributed(self.sim.workspace, plan, self.rank, self.world, self.group)
+        self.main.wait_stream(self.side)
+        for k0, k1 in self.boundary:
+            self.sim.step_phase_planes(phase, k0, k1)
+        if i1 <= i0 and not self.boundary:
+            self.sim.step_phase(phase)
 
     def step(self, n=1):
-        ws = self.sim.workspace
         for _ in range(int(n)):
             self.sim.step_phase(0)
-            exchange_distributed(ws, self.plan_s, self.rank, self.world, self.group)
-            self.sim.step_phase(1)
-            exchange_distributed(ws, self.plan_v, self.rank, self.world, self.group)
-            self.sim.step_phase(2)
+            self._pass(1, self.plan_s)
+            self._pass(2, self.plan_v)
 
     def close(self):
         self.sim.close()
@@ -167,9 +241,25 @@ class SlabRank(_Slab):
 class SlabGroup:
     """All slabs of a run in one process on one device, stepped in lock step (a correctness vehicle)."""
 
-    def __init__(self, w, n_slabs, device="cuda:0", flags=0):
+    def __init__(self, w, n_slabs, device="cuda:0", flags=0, split=False):
         self.w = w
         self.slabs = [_Slab(w, r, n_slabs, device, flags) for r in range(n_slabs)]
+        self.split = split          # run every pass the way SlabRank overlaps it: interior planes, exchange, boundary planes
+
+    def _pass(self, phase, ws, plans):
+        if not self.split:
+            exchange_local(ws, plans)
+            for s in self.slabs:
+                s.sim.step_phase(phase)
+            return
+        ranges = [split_ranges(s.w.nz, s.meta["lo"], s.meta["hi"]) for s in self.slabs]
+        for s, ((i0, i1), _) in zip(self.slabs, ranges):
+            if i1 > i0:
+                s.sim.step_phase_planes(phase, i0, i1)
+        exchange_local(ws, plans)
+        for s, (_, boundary) in zip(self.slabs, ranges):
+            for k0, k1 in boundary:
+                s.sim.step_phase_planes(phase, k0, k1)
 
     def step(self, n=1):
         ws = [s.sim.workspace for s in self.slabs]
@@ -178,12 +268,8 @@ class SlabGroup:
         for _ in range(int(n)):
             for s in self.slabs:
                 s.sim.step_phase(0)
-            exchange_local(ws, ps)
-            for s in self.slabs:
-                s.sim.step_phase(1)
-            exchange_local(ws, pv)
-            for s in self.slabs:
-                s.sim.step_phase(2)
+            self._pass(1, ws, ps)
+            self._pass(2, ws, pv)
 
     def read_fields(self, name):
         return np.concatenate([s.owned(s.sim.read_fields(name)) for s in self.slabs], axis=0)

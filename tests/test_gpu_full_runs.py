@@ -32,6 +32,7 @@ from test_gpu_parity import GROUPS, compare_map
 pytestmark = pytest.mark.gpu
 
 DEFAULT_MODE = "tiled, tile-class skipping, fused sweep in all-fluid tile columns"
+SMALL_MODE = "tiled, tile-class skipping"
 CACHE = os.environ.get("BVFDTD_ORACLE_CACHE", "/tmp/bvfdtd_oracle_cache")
 OUT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
 
@@ -135,11 +136,12 @@ def _run_and_compare(bv, w, steps, state=None, tag=None):
     ref = OracleResult(w, steps, state)
     sim = bv.Simulation.from_workload(w)
     # the default path on these grids: tile-class skipping, the fused sweep in the all-fluid tile columns, graphs
-    assert sim.kernel_mode() == DEFAULT_MODE and sim.mode_bits() & bv.MODE_GRAPH
+    want_mode = DEFAULT_MODE if w.cells >= 6000000 else SMALL_MODE      # (the library fuses from 6 M cells on)
+    assert sim.kernel_mode() == want_mode and sim.mode_bits() & bv.MODE_GRAPH
     for n, a in (state or {}).items():
         assert n in ("vx", "vy", "vz")                # anything else would switch optimisations off
         sim.write_fields(n, a)
-    assert sim.kernel_mode() == DEFAULT_MODE
+    assert sim.kernel_mode() == want_mode
     sim.step(steps)
     rep = compare_full(sim, ref)
     peak, rms = sim.read_peak_pressure()
@@ -172,6 +174,13 @@ def _run_and_compare(bv, w, steps, state=None, tag=None):
         except OSError:
             pass
     return out
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_config01_full_length(bv, cfg):
+    """configs 0 and 1 over their 300 / 800 steps on the default path (two passes, graph replay)"""
+    w = wl.make(cfg)
+    _run_and_compare(bv, w, w.steps, tag=f"cfg{cfg}")
 
 
 def test_config2_all_3000_steps_from_zero_state(bv):

@@ -108,3 +108,32 @@ def test_gpu_rayleigh_matches_oracle():
     p2 = bv.rayleigh(pos, 0.01 * area, np.array([[0.0, 0.0, 64e-3]]), F, C0, RHO, want_source=False)
     ref2 = 1j * RHO * C0 * K / (2 * math.pi) * 0.01 * area.sum() * np.exp(-1j * K * 64e-3) / 64e-3
     assert abs(p2[0] - ref2) < 2e-4 * abs(ref2)
+
+
+def test_oracle_receiver_on_a_source_point_takes_the_other_sources():
+    """reading: a pair with R = 0 is left out; the field there is the plain sum of the rest"""
+    rng = np.random.Generator(np.random.PCG64(wl.SEED_BASE + 78))
+    pos = rng.random((7, 3)) * 1e-2
+    wgt = rng.random(7) + 1j * rng.random(7)
+    got = rs.rayleigh(pos, wgt, pos[[3]], F, C0, RHO)[0]
+    rest = np.delete(np.arange(7), 3)
+    want = rs.rayleigh(pos[rest], wgt[rest], pos[[3]], F, C0, RHO)[0]
+    assert np.isfinite(got) and abs(got - want) <= 1e-14 * abs(want)
+
+
+@pytest.mark.gpu
+def test_gpu_rayleigh_receiver_on_a_source_point_and_mufu_probe():
+    from paper_2301_12727_b200 import build as bv_build
+    bv_build.build()
+    from paper_2301_12727_b200 import binding as bv
+    pos, area = wl.disc_elements(5e-3, LAM / 4)
+    rcv = np.concatenate([pos[[0, 17]], [[0.0, 0.0, 4e-3]]], axis=0)      # two receivers ON source points
+    p, amp, delay = bv.rayleigh(pos, 0.01 * area, rcv, F, C0, RHO)
+    ref = rs.rayleigh(pos.astype(np.float32), (0.01 * area).astype(np.complex64), rcv.astype(np.float32), F, C0, RHO)
+    assert np.isfinite(p).all() and np.isfinite(amp).all() and np.isfinite(delay).all()
+    assert np.abs(p - ref).max() <= 2e-4 * np.abs(ref).max()
+    # the measured MUFU rate that k_rayleigh's roofline uses: at least one lane per scheduler, at most 32 per SM
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    rate = bv.probe_mufu()
+    assert 4 * sms * 1e9 < rate < 32 * sms * 2.2e9, rate

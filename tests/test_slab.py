@@ -3,7 +3,9 @@
 CPU: the partition, the local workloads, the halo plan (``bvfdtd_plane_span`` is host-only) and the
 point-to-point exchange itself on CPU byte tensors under gloo with 2 and 3 ranks.
 GPU (one device): all slabs of a run in one process, stepped in lock step, reproduce the undivided
-run BIT FOR BIT on every owned plane (state, peak, rms), with the tiled and the per-cell kernels.
+run BIT FOR BIT on every owned plane (state, peak, rms), with the tiled and the per-cell kernels, whole passes
+and passes split around the exchange; SlabRank as a two-process torch.distributed job (gloo, staged exchange) on
+the one GPU, against the undivided run and the oracle.
 """
 from __future__ import annotations
 
@@ -171,3 +173,116 @@ def test_gpu_step_phase_order_is_enforced():
     b.step_phase(1); b.step_phase(2)
     assert b.step_index == 4
     a.close(); b.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n_slabs", [2, 3])
+def test_gpu_slabs_split_passes_match_bitwise_and_the_oracle(n_slabs):
+    """every pass split the way SlabRank overlaps it with the exchange (planes that read no halo first, the planes
+    next to the interfaces after the exchange, bvfdtd_step_phase_planes): bit-identical to the undivided run, and
+    the stitched field meets the oracle within north_star's bars"""
+    from oracle import fdtd_oracle as orc
+    from test_gpu_parity import compare_map
+    w = wl.random_domain(70, 45, 96, 6, seed=33, steps=40, waveform=1)
+    w.rms_begin = 18
+    full = bv.Simulation.from_workload(w, device="cuda:0")
+    full.step(w.steps)
+    grp = slab.SlabGroup(w, n_slabs, device="cuda:0", split=True)
+    grp.step(w.steps)
+    o = orc.Oracle.from_workload(w)
+    o.step(w.steps)
+    for name in bv.FIELDS:
+        a, b = full.read_fields(name), grp.read_fields(name)
+        assert np.array_equal(a, b), name
+        ref = o.get(name)
+        nrm = np.linalg.norm(ref)
+        if nrm > 0:
+            assert np.linalg.norm(b - ref) / nrm <= 1e-4, name
+    pk, rm = full.read_peak_pressure()
+    pk2, rm2 = grp.read_peak_pressure()
+    assert np.array_equal(pk, pk2) and np.array_equal(rm, rm2)
+    compare_map(pk2, o.get("peak"))
+    compare_map(rm2, o.get("rms_amp"))
+    full.close(); grp.close()
+
+
+@pytest.mark.gpu
+def test_gpu_step_phase_planes_rules():
+    w = wl.random_domain(40, 36, 60, 6, seed=3, steps=4)
+    a = bv.Simulation.from_workload(w, device="cuda:0")
+    b = bv.Simulation.from_workload(w, device="cuda:0")
+    a.step(2)
+    for _ in range(2):
+        b.step_phase(0)
+        b.step_phase_planes(1, 40, 60); b.step_phase_planes(1, 0, 13); b.step_phase_planes(1, 13, 40)     # any order
+        with pytest.raises(bv.BvfdtdError):
+            b.step_phase_planes(1, 0, 5)              # the velocity pass is complete
+        b.step_phase_planes(2, 0, 31)
+        with pytest.raises(bv.BvfdtdError):
+            b.step_phase(2)                           # a split pass is in progress
+        with pytest.raises(bv.BvfdtdError):
+            b.step_phase_planes(2, 20, 60)            # more planes than the grid has: an overlap
+        b.step_phase_planes(2, 31, 60)
+    assert b.step_index == 2
+    for name in bv.FIELDS:
+        assert np.array_equal(a.read_fields(name), b.read_fields(name)), name
+    with pytest.raises(bv.BvfdtdError):
+        b.step_phase_planes(1, 0, 60)                 # velocity before inject
+    a.close(); b.close()
+
+
+def _rank_worker(rank, world, port, q, overlap):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = wl.random_domain(70, 45, 96, 6, seed=35, steps=30, waveform=1)
+        w.rms_begin = 12
+        r = slab.SlabRank(w, rank, world, "cuda:0", overlap=overlap)
+        r.step(w.steps)
+        out = {n: r.owned(r.sim.read_fields(n)) for n in ("vx", "vz", "sxx", "sxy", "rzz", "p")}
+        pk, rm = r.sim.read_peak_pressure()
+        out["peak"], out["rms"] = r.owned(pk), r.owned(rm)
+        q.put((rank, out))
+        dist.barrier()
+        r.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("overlap", [True, False])
+def test_gpu_slab_ranks_as_two_processes(overlap):
+    """SlabRank as a real torch.distributed job: two processes, one rank each, both on this box's one GPU, halo
+    blocks staged through pinned host memory because gloo cannot move device memory (NCCL refuses two ranks on one
+    device; the kernels of the two ranks never wait on one another, only the hosts do).  The stitched result is
+    bit-identical to the undivided run and meets the oracle."""
+    import torch.multiprocessing as mp
+    from oracle import fdtd_oracle as orc
+    w = wl.random_domain(70, 45, 96, 6, seed=35, steps=30, waveform=1)
+    w.rms_begin = 12
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rank_worker, args=(r, 2, port, q, overlap)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=300) for _ in procs)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    full = bv.Simulation.from_workload(w, device="cuda:0")
+    full.step(w.steps)
+    o = orc.Oracle.from_workload(w)
+    o.step(w.steps)
+    for n in ("vx", "vz", "sxx", "sxy", "rzz", "p"):
+        got = np.concatenate([res[0][n], res[1][n]], axis=0)
+        assert np.array_equal(got, full.read_fields(n)), n
+        ref = o.get(n)
+        assert np.linalg.norm(got - ref) <= 1e-4 * np.linalg.norm(ref), n
+    pk, rm = full.read_peak_pressure()
+    assert np.array_equal(np.concatenate([res[0]["peak"], res[1]["peak"]], axis=0), pk)
+    assert np.array_equal(np.concatenate([res[0]["rms"], res[1]["rms"]], axis=0), rm)
+    full.close()
