@@ -165,7 +165,8 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
  * t < n_cycles/f, 1 after; w = 0 for t < 0.
  *   cell, amp, delay_s   host arrays of n_src entries; cells are linear indices, unique, inside
  *                        the grid and outside the PML mask.  n_src = 0 removes the source.
- * The library keeps its own device copy (the only device memory it allocates itself).
+ * The library keeps its own device copy in the workspace (room for 4 nx ny source cells; only a longer list gets a
+ * library-owned allocation).  The call does not synchronise: the arrays are packed on the host before it returns.
  * Errors: EINVAL (cell outside the grid / inside the PML / duplicate, f_src <= 0, n_cycles < 1,
  * waveform not 0/1), ECUDA.
  */
@@ -177,6 +178,11 @@ int bvfdtd_set_source(bvfdtd_ctx *ctx, int64_t n_src, const int64_t *cell, const
  * velocity update (Eq. 1 rows 1-3) -> S3 stress + memory-variable update (Eq. 1 rows 4-9, L148-L152)
  * with the S4 sensor (running peak of |p|, sum of p^2) fused into it.  No host<->device traffic.
  * Legal before bvfdtd_set_source (zero source).  n >= 0.
+ * How the steps are launched is the library's choice and never changes a bit of the result (bvfdtd_kernel_mode
+ * names it): for n >= 2 it replays CUDA graphs of 8 steps / 1 step per sensor regime (captured on a stream of its
+ * own on first use; the injection then takes the step index from a device counter); on grids of 6 M cells or more
+ * the tile columns without a solid cell within reach run a fused single sweep (v and sigma in one z-march over
+ * ping-ponged copies of v and the normal stresses) and only the others the two passes.
  */
 int bvfdtd_step(bvfdtd_ctx *ctx, int64_t n);
 

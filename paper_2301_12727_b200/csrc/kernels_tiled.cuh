@@ -1136,6 +1136,17 @@ inline int round128(int v) { return (v + 127) / 128 * 128; }
 // 90 90 90 90 45 25 12 8 planes -> 39.0 Gcell/s, nine equal chunks of 50 -> 36.6, three of 150 -> 33.6.
 inline ZChunks plan_chunks(int nz, long long tiles, long long slots, double waves) {
     ZChunks z;
+    // small grids (configs 0, 1): the whole launch fits the resident CTAs about once.  A CTA's time is its number
+    // of iterations (planes + 4 priming planes; the data sits in L2), so the launch is cut into as many equal
+    // chunks as fill ONE wave -- config 0: 8 tiles x 32 chunks of 2 planes (6 iterations instead of 12), config 1:
+    // 32 tiles x 9 chunks instead of 16 chunks in two waves
+    if (tiles * ((nz + 7) / 8) <= slots + slots / 3 && tiles <= slots) {
+        int n = (int)std::min<long long>(slots / tiles, std::min(nz / 2, MAX_CHUNKS));
+        n = std::max(1, n);
+        for (int c = 0; c <= n; ++c) z.b[c] = (int)((long long)nz * c / n);
+        z.n = n;
+        return z;
+    }
     int big = (int)std::floor(waves * (double)slots / (double)tiles + 0.5);
     big = std::max(1, std::min(big, std::min(nz / 8, MAX_CHUNKS - 8)));
     const int len = std::max(8, (nz + big) / (big + 1));

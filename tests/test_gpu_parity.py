@@ -31,12 +31,13 @@ def bv():
 
 
 def compare_state(sim, o, rel=REL_L2, fields=None):
-    """rel-L2 per field; returns the worst ratio (error / bar)."""
+    """rel-L2 per field (bar `rel`) and max abs error against the largest value of the field's group (bar 20 rel)."""
     worst = 0.0
     report = {}
     for group in GROUPS:
         ref = {n: o.get(n) for n in group}
         gmax = max(np.linalg.norm(ref[n]) for n in group)
+        gabs = max(float(np.abs(ref[n]).max()) for n in group)
         for n in group:
             if fields is not None and n not in fields:
                 continue
@@ -48,6 +49,11 @@ def compare_state(sim, o, rel=REL_L2, fields=None):
             r = err / denom if denom > 0 else err
             report[n] = r
             worst = max(worst, r / rel)
+            # no single cell far off either: max abs error against the largest value of the group
+            if gabs > 0:
+                m = float(np.abs(got - ref[n]).max()) / gabs
+                report[n + ":max_abs"] = m
+                worst = max(worst, m / (20.0 * rel))
     assert worst <= 1.0, report
     return report
 
