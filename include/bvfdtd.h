@@ -413,7 +413,9 @@ int bvfdtd_heat_source(bvfdtd_ctx *ctx, const double *absorbed_fraction, double 
  * contiguous block that holds planes k .. k + n_planes - 1 of state field `field_id` (0-14) in the
  * private layout.  The block includes the layout's padding, which is identical on both sides of an
  * interface because x and y extents are: a halo exchange is a plain copy of this block between the
- * workspaces of two ranks (device-to-device, NCCL send/recv or a peer-to-peer put).
+ * workspaces of two ranks (device-to-device, NCCL send/recv or a peer-to-peer put).  The block is where a z-slab
+ * context (BVFDTD_FLAG_ZLO_OPEN / _ZHI_OPEN) keeps the field: such contexts never run the fused mode, whose steps
+ * alternate between two copies of v and the normal stresses.
  */
 int bvfdtd_step_phase(bvfdtd_ctx *ctx, int32_t phase);
 /* The same pass (phase 1 velocity or 2 stress + sensor) over the z planes [k0, k1) only, so that a rank can run the
