@@ -246,6 +246,14 @@ int bvfdtd_kernel_times(bvfdtd_ctx *ctx, double ms[4], int64_t launches[4]);
 /* How much of the grid the fused single sweep takes: 64 x 8 tile-planes it runs / all tile-planes
  * (0 when the context is not in the fused mode, BVFDTD_MODE_FUSED).  Host-side query. */
 int bvfdtd_fused_coverage(const bvfdtd_ctx *ctx, int64_t *planes_fused, int64_t *planes_all);
+/* Host only (no CUDA device needed): the work lists the fused mode builds from the per-(64 x 8 tile, plane) class
+ * bytes of S0 (bit 0: no solid cell within 4 cells of the tile in this plane, bit 1: a lossy cell in the tile;
+ * cls[(tile_x + ntx * tile_y) * nz + k], ntx = ceil(nx / 64), nty = ceil(ny / 8)).  Same code path bvfdtd_create
+ * uses; exposed so that the partition and the z-slab rules can be tested anywhere.  which / items / n_items as in
+ * bvfdtd_work_items; slots = resident CTAs assumed for every kernel; flags (or NULL): ntx * nty * (nz + 4) words,
+ * (tile, plane + 2), bit 2 = plane in a fused run, bit 3 / 4 = the run also writes sigma_yy / sigma_zz there. */
+int bvfdtd_fused_lists_host(const bvfdtd_grid *grid, const uint8_t *cls, int32_t stress_tile_rows, int32_t slots,
+                            int32_t which, int32_t *items, int64_t capacity, int64_t *n_items, uint32_t *flags);
 /* Self-check (compute-sanitizer is not available everywhere): the number of non-zero floats in the zero gaps of
  * the private layout of all 25 grid arrays (x beyond nx, the two extra rows, the two planes before and after: the
  * zero ghost of reading P4, which no kernel may write).  0 on a healthy context.  Synchronises the stream. */

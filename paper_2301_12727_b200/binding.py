@@ -42,7 +42,7 @@ SYMBOLS = (
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_step_phase_planes", "bvfdtd_plane_span",
-    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage", "bvfdtd_work_items", "bvfdtd_padding_nonzeros",
+    "bvfdtd_refocus_weights", "bvfdtd_rms_count", "bvfdtd_kernel_mode", "bvfdtd_fused_coverage", "bvfdtd_work_items", "bvfdtd_padding_nonzeros", "bvfdtd_fused_lists_host",
 )
 MODE_REFERENCE, MODE_DENSE, MODE_SIGMA_WRITTEN, MODE_FUSED, MODE_GRAPH = 1, 2, 4, 8, 16
 BHTE_TRACK_MAX = 1
@@ -101,6 +101,7 @@ def lib():
         L.bvfdtd_rms_count.restype = i64
         L.bvfdtd_kernel_mode.argtypes = [vp, C.POINTER(u32)]
         L.bvfdtd_fused_coverage.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+        L.bvfdtd_fused_lists_host.argtypes = [C.POINTER(Grid), vp, i32, i32, i32, vp, i64, C.POINTER(i64), vp]
         L.bvfdtd_padding_nonzeros.argtypes = [vp, C.POINTER(i64)]
         L.bvfdtd_work_items.argtypes = [vp, i32, vp, i64, C.POINTER(i64), C.POINTER(i32)]
         L.bvfdtd_read_fields.argtypes = [vp, u32, vp, C.c_size_t, i32]
@@ -183,6 +184,25 @@ def pml_mask(nx, ny, nz, pml):
     m = np.zeros((nz, ny, nx), dtype=np.uint8)
     _check(lib().bvfdtd_pml_mask(C.byref(g), m.ctypes.data), "bvfdtd_pml_mask")
     return m
+
+
+def fused_lists_host(nx, ny, nz, pml, cls, stress_tile_rows=8, slots=444):
+    """host-only: (fused items, velocity items, stress items, flag words (nty, ntx, nz + 4)) for class bytes
+    cls[(nty, ntx, nz)] (bit 0 fluid within reach, bit 1 lossy), as bvfdtd_create builds them"""
+    g = Grid(nx, ny, nz, pml)
+    ntx, nty = (nx + 63) // 64, (ny + 7) // 8
+    c = np.ascontiguousarray(cls, dtype=np.uint8).reshape(nty, ntx, nz)
+    flags = np.zeros((nty, ntx, nz + 4), dtype=np.uint32)
+    out = []
+    for which in range(3):
+        n = C.c_int64(0)
+        _check(lib().bvfdtd_fused_lists_host(C.byref(g), c.ctypes.data, stress_tile_rows, slots, which, None, 0, C.byref(n), None),
+               "bvfdtd_fused_lists_host")
+        a = np.zeros((max(1, n.value), 4), dtype=np.int32)
+        _check(lib().bvfdtd_fused_lists_host(C.byref(g), c.ctypes.data, stress_tile_rows, slots, which, a.ctypes.data, n.value,
+                                             C.byref(n), flags.ctypes.data), "bvfdtd_fused_lists_host")
+        out.append(a[:n.value])
+    return out[0], out[1], out[2], flags
 
 
 def max_courant(table, f0, dt, dx):

@@ -1210,6 +1210,22 @@ int bvfdtd_work_items(bvfdtd_ctx *c, int32_t which, int32_t *items, int64_t capa
     return BVFDTD_OK;
 }
 
+int bvfdtd_fused_lists_host(const bvfdtd_grid *grid, const uint8_t *cls, int32_t stress_tile_rows, int32_t slots, int32_t which,
+                            int32_t *items, int64_t capacity, int64_t *n_items, uint32_t *flags) {
+    if (!grid_ok(grid) || !cls || (stress_tile_rows != 8 && stress_tile_rows != 16) || slots < 1 || which < 0 || which > 2 ||
+        !n_items || capacity < 0 || (capacity > 0 && !items))
+        return BVFDTD_EINVAL;
+    const Layout L = make_layout(*grid);
+    const std::vector<uint8_t> c(cls, cls + (size_t)L.ntxV * L.ntyV * L.nz);
+    const FusedLists lists = fused_lists(L, c, stress_tile_rows, slots, slots, slots);
+    const std::vector<int4> &v = which == 0 ? lists.f : which == 1 ? lists.v : lists.s;
+    *n_items = (int64_t)v.size();
+    const size_t m = (size_t)std::min<int64_t>((int64_t)v.size(), capacity);
+    if (m) std::memcpy(items, v.data(), m * sizeof(int4));
+    if (flags) std::memcpy(flags, lists.flags.data(), lists.flags.size() * 4);
+    return BVFDTD_OK;
+}
+
 int bvfdtd_fused_coverage(const bvfdtd_ctx *c, int64_t *planes_fused, int64_t *planes_all) {
     if (!c || !planes_fused || !planes_all) return BVFDTD_EINVAL;
     *planes_fused = c->ff_active ? c->fplan.planes_f : 0;
