@@ -283,7 +283,8 @@ int fused_setup(bvfdtd_ctx *c) {
     // small grids are launch-bound and L2-resident: a third kernel per step costs more than the bytes it saves
     // (config 1, 128^3: 22 Gcell/s with the two passes, 17.7 fused); BVFDTD_TUNE_FUSED forces the fused mode
     if ((long long)L.nx * L.ny * L.nz < 6000000LL && !(c->opts.tuning & BVFDTD_TUNE_FUSED)) return BVFDTD_OK;
-    int rc = fused_plan_create(c->fplan, c->plan, L, c->prm, c->ws + c->W.psi[6], (long long)(c->W.psi[7] - c->W.psi[6]));
+    int rc = fused_plan_create(c->fplan, c->plan, L, c->prm, c->ws + c->W.psi[6], (long long)(c->W.psi[7] - c->W.psi[6]),
+                               (int)((c->opts.tuning >> 16) & 3u));
     if (rc == BVFDTD_EINVAL) return BVFDTD_OK;                 // the stages do not fit: stay with the two passes
     if (rc) return cuda_fail(cudaGetLastError(), "fused_plan_create");
     uint8_t *d_cls = (uint8_t *)(c->ws + c->W.cls);
@@ -297,7 +298,7 @@ int fused_setup(bvfdtd_ctx *c) {
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_fluid_fused<CfgF>, CfgF::NT, c->fplan.smem));
     const int sty = c->plan.s16 ? CfgS::TY : CfgS8::TY;
     const FusedLists lists = fused_lists(L, cls, sty, sms * std::max(1, occ_f), sms * std::max(1, c->plan.occ_v_res),
-                                         sms * std::max(1, c->plan.occ_s_res));
+                                         sms * std::max(1, c->plan.occ_s_res), (int)((c->opts.tuning >> 8) & 0xffu));
     const long long planes_all = (long long)L.ntxV * L.ntyV * L.nz;
     c->fplan.planes_f = lists.planes_f;
     c->fplan.planes_all = planes_all;
@@ -421,7 +422,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     if (!grid_ok(grid) || !table || !index_map || !opts || !d_workspace) return BVFDTD_EINVAL;
     if (!(dx > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dt)) return BVFDTD_EINVAL;
     constexpr uint32_t TUNE_ALL = BVFDTD_TUNE_VEL_2CTA | BVFDTD_TUNE_VEL_3CTA | BVFDTD_TUNE_STRESS_8 | BVFDTD_TUNE_STRESS_16 |
-                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED | BVFDTD_TUNE_FUSED;
+                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED | BVFDTD_TUNE_FUSED | 0x3ff00u;   // + the two experiment fields
     if (!(opts->f0 > 0.0) || (opts->tuning & ~TUNE_ALL) != 0) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_VEL_2CTA) && (opts->tuning & BVFDTD_TUNE_VEL_3CTA)) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_STRESS_8) && (opts->tuning & BVFDTD_TUNE_STRESS_16)) return BVFDTD_EINVAL;
@@ -528,6 +529,8 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
         PlanTuning tune;
         tune.occ_v = (opts->tuning & BVFDTD_TUNE_VEL_2CTA) ? 2 : (opts->tuning & BVFDTD_TUNE_VEL_3CTA) ? 3 : 0;
         tune.stress_ty = (opts->tuning & BVFDTD_TUNE_STRESS_8) ? 8 : (opts->tuning & BVFDTD_TUNE_STRESS_16) ? 16 : 0;
+        tune.fused_chunk = (int)((opts->tuning >> 8) & 0xffu);
+        tune.l2_promotion = (int)((opts->tuning >> 16) & 3u);
         rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride, (opts->flags & BVFDTD_FLAG_DENSE) != 0, tune);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
         c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;

@@ -478,7 +478,8 @@ struct FusedLists {
 
 // cls: one byte per (64 x 8 tile, plane) from k_fused_class.  sty = rows of a stress tile (8 or 16): a stress
 // tile of 16 rows is fused only as a whole.  slots_* = resident CTAs of the device for each kernel.
-inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, int sty, int slots_f, int slots_v, int slots_s) {
+inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, int sty, int slots_f, int slots_v, int slots_s,
+                              int fused_chunk = 0) {
     FusedLists out;
     const int ntx = L.ntxV, nty = L.ntyV, nz = L.nz, P = L.P, TX = CfgF::TX, TY = CfgF::TY;
     const int LMIN = 16;
@@ -590,7 +591,7 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
             k0 = k1;
         }
     };
-    const int len_f = wave_len(rf, slots_f, 24, 128), len_v = wave_len(rv, slots_v, 16, 96), len_s = wave_len(rs, slots_s, 16, 96);
+    const int len_f = fused_chunk > 0 ? fused_chunk : wave_len(rf, slots_f, 24, 128), len_v = wave_len(rv, slots_v, 16, 96), len_s = wave_len(rs, slots_s, 16, 96);
     for (const Run &r : rf) split(out.f, r.bx, r.by, r.a, r.b, len_f, true);
     for (const Run &r : rv) split(out.v, r.bx, r.by, r.a, r.b, len_v, false);
     for (const Run &r : rs) split(out.s, r.bx, r.by, r.a, r.b, len_s, false);
@@ -615,7 +616,7 @@ inline size_t fused_items_capacity(const Layout &L) { return (size_t)L.ntxV * L.
 
 // tensor maps and stage plans of the fused sweep (after tiled_plan_create)
 inline int fused_plan_create(FusedPlan &fp, const TiledPlan &tp, const Layout &L, const Params &p, char *psi_y_base,
-                             long long psi_y_stride) {
+                             long long psi_y_stride, int l2_promotion = 0) {
     using C = CfgF;
     using FS = FStage<C>;
     void *fn = nullptr;
@@ -634,7 +635,7 @@ inline int fused_plan_create(FusedPlan &fp, const TiledPlan &tp, const Layout &L
         const cuuint64_t gstr[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.sz * 4, (cuuint64_t)fstride};
         const cuuint32_t box[4] = {(cuuint32_t)FS::EX, (cuuint32_t)FS::EY, 1, 1};
         if (enc(&fp.maps.boxE, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                CU_TENSOR_MAP_SWIZZLE_NONE, l2_promotion_of(l2_promotion), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return BVFDTD_ECUDA;
     }
     {
@@ -642,7 +643,7 @@ inline int fused_plan_create(FusedPlan &fp, const TiledPlan &tp, const Layout &L
         const cuuint64_t mstr[2] = {(cuuint64_t)L.px, (cuuint64_t)L.sz};
         const cuuint32_t mbox[3] = {(cuuint32_t)FS::MXF, (cuuint32_t)FS::MYF, 1};
         if (enc(&fp.maps.mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void *)p.mat, mdim, mstr, mbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                CU_TENSOR_MAP_SWIZZLE_NONE, l2_promotion_of(l2_promotion), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return BVFDTD_ECUDA;
     }
     if (L.P > 0) {
@@ -650,7 +651,7 @@ inline int fused_plan_create(FusedPlan &fp, const TiledPlan &tp, const Layout &L
         const cuuint64_t s[3] = {(cuuint64_t)L.px * 4, (cuuint64_t)L.px * 2 * L.P * 4, (cuuint64_t)psi_y_stride};
         const cuuint32_t b[4] = {(cuuint32_t)C::TX, (cuuint32_t)C::BY, 1, 1};
         if (enc(&fp.maps.psyE, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, psi_y_base, d, s, b, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                CU_TENSOR_MAP_SWIZZLE_NONE, l2_promotion_of(l2_promotion), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
             return BVFDTD_ECUDA;
     }
     // stage plans: fixed slots, then 2 x-psi slots, [psi[7] rows (B box) + psi[10] (D box)], [2 z-psi D boxes]

@@ -1130,6 +1130,10 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 inline int round128(int v) { return (v + 127) / 128 * 128; }
+inline CUtensorMapL2promotion l2_promotion_of(int k) {
+    return k == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : k == 2 ? CU_TENSOR_MAP_L2_PROMOTION_NONE
+         : k == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+}
 
 // z chunks: a few long equal chunks (about 2.6 waves of resident CTAs; every chunk costs 4 priming
 // planes) followed by a tail of chunks of halving length, not below 8 planes.  Measured on config 2:
@@ -1177,12 +1181,12 @@ inline bool parse_chunks(const char *env, int nz, ZChunks &z) {   // "56,56,..."
 
 template <class C>
 inline int encode_maps(PFN_encodeTiled enc, TiledMaps &maps, const Layout &L, const Params &p, char *const psi_base[3],
-                       const long long psi_stride[3], int wxb) {
+                       const long long psi_stride[3], int wxb, int l2_promotion = 0) {
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     auto encode = [&](CUtensorMap *m, CUtensorMapDataType ty, int rank, void *base, const cuuint64_t *gdim, const cuuint64_t *gstr,
                       const cuuint32_t *box, const char *what) -> int {
         CUresult r = enc(m, ty, rank, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                         l2_promotion_of(l2_promotion), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) {
             std::snprintf(tiled_err_buf(), 256, "cuTensorMapEncodeTiled(%s) failed: %d", what, (int)r);
             return BVFDTD_ECUDA;
@@ -1261,7 +1265,10 @@ inline StagePlan make_stage(const Layout &L, int fixed, int ns, int extra, int w
 struct PlanTuning {
     int occ_v = 0;      // 0 auto, 2 or 3 resident CTAs of the velocity pass
     int stress_ty = 0;  // 0 auto, 8 or 16 rows per stress tile
+    int l2_promotion = 0;   // experiments: 0 = 128 B (default), 1 = 64 B, 2 = none, 3 = 256 B (field tensor maps)
+    int fused_chunk = 0;    // experiments: planes per chunk of the fused sweep (0 = the library's choice)
 };
+
 inline const char *dev_knob(const char *name) {
 #ifdef BVFDTD_DEV_KNOBS
     return std::getenv(name);
@@ -1291,7 +1298,7 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     if ((const char *)p.phre - (const char *)p.f[0] != fstride * F_PHRE) return BVFDTD_EINVAL;
     if ((const char *)p.phim - (const char *)p.f[0] != fstride * F_PHIM) return BVFDTD_EINVAL;
     const int wxb = L.P > 0 ? std::min(L.xph, CfgV::TX) : 4;
-    if (int rc = encode_maps<CfgV>(enc, plan.mv, L, p, psi_base, psi_stride, wxb)) return rc;
+    if (int rc = encode_maps<CfgV>(enc, plan.mv, L, p, psi_base, psi_stride, wxb, tune.l2_promotion)) return rc;
 
     const int bar_bytes = 2 * MAX_STAGES * 8;
     int dev = 0, sms = 148, smem_max = 227 * 1024;
@@ -1383,8 +1390,8 @@ inline int tiled_plan_create(TiledPlan &plan, Layout &L, Params &p, char *const 
     L.ntxS = (L.nx + CfgS::TX - 1) / CfgS::TX;
     L.ntyS = (L.ny + sty - 1) / sty;
     p.ntxS = L.ntxS; p.ntyS = L.ntyS;
-    if (int rc = plan.s16 ? encode_maps<CfgS>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)
-                          : encode_maps<CfgS8>(enc, plan.ms, L, p, psi_base, psi_stride, wxb)) return rc;
+    if (int rc = plan.s16 ? encode_maps<CfgS>(enc, plan.ms, L, p, psi_base, psi_stride, wxb, tune.l2_promotion)
+                          : encode_maps<CfgS8>(enc, plan.ms, L, p, psi_base, psi_stride, wxb, tune.l2_promotion)) return rc;
     int occ_v = 1, occ_s = 1;
     const bool trim_v = plan.sv.spw > 0 || plan.sv.nrho > 0;
     if (plan.occ_v == 3 && trim_v) {

@@ -171,6 +171,8 @@ def split_ranges(nz_local, lo, hi):
     be swept for the pass to complete."""
     i0 = lo + HALO if lo else 0
     i1 = nz_local - hi - HALO if hi else nz_local
+    if i1 <= i0:                       # a slab too thin to have such planes: everything runs after the exchange
+        return (0, 0), [(0, nz_local)]
     boundary = []
     if i0 > 0:
         boundary.append((0, i0))
@@ -225,8 +227,6 @@ class SlabRank(_Slab):
         self.main.wait_stream(self.side)
         for k0, k1 in self.boundary:
             self.sim.step_phase_planes(phase, k0, k1)
-        if i1 <= i0 and not self.boundary:
-            self.sim.step_phase(phase)
 
     def step(self, n=1):
         for _ in range(int(n)):
