@@ -40,6 +40,7 @@
  */
 #include <math.h>
 #include <stdint.h>
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -607,6 +608,55 @@ int orc_set_field(orc *o, int field, const double *in)
                 o->f[field][AT(o, i, j, k)] = in[DENSE(o, i, j, k)];
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------ */
+/* Checkpoint of the time-dependent state (fields, psi, sensor maps, counters) to a file */
+/* and back: test infrastructure for runs that outlast one job (the full-length runs of  */
+/* configs 3 and 4 take hours).  No arithmetic: a resumed run is bit-identical to an      */
+/* uninterrupted one (tests/test_oracle_pins.py::test_checkpoint_resume_is_bit_identical).*/
+/* The context that loads must have been created with the same arguments.                */
+/* ------------------------------------------------------------------------------------ */
+static int io_block(FILE *fp, void *p, size_t bytes, int write)
+{
+    const size_t chunk = (size_t)1 << 28;
+    char *c = (char *)p;
+    while (bytes) {
+        size_t n = bytes < chunk ? bytes : chunk;
+        size_t done = write ? fwrite(c, 1, n, fp) : fread(c, 1, n, fp);
+        if (done != n) return -1;
+        c += n; bytes -= n;
+    }
+    return 0;
+}
+static int state_io(orc *o, const char *path, int write)
+{
+    FILE *fp = fopen(path, write ? "wb" : "rb");
+    if (!fp) return -1;
+    int64_t hdr[8] = { 0x4f52434b50543031LL, o->n[0], o->n[1], o->n[2], o->P, o->nmat, o->step, o->count };
+    int rc = 0;
+    if (write) rc = io_block(fp, hdr, sizeof(hdr), 1);
+    else {
+        int64_t in[8];
+        rc = io_block(fp, in, sizeof(in), 0);
+        for (int q = 0; q < 6 && !rc; ++q) if (in[q] != hdr[q]) rc = -2;
+        if (!rc) { o->step = in[6]; o->count = in[7]; }
+    }
+    const size_t nc = (size_t)o->n[0] * o->n[1] * o->n[2];
+    for (int q = 0; q < NFIELD && !rc; ++q) rc = io_block(fp, o->f[q], sizeof(double) * padded_cells(o), write);
+    for (int a = 0; a < 3 && !rc; ++a)
+        for (int t = 0; t < 6 && !rc; ++t) {
+            size_t pc = psi_cells(o, a);
+            if (pc) rc = io_block(fp, o->psi[a * 6 + t], sizeof(double) * pc, write);
+        }
+    if (!rc) rc = io_block(fp, o->peak, sizeof(double) * nc, write);
+    if (!rc) rc = io_block(fp, o->sumsq, sizeof(double) * nc, write);
+    if (!rc && o->phre) rc = io_block(fp, o->phre, sizeof(double) * nc, write);
+    if (!rc && o->phim) rc = io_block(fp, o->phim, sizeof(double) * nc, write);
+    if (fclose(fp)) rc = rc ? rc : -3;
+    return rc;
+}
+int orc_save_state(orc *o, const char *path) { return state_io(o, path, 1); }
+int orc_load_state(orc *o, const char *path) { return state_io(o, path, 0); }
 
 /* values of one field (0..15) at a list of dense cell indices (cheap probes for traces) */
 int orc_probe(const orc *o, int field, int64_t ncell, const int64_t *cell, double *out)

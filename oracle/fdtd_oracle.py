@@ -52,6 +52,8 @@ def lib():
         L.orc_set_source.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, dp, dp, C.c_int,
                                      C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_save_state.argtypes = [C.c_void_p, C.c_char_p]
+        L.orc_load_state.argtypes = [C.c_void_p, C.c_char_p]
         for fn in ("orc_inject", "orc_velocity_pass", "orc_stress_pass", "orc_sensor"):
             getattr(L, fn).argtypes = [C.c_void_p]
         L.orc_step_index.restype = C.c_int64
@@ -150,6 +152,16 @@ class Oracle:
 
     def step(self, n=1):
         lib().orc_step(self._h, int(n))
+
+    def save_state(self, path):
+        """checkpoint of the time-dependent state (fields, psi, sensor maps, counters); no arithmetic"""
+        if lib().orc_save_state(self._h, os.fsencode(path)):
+            raise OSError(f"could not write {path}")
+
+    def load_state(self, path):
+        """resume from a checkpoint written by an oracle created with the same arguments"""
+        if lib().orc_load_state(self._h, os.fsencode(path)):
+            raise OSError(f"could not read {path} (or it belongs to another grid)")
 
     def inject(self):
         lib().orc_inject(self._h)

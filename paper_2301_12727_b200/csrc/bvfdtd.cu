@@ -298,7 +298,8 @@ int fused_setup(bvfdtd_ctx *c) {
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_fluid_fused<CfgF>, CfgF::NT, c->fplan.smem));
     const int sty = c->plan.s16 ? CfgS::TY : CfgS8::TY;
     const FusedLists lists = fused_lists(L, cls, sty, sms * std::max(1, occ_f), sms * std::max(1, c->plan.occ_v_res),
-                                         sms * std::max(1, c->plan.occ_s_res), (int)((c->opts.tuning >> 8) & 0xffu));
+                                         sms * std::max(1, c->plan.occ_s_res), (int)((c->opts.tuning >> 8) & 0xffu),
+                                         (int)((c->opts.tuning >> 18) & 0xffu));
     const long long planes_all = (long long)L.ntxV * L.ntyV * L.nz;
     c->fplan.planes_f = lists.planes_f;
     c->fplan.planes_all = planes_all;
@@ -422,7 +423,7 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
     if (!grid_ok(grid) || !table || !index_map || !opts || !d_workspace) return BVFDTD_EINVAL;
     if (!(dx > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dt)) return BVFDTD_EINVAL;
     constexpr uint32_t TUNE_ALL = BVFDTD_TUNE_VEL_2CTA | BVFDTD_TUNE_VEL_3CTA | BVFDTD_TUNE_STRESS_8 | BVFDTD_TUNE_STRESS_16 |
-                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED | BVFDTD_TUNE_FUSED | 0x3ff00u;   // + the two experiment fields
+                                  BVFDTD_TUNE_NO_GRAPH | BVFDTD_TUNE_NO_FUSED | BVFDTD_TUNE_FUSED | 0x3ffff00u;   // + the three experiment fields
     if (!(opts->f0 > 0.0) || (opts->tuning & ~TUNE_ALL) != 0) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_VEL_2CTA) && (opts->tuning & BVFDTD_TUNE_VEL_3CTA)) return BVFDTD_EINVAL;
     if ((opts->tuning & BVFDTD_TUNE_STRESS_8) && (opts->tuning & BVFDTD_TUNE_STRESS_16)) return BVFDTD_EINVAL;

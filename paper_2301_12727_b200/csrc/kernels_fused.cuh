@@ -479,7 +479,7 @@ struct FusedLists {
 // cls: one byte per (64 x 8 tile, plane) from k_fused_class.  sty = rows of a stress tile (8 or 16): a stress
 // tile of 16 rows is fused only as a whole.  slots_* = resident CTAs of the device for each kernel.
 inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, int sty, int slots_f, int slots_v, int slots_s,
-                              int fused_chunk = 0) {
+                              int fused_chunk = 0, int pass_chunk = 0) {
     FusedLists out;
     const int ntx = L.ntxV, nty = L.ntyV, nz = L.nz, P = L.P, TX = CfgF::TX, TY = CfgF::TY;
     const int LMIN = 16;
@@ -591,7 +591,8 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
             k0 = k1;
         }
     };
-    const int len_f = fused_chunk > 0 ? fused_chunk : wave_len(rf, slots_f, 24, 128), len_v = wave_len(rv, slots_v, 16, 96), len_s = wave_len(rs, slots_s, 16, 96);
+    const int len_f = fused_chunk > 0 ? fused_chunk : 16;
+    const int len_v = pass_chunk > 0 ? pass_chunk : wave_len(rv, slots_v, 16, 96), len_s = pass_chunk > 0 ? pass_chunk : wave_len(rs, slots_s, 16, 96);
     for (const Run &r : rf) split(out.f, r.bx, r.by, r.a, r.b, len_f, true);
     for (const Run &r : rv) split(out.v, r.bx, r.by, r.a, r.b, len_v, false);
     for (const Run &r : rs) split(out.s, r.bx, r.by, r.a, r.b, len_s, false);

@@ -766,3 +766,30 @@ def test_T8_cyclic_axis_symmetry():
         a2 = o2.get(new)
         assert np.abs(a1).max() > 0
         assert np.abs(a1 - a2).max() <= 1e-13 * np.abs(a1).max(), (name, new)
+
+
+def test_checkpoint_resume_is_bit_identical(tmp_path):
+    """orc_save_state / orc_load_state (test infrastructure for runs that outlast one job): a run resumed from a
+    checkpoint in a FRESH oracle equals the uninterrupted run bit for bit, on every field, psi included (the
+    PML is on and the wave has reached it), with the sensors and their counters"""
+    from paper_2301_12727_b200 import workloads as wl
+    w = wl.random_domain(30, 26, 28, 5, seed=12, steps=40, waveform=1)
+    w.rms_begin = 9
+    a = fo.Oracle.from_workload(w)
+    a.step(40)
+    b = fo.Oracle.from_workload(w)
+    b.step(17)
+    b.save_state(str(tmp_path / "ckpt.bin"))
+    b.close()
+    c = fo.Oracle.from_workload(w)
+    c.load_state(str(tmp_path / "ckpt.bin"))
+    assert c.step_index == 17
+    c.step(23)
+    assert c.step_index == 40 and c.rms_count == a.rms_count == 31
+    for n in fo.FIELDS + ("p", "peak", "rms_amp", "sumsq"):
+        x, y = a.get(n), c.get(n)
+        assert np.abs(x).max() > 0 or n.startswith("r") or n in ("sxy", "sxz", "syz")
+        assert np.array_equal(x, y), n
+    other = fo.Oracle.from_workload(wl.random_domain(30, 26, 29, 5, seed=12, steps=4))
+    with pytest.raises(OSError):
+        other.load_state(str(tmp_path / "ckpt.bin"))          # another grid
