@@ -567,14 +567,15 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
                 a = b;
             }
         }
-    // chunk length of a kind: about three rounds of the resident CTAs.  (Choosing the length that minimises
-    // rounds x (planes + priming planes) in a model of equal items -- 2 rounds of 90 planes instead of 3.5 of 50 on
-    // config 2 -- measured 2-8 % slower: the passes are limited by memory-level parallelism, not by the round count.)
-    auto wave_len = [&](const std::vector<Run> &runs, int slots, int lo, int hi) {
-        long long planes = 0;
-        for (const Run &r : runs) planes += r.b - r.a;
-        return (int)std::max<long long>(lo, std::min<long long>(hi, planes / std::max(1, 3 * slots)));
-    };
+    // Chunk lengths: SHORT chunks win, although a chunk costs 6 (fused) or 4 (two passes) priming planes: the CTAs of
+    // one z range start together and stay within a few planes of each other, so the halo rows and columns a
+    // neighbour needs are still in L2 (126 MB hold about 25 us of traffic), and many small items balance the last
+    // round.  Measured (20-step bench, both sensors on; profiles/r2_fused.md): fused sweep on config 2 with chunks
+    // of 50 / 24 / 16 / 12 planes 0.446 / 0.407 / 0.388 / 0.385 ms, on config 3 with 128 / 32 / 16: 1.65 / 1.50 / 1.29
+    // ms; two-pass lists on config 4 with 66-96 / 32 / 16 / 12 planes: stress 0.84 / 0.75 / 0.70 / 0.70 ms.
+    // (Choosing the length that minimises rounds x (planes + priming planes) in a model of equal items -- 2 rounds of
+    // 90 planes on config 2 -- measured 2-8 % slower.)
+    (void)slots_f; (void)slots_v; (void)slots_s;
     // [a, b) in about equal chunks of at most `len` planes; with `fused` no chunk boundary falls inside, or within
     // two planes of, a z slab (a fused chunk recomputes vz at kz0-2, kz0-1 and kz1 without their psi)
     auto split = [&](std::vector<int4> &dst, int bx, int by, int a, int b, int len, bool fused) {
@@ -591,8 +592,7 @@ inline FusedLists fused_lists(const Layout &L, const std::vector<uint8_t> &cls, 
             k0 = k1;
         }
     };
-    const int len_f = fused_chunk > 0 ? fused_chunk : 16;
-    const int len_v = pass_chunk > 0 ? pass_chunk : wave_len(rv, slots_v, 16, 96), len_s = pass_chunk > 0 ? pass_chunk : wave_len(rs, slots_s, 16, 96);
+    const int len_f = fused_chunk > 0 ? fused_chunk : 16, len_v = pass_chunk > 0 ? pass_chunk : 12, len_s = len_v;
     for (const Run &r : rf) split(out.f, r.bx, r.by, r.a, r.b, len_f, true);
     for (const Run &r : rv) split(out.v, r.bx, r.by, r.a, r.b, len_v, false);
     for (const Run &r : rs) split(out.s, r.bx, r.by, r.a, r.b, len_s, false);
