@@ -403,7 +403,7 @@ def next_rows(dev):
         bv._check(bv.lib().bvfdtd_rayleigh(s.shape[0], s.data_ptr(), wg.data_ptr(), r.shape[0], r.data_ptr(), f, c0, rho0,
                                            out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(), out[3].data_ptr(),
                                            stream), "bvfdtd_rayleigh")
-    for _ in range(3):
+    for _ in range(40):                 # (the GPU idled through the CPU baseline: let the clocks come back up)
         launch()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
