@@ -628,10 +628,27 @@ static int io_block(FILE *fp, void *p, size_t bytes, int write)
     }
     return 0;
 }
+/* first touch of a freshly calloc'ed array by the threads that will sweep it (static schedule over contiguous
+ * slabs, like the loop nests of the step): without it a resumed run has every page placed by the one thread
+ * that reads the file */
+static void touch_parallel(double *a, size_t n)
+{
+    const long long blocks = (long long)((n + 511) / 512);
+#pragma omp parallel for schedule(static)
+    for (long long b = 0; b < blocks; ++b) a[(size_t)b * 512] = 0.0;
+}
 static int state_io(orc *o, const char *path, int write)
 {
     FILE *fp = fopen(path, write ? "wb" : "rb");
     if (!fp) return -1;
+    if (!write) {
+        const size_t ncell = (size_t)o->n[0] * o->n[1] * o->n[2];
+        if (o->step == 0) {
+            for (int q = 0; q < NFIELD; ++q) touch_parallel(o->f[q], padded_cells(o));
+            touch_parallel(o->peak, ncell);
+            touch_parallel(o->sumsq, ncell);
+        }
+    }
     int64_t hdr[8] = { 0x4f52434b50543031LL, o->n[0], o->n[1], o->n[2], o->P, o->nmat, o->step, o->count };
     int rc = 0;
     if (write) rc = io_block(fp, hdr, sizeof(hdr), 1);
