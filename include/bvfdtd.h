@@ -329,6 +329,26 @@ int bvfdtd_energy_loss(const double *sum_tissue, const double *sum_water, const 
  *   cuda_stream the launch is asynchronous on this stream
  * fp32 arithmetic, one thread per receiver; no context is needed.
  */
+/*
+ * The same field as bvfdtd_rayleigh for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): this entry point allocates NOTHING -- no cudaMalloc / cudaMallocAsync,
+ * no cudaFree, no allocating library routine.  bvfdtd_rayleigh packs the sources into a scratch array it allocates
+ * per call; here that scratch is a static device array of the library, BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC float4
+ * entries (1 MiB), which every GPU that loads the library holds until the process exits.
+ *   - arguments, layouts and results as bvfdtd_rayleigh (same field kernel, same bits);
+ *   - n_src > BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC returns BVFDTD_ENOMEM (bvfdtd_last_cuda_error names the limit): use
+ *     bvfdtd_rayleigh for larger source sets;
+ *   - all calls on one device SHARE the scratch, which keeps the last call's contents: every entry a call reads is
+ *     rewritten by that call first (nothing needs to start at zero), but two calls that overlap on the GPU --
+ *     different streams, or threads, without an ordering between them -- race on it.  Calls on one stream are safe;
+ *   - the first call on each device resolves the scratch's device address (cudaGetSymbolAddress, cached per device;
+ *     not an allocation): make that call once before starting a graph capture.
+ * Asynchronous on cuda_stream.
+ */
+enum { BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC = 65536 };
+int bvfdtd_rayleigh_noalloc(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv,
+                            const float *rcv_xyz, double f, double c0, double rho0, float *p_re, float *p_im,
+                            float *amp, float *delay_s, void *cuda_stream);
 /* Measured MUFU (special-function unit) rate of the current device in operations per second: a short probe
  * kernel of independent sin.approx chains, timed with CUDA events.  bvfdtd_rayleigh spends three MUFU operations
  * per (source, receiver) pair, so its roofline is this rate / 3.  Synchronises. */

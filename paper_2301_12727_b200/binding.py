@@ -38,7 +38,7 @@ SYMBOLS = (
     "bvfdtd_read_peak_pressure", "bvfdtd_destroy", "bvfdtd_strerror", "bvfdtd_last_cuda_error",
     "bvfdtd_enable_kernel_timing", "bvfdtd_kernel_times", "bvfdtd_derive_materials",
     "bvfdtd_pml_profiles", "bvfdtd_pml_mask", "bvfdtd_max_courant",
-    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_probe_mufu", "bvfdtd_read_phasor",
+    "bvfdtd_plane_intensity", "bvfdtd_energy_loss", "bvfdtd_rayleigh", "bvfdtd_rayleigh_noalloc", "bvfdtd_probe_mufu", "bvfdtd_read_phasor",
     "bvfdtd_bhte_workspace_bytes", "bvfdtd_bhte_create", "bvfdtd_bhte_set_heat",
     "bvfdtd_bhte_set_temperature", "bvfdtd_bhte_step", "bvfdtd_bhte_read", "bvfdtd_bhte_destroy",
     "bvfdtd_heat_source", "bvfdtd_step_phase", "bvfdtd_step_phase_planes", "bvfdtd_plane_span",
@@ -72,7 +72,7 @@ class BvfdtdError(RuntimeError):
     def __init__(self, code, where):
         self.code = code
         msg = lib().bvfdtd_strerror(code).decode()
-        if code == ECUDA:
+        if code == ECUDA or (code == ENOMEM and where == "bvfdtd_rayleigh_noalloc"):
             msg += ": " + lib().bvfdtd_last_cuda_error().decode()
         super().__init__(f"{where}: {msg} ({code})")
 
@@ -120,6 +120,7 @@ def lib():
         L.bvfdtd_plane_intensity.argtypes = [vp, vp, vp]
         L.bvfdtd_read_phasor.argtypes = [vp, vp, vp, i32]
         L.bvfdtd_rayleigh.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
+        L.bvfdtd_rayleigh_noalloc.argtypes = [i64, vp, vp, i64, vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
         L.bvfdtd_probe_mufu.argtypes = [C.POINTER(dbl), vp]
         L.bvfdtd_energy_loss.argtypes = [vp, vp, vp, i32, i32, C.POINTER(i32), C.POINTER(dbl), C.POINTER(dbl)]
         L.bvfdtd_max_courant.restype = dbl
@@ -246,6 +247,29 @@ def rayleigh(src_xyz, src_weight, rcv_xyz, f, c0=1500.0, rho0=1000.0, device="cu
     o = out.cpu().numpy()
     p = o[0].astype(np.complex64) + 1j * o[1].astype(np.complex64)
     return (p, o[2], o[3]) if want_source else p
+
+
+RAYLEIGH_NOALLOC_MAX_SRC = 65536
+
+
+def rayleigh_noalloc(src_xyz, src_weight, rcv_xyz, f, c0=1500.0, rho0=1000.0, device="cuda:0"):
+    """``bvfdtd_rayleigh_noalloc``: the field of ``rayleigh`` through the entry point that allocates nothing on the
+    device (static scratch of RAYLEIGH_NOALLOC_MAX_SRC sources).  Returns (p complex64, amp, delay).  (The torch
+    tensors below are this binding's marshalling of numpy inputs; a caller with device arrays passes its pointers.)"""
+    import torch
+    dev = torch.device(device)
+    s = torch.from_numpy(np.ascontiguousarray(src_xyz, dtype=np.float32)).to(dev)
+    wc = np.ascontiguousarray(src_weight, dtype=np.complex64)
+    w = torch.from_numpy(wc.view(np.float32).reshape(-1, 2).copy()).to(dev)
+    r = torch.from_numpy(np.ascontiguousarray(rcv_xyz, dtype=np.float32)).to(dev)
+    out = torch.empty((4, r.shape[0]), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    _check(lib().bvfdtd_rayleigh_noalloc(s.shape[0], s.data_ptr(), w.data_ptr(), r.shape[0], r.data_ptr(), float(f), float(c0),
+                                         float(rho0), out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(),
+                                         out[3].data_ptr(), stream), "bvfdtd_rayleigh_noalloc")
+    torch.cuda.synchronize(dev)
+    o = out.cpu().numpy()
+    return o[0].astype(np.complex64) + 1j * o[1].astype(np.complex64), o[2], o[3]
 
 
 def probe_mufu(device="cuda:0"):

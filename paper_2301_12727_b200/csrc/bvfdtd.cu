@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -21,6 +22,41 @@
 #include "kernels_rs.cuh"
 
 using namespace bvfdtd;
+
+// ---------------------------------------------------------------------------------------------------
+// Scratch of bvfdtd_rayleigh_noalloc (the entry point for callers that cannot call cudaMalloc): the
+// sources packed as float4 (x, y, z, 0).  A file-scope device array: every GPU that loads the library holds
+// these BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC * 16 bytes = 1 MiB until the process exits.  In HOST code the name
+// below is only a stand-in for the symbol, not a device address: the address each device gives it is
+// resolved once per device, with that device current, by cudaGetSymbolAddress (rs_noalloc_scratch()).
+// ---------------------------------------------------------------------------------------------------
+static __device__ __align__(256) float4 g_rs_noalloc_src[BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC];
+
+// (x, y, z) triples -> float4 (x, y, z, 0) in the scratch: every entry the field kernel will read is written
+// here, .w included, so nothing of an earlier call is seen; entries from n_src on keep old contents, unread
+static __global__ void k_rs_noalloc_pack(const int n_src, const float *__restrict__ src_xyz, float4 *__restrict__ dst) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n_src) dst[q] = make_float4(src_xyz[3 * q], src_xyz[3 * q + 1], src_xyz[3 * q + 2], 0.0f);
+}
+
+// device address of g_rs_noalloc_src on the CURRENT device (resolved on first use per device, then cached)
+static int rs_noalloc_scratch(float4 **out) {
+    enum { MAX_DEVICES = 64 };
+    static std::mutex mu;
+    static float4 *addr[MAX_DEVICES] = {};
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return cuda_fail(cudaErrorInvalidDevice, "bvfdtd_rayleigh_noalloc: device ordinal out of range");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_rs_noalloc_src));
+        if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_rs_noalloc_src) returned null");
+        addr[dev] = (float4 *)p;
+    }
+    *out = addr[dev];
+    return BVFDTD_OK;
+}
 
 namespace {
 thread_local char g_cuda_err[256] = "";
@@ -1125,6 +1161,27 @@ int bvfdtd_rayleigh(int64_t n_src, const float *src_xyz, const float *src_weight
                                                               (float)(rho0 * c0 * k / (2.0 * 3.14159265358979323846)), (float)w, p_re, p_im, amp, delay_s);
     CU(cudaGetLastError());
     CU(cudaFreeAsync(d_src, st));
+    return BVFDTD_OK;
+}
+
+int bvfdtd_rayleigh_noalloc(int64_t n_src, const float *src_xyz, const float *src_weight, int64_t n_rcv, const float *rcv_xyz,
+                            double f, double c0, double rho0, float *p_re, float *p_im, float *amp, float *delay_s, void *cuda_stream) {
+    if (n_src <= 0 || n_rcv <= 0 || n_rcv > (1 << 30) || !src_xyz || !src_weight || !rcv_xyz || !p_re || !p_im) return BVFDTD_EINVAL;
+    if (!(f > 0.0) || !(c0 > 0.0) || !(rho0 > 0.0) || (amp == nullptr) != (delay_s == nullptr)) return BVFDTD_EINVAL;
+    if (n_src > BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC) {
+        std::snprintf(g_cuda_err, sizeof(g_cuda_err), "bvfdtd_rayleigh_noalloc: n_src = %lld exceeds BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC = %d "
+                      "(the static scratch); use bvfdtd_rayleigh", (long long)n_src, (int)BVFDTD_RAYLEIGH_NOALLOC_MAX_SRC);
+        return BVFDTD_ENOMEM;
+    }
+    DeviceScope scope(device_of(p_re));      // the caller's arrays say which device the launch belongs to
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float4 *d_src = nullptr;                 // this device's address of the static scratch: no allocation anywhere
+    if (int rc = rs_noalloc_scratch(&d_src)) return rc;
+    const double w = 2.0 * 3.14159265358979323846 * f, k = w / c0;
+    k_rs_noalloc_pack<<<(unsigned)((n_src + 255) / 256), 256, 0, st>>>((int)n_src, src_xyz, d_src);
+    k_rayleigh<<<(unsigned)((n_rcv + 127) / 128), 128, 0, st>>>((int)n_src, d_src, (const float2 *)src_weight, (int)n_rcv, rcv_xyz, (float)k,
+                                                              (float)(rho0 * c0 * k / (2.0 * 3.14159265358979323846)), (float)w, p_re, p_im, amp, delay_s);
+    CU(cudaGetLastError());
     return BVFDTD_OK;
 }
 
