@@ -545,9 +545,30 @@ void orc_sensor(orc *o)
     if (do_rms) o->count++;
 }
 
+/* Subnormal numbers (reading P9): values below the smallest normal double, 2.2e-308, count as
+ * the zero initial state while orc_step runs (x86 flush-to-zero + denormals-are-zero on the stepping threads, put
+ * back afterwards).  Why: the 4-point stencils carry the discrete solution two cells per step, far ahead of the
+ * physical wave front, where it decays super-exponentially; for most of a long run a large part of the domain holds
+ * values between 5e-324 and 2e-308, every operation on which an x86 core executes in microcode.  Measured on
+ * config 2: 1.1 s per step at step 50, 3.2 s at step 150 (0.9 M subnormal cells per field), 21 minutes for the
+ * 3000 steps instead of 8; configs 3 / 4 up to 30x slower.  The change is below 1e-307 in absolute value, 300 orders
+ * of magnitude under every tolerance, and no pin moves. */
+#if defined(__x86_64__) || defined(__i386__)
+#include <xmmintrin.h>
+#define ORC_MXCSR_FTZ_DAZ 0x8040u
+static void subnormals_as_zero(int on)
+{
+#pragma omp parallel
+    { _mm_setcsr(on ? (_mm_getcsr() | ORC_MXCSR_FTZ_DAZ) : (_mm_getcsr() & ~ORC_MXCSR_FTZ_DAZ)); }
+}
+#else
+static void subnormals_as_zero(int on) { (void)on; }
+#endif
+
 /* one full step: S1 -> S2 -> S3 -> S4 ("Per-step order is S1 -> S2 -> S3(+S4)") */
 void orc_step(orc *o, int64_t nsteps)
 {
+    subnormals_as_zero(1);
     for (int64_t s = 0; s < nsteps; ++s) {
         orc_inject(o);
         orc_velocity_pass(o);
@@ -555,6 +576,7 @@ void orc_step(orc *o, int64_t nsteps)
         orc_sensor(o);
         o->step++;
     }
+    subnormals_as_zero(0);
 }
 
 int64_t orc_step_index(const orc *o) { return o->step; }
