@@ -290,13 +290,16 @@ def test_config1_full(bv):
 
 
 def test_config2_full_size_short_run(bv):
-    """Config 2 at its full 300x300x450 size, in the launch configuration bench.py times: 8 steps
-    from a seeded random state (every cell carries data, so every tile, slab and ragged tail is
-    checked element by element against the oracle) with the focused source on."""
+    """Config 2 at its full 300x300x450 size on the DENSE sweep: 8 steps from a seeded random state of all 15
+    fields (every cell carries data, so every tile, slab and ragged tail is checked element by element against
+    the oracle) with the focused source on.  Writing a shear stress or a memory variable switches the context
+    to the dense sweep, and writing any stress ends the fused mode, so this is NOT the path bench.py times: that
+    one is checked by tests/test_gpu_full_runs.py (zero state / velocity-only state, default path)."""
     w = wl.make(2, steps=8)
     w.rms_begin = 4
     st = wl.random_state(w, 7)
     sim, o = run_both(bv, w, state=st)
+    assert sim.kernel_mode().startswith("tiled, dense sweep")
     compare_state(sim, o, rel=1e-5)
     peak, rms = sim.read_peak_pressure()
     compare_map(peak, o.get("peak"), rel=1e-4)
@@ -308,9 +311,11 @@ def test_config2_full_size_short_run(bv):
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_config34_full_size_short_run(bv, cfg):
     """Configs 3 (504x504x672, P 20, 255 materials) and 4 (480x480x600, P 24, array source) at their
-    full sizes in the default launch configuration (tile-class skipping on): 6 steps from a seeded
-    random velocity / normal-stress state (every cell carries data; shear stresses and memory
-    variables start at zero as in a real run), element by element against the fp64 oracle."""
+    full sizes on the two tiled passes with tile-class skipping: 6 steps from a seeded random velocity /
+    normal-stress state (every cell carries data; shear stresses and memory variables start at zero as in a real
+    run), element by element against the fp64 oracle.  Writing the normal stresses ends the fused mode and the
+    sigma_xx-for-all shortcut of the fluid velocity tiles; the default path with every optimisation on is checked
+    by tests/test_gpu_full_runs.py::test_config34_150_steps_default_path."""
     w = wl.make(cfg, steps=6)
     w.rms_begin = 3
     st = wl.random_state(w, 7 + cfg, fields=("vx", "vy", "vz", "sxx", "syy", "szz"))
