@@ -570,6 +570,29 @@ int bvfdtd_create(bvfdtd_ctx **out, const bvfdtd_grid *grid, double dx, double d
         tune.l2_promotion = (int)((opts->tuning >> 16) & 3u);
         rc = tiled_plan_create(c->plan, c->L, c->prm, psi_base, psi_stride, (opts->flags & BVFDTD_FLAG_DENSE) != 0, tune);
         if (rc) return rc == BVFDTD_ECUDA ? cuda_fail(cudaErrorUnknown, tiled_plan_error()) : rc;
+        {
+            // z chunks of the two passes when they sweep a whole large grid (dense sweep, z-slab contexts, phasor runs,
+            // BVFDTD_TUNE_NO_FUSED): short chunks, the z slabs in chunks of their own -- what the work lists of the
+            // fused mode use and for the same reason (kernels_fused.cuh: CTAs of one z range share their halo rows in
+            // L2).  Experiment field of opts.tuning: planes per chunk; 0 = the plan of tiled_plan_create.
+            const int want = (int)((opts->tuning >> 18) & 0xffu);
+            if (want > 0) {
+                const int nz = c->L.nz, P = c->L.P;
+                const int len = std::max(want, (nz + MAX_CHUNKS - 7) / (MAX_CHUNKS - 6));
+                ZChunks z;
+                int n = 0;
+                z.b[0] = 0;
+                auto add = [&](int a, int b) {
+                    const int m = std::max(1, (b - a + len - 1) / len);
+                    for (int q = 1; q <= m; ++q) z.b[++n] = a + (int)((long long)(b - a) * q / m);
+                };
+                if (P >= 8 && nz - 2 * P >= 16) { add(0, P); add(P, nz - P); add(nz - P, nz); }
+                else add(0, nz);
+                z.n = n;
+                c->plan.zv = z;
+                c->plan.zs = z;
+            }
+        }
         c->dense = (opts->flags & BVFDTD_FLAG_DENSE) != 0;
         tiled_flags(c->plan, c->prm, (uint32_t *)(c->ws + c->W.flagsV), (uint32_t *)(c->ws + c->W.flagsS), c->dense, c->stream);
         CU(cudaGetLastError());
