@@ -1,8 +1,9 @@
 """Full-length parity of configs 3 and 4 on sampled planes, in three steps that need not run on one machine.
 
-The oracle needs about 2.5 hours per configuration for the 5000 / 6000 steps (fp64, 138-171 M cells); a GPU call
-of this build environment is limited to one hour, so `test_gpu_full_runs.py::test_config34_full_length` cannot
-finish there.  The tier's rule for full sizes is "on sampled outputs the oracle can compute": the comparison runs on
+The oracle needs about an hour per configuration for the 5000 / 6000 steps (fp64, 171-173 M cells, 16 cores) and a
+GPU call of this build environment is limited to one hour: `test_gpu_full_runs.py::test_config34_full_length`
+checkpoints and resumes the oracle across calls; this script is the other way round it -- the oracle leg can run
+anywhere, without a GPU.  The tier's rule for full sizes is "on sampled outputs the oracle can compute": the comparison runs on
 whole planes of every field.
 
     python tests/full_length_sampled.py oracle  CFG OUT.npz     # CPU only: calls nothing but oracle/ and the inputs

@@ -10,7 +10,7 @@ r_xx-only in lossy fluid) -- nothing is written through
   * configs 3 and 4, 150 steps with the source on, from a seeded random velocity field (so every tile,
     slab and material class carries data from the first step).
   * configs 3 and 4 at their full 5000 / 6000 steps: only when BVFDTD_FULL_RUNS lists them (the oracle needs
-    about 2.5 hours each on 16 cores; with BVFDTD_ORACLE_BUDGET_S it checkpoints and resumes across calls); the
+    about an hour each on 16 cores; with BVFDTD_ORACLE_BUDGET_S it checkpoints and resumes across calls); the
     numbers go to gpurun_out/full_run_cfg<N>.json and into BASELINE.md section 4.
 
 The oracle's outputs are cached as fp32 under $BVFDTD_ORACLE_CACHE (default /tmp/bvfdtd_oracle_cache)
@@ -69,7 +69,7 @@ class OracleResult:
     BVFDTD_ORACLE_BUDGET_S set, a run that does not finish within the budget checkpoints the oracle's state next to
     the cache file (orc_save_state: no arithmetic, a resumed run is bit-identical) and raises OracleCheckpointed; the
     next call resumes it -- a GPU job of this build environment is limited to one hour, the full-length runs of
-    configs 3 and 4 need about 2.5 hours of oracle time."""
+    configs 3 and 4 need about an hour of oracle time each."""
 
     def __init__(self, w, steps, state=None):
         self.path = os.path.join(CACHE, f"{w.name}_{_key(w, steps, state)}.npz")
@@ -303,6 +303,6 @@ FULL = [int(c) for c in os.environ.get("BVFDTD_FULL_RUNS", "").replace(",", " ")
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_config34_full_length(bv, cfg):
     if cfg not in FULL:
-        pytest.skip("set BVFDTD_FULL_RUNS=3,4 (the oracle needs about 2.5 hours per configuration)")
+        pytest.skip("set BVFDTD_FULL_RUNS=3,4 (the oracle needs about an hour per configuration)")
     w = wl.make(cfg)
     _run_and_compare(bv, w, w.steps, tag=f"cfg{cfg}")
