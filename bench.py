@@ -578,8 +578,12 @@ def ours(args):
     alg = {"fused": (33.0 + 8.0 * lossy_fluid_frac + 8.0 + 8.0 * rms_frac + 16.0 * bits) * cells_f,
            "velocity": (49.0 + 24.0 * bits) * cells_2,
            "stress_sensor": (109.0 + 8.0 + 8.0 * rms_frac + 24.0 * bits) * cells_2}
-    traffic, traffic_source = ({}, "dense / per-cell kernels: B_dense is what moves") if (args.dense or args.reference_kernels) \
-        else ncu_traffic(args.config)
+    if args.dense or args.reference_kernels:
+        traffic, traffic_source = {}, "dense / per-cell kernels: B_dense is what moves"
+    elif args.tuning:
+        traffic, traffic_source = {}, "experiment (--tuning): the committed capture describes the default launch plan, not used"
+    else:
+        traffic, traffic_source = ncu_traffic(args.config)
     kern = {}
     for name in ("fused", "velocity", "stress_sensor"):
         n = kt[name]["launches"]
